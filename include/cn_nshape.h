@@ -1,0 +1,130 @@
+/*
+ * cn_nshape.h -- C ABI of the B200-native N-shaped partition Crank-Nicolson stepper.
+ *
+ * The library advances the 1-D time-dependent Schroedinger equation by the Crank-Nicolson
+ * propagator
+ *        T psi(t+dt) = T^dagger psi(t),     T = 1 + (i dt / 2) H              PAPER.md:48-52 (Eq. 2)
+ * i.e. per step the explicit half-step d = T^dagger psi (Eq. 3) followed by the
+ * implicit half-step T psi' = d (Eq. 4), a complex tridiagonal system
+ *        b_i psi_{i-1} + a_i psi_i + c_i psi_{i+1} = d_i,  psi_0 = psi_{N+1} = 0   PAPER.md:80-84 (Eq. 5)
+ * which is solved by the N-shaped partition method of PAPER.md:78-149 (section 4) and Appendix I
+ * (PAPER.md:298-337): the N unknowns are split into P contiguous blocks, every block eliminates
+ * locally (stages RD, RU), adds its contributions to its joint lines (JD, JU), a reduced system
+ * on the joint lines is solved (RS) and every block substitutes the two support values (SS).
+ *
+ * Conventions:
+ *   H = -1/2 d^2/dx^2 + V(x) in atomic units, 3-point stencil, Dirichlet ends:
+ *       (H psi)_j = -(psi_{j-1} - 2 psi_j + psi_{j+1}) / (2 dx^2) + V_j psi_j
+ *   so  b = c = -i s,  a_j = 1 + i (2 s + dt V_j / 2),  s = dt / (4 dx^2).   V is real.
+ *   Block w (w = 0..P-1) owns rows [floor(w N / P), floor((w+1) N / P)); its LAST row is the joint
+ *   line J_w; a virtual joint line "row -1, psi = 0" closes the first block (PAPER.md:92 fixes only
+ *   J_0 = first row, J_P = last row and allows unequal blocks).
+ *   psi is N interleaved complex128 values (re, im), 16-byte aligned, updated IN PLACE.
+ *
+ * All functions return a cn_status and never throw.  Pointers are labelled HOST or DEVICE.  No
+ * function allocates inside cn_step / cn_batched_sweep.  All work is enqueued on the given CUDA
+ * stream (a cudaStream_t passed as void*; NULL = the legacy default stream) and, unless stated,
+ * does not synchronise.  There is NO CPU fallback: without a CUDA device every call that needs one
+ * returns CN_ECUDA.
+ */
+#ifndef CN_NSHAPE_H
+#define CN_NSHAPE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cn_plan cn_plan; /* opaque, owned by the library */
+
+typedef enum {
+    CN_OK = 0,
+    CN_EINVAL = 1,         /* bad argument (N < 2, P < 1, P > N, dx <= 0, non-finite dx/dt, dt == 0, NULL, misaligned) */
+    CN_ENOMEM = 2,         /* host or device allocation failed / device budget too small */
+    CN_ECUDA = 3,          /* a CUDA call failed; see cn_last_cuda_error */
+    CN_ENOTFACTORIZED = 4, /* cn_step / cn_batched_sweep before cn_factorize */
+    CN_EBREAKDOWN = 5      /* zero or non-finite pivot met by cn_factorize */
+} cn_status;
+
+/* Options for cn_plan_set_option (all optional; call before cn_factorize). */
+typedef enum {
+    CN_OPT_PATH = 1,        /* 0 = auto (default), 1 = force the generic thread-per-block kernels,
+                               2 = force the tiled TMA kernels (CN_EINVAL at factorize if the shape does not fit) */
+    CN_OPT_TILE_THREADS = 2,/* threads per CTA of the tiled kernels: 0 = auto, else 64/128/256/512 (8 points per thread) */
+    CN_OPT_RS_THREADS = 3,  /* threads of the single-CTA reduced-system kernel (32..1024, power of two) */
+    CN_OPT_USE_GRAPH = 4,   /* 1 = replay the per-step launches from a CUDA graph inside cn_step (default 0) */
+    CN_OPT_RS_LEVELS = 5    /* 0 = auto, 1 = single-CTA RS, 2 = two-level (nested, Eq. 6) RS */
+} cn_option;
+
+typedef struct {
+    int64_t N, P;
+    int32_t path;            /* 1 generic, 2 tiled */
+    int32_t tile_threads;    /* threads per CTA of the pass kernel (tiled path) */
+    int64_t tile_points;     /* points per CTA (tiled path) */
+    int32_t rs_levels;
+    int32_t out_of_core;     /* 1 if a device budget forces host streaming */
+    size_t device_bytes;     /* device memory owned by the plan */
+    int64_t launches;        /* kernels launched by this plan so far (all entry points) */
+    double bytes_per_point_step; /* algorithmic HBM bytes per point per fused step of the chosen path */
+} cn_plan_info;
+
+/*
+ * cn_plan_create -- describe one Hamiltonian / time step.
+ *   out : HOST, receives the plan.            N : number of grid points (rows of T), N >= 2.
+ *   P   : number of blocks n_bl, 1 <= P <= N.  Blocks need not be equal.
+ *   dx, dt : grid spacing (> 0) and time step (!= 0, negative = backward propagation).
+ *   V   : N real potential values, HOST or DEVICE pointer (detected); copied, caller keeps ownership.
+ * Allocates nothing on the device yet except the copy of V.
+ */
+cn_status cn_plan_create(cn_plan **out, int64_t N, int64_t P, double dx, double dt, const double *V);
+
+/* Cap the device memory the library may own for this plan (config "out-of-core", PAPER.md:94, 161-165:
+ * "neither the matrix nor the wavefunction ever need to be placed entirely on a single process").
+ * When the factors do not fit, cn_step expects psi in PINNED HOST memory and streams partitions
+ * H2D / solve / D2H; factors are recomputed per chunk.  bytes = 0 removes the cap. */
+cn_status cn_plan_set_device_budget(cn_plan *plan, size_t bytes);
+
+cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t value);
+
+/*
+ * cn_factorize -- everything that does not depend on d, once per (H, dt) (section 5.2.4:
+ * "storage of a column of the values of r_i factors"; precomputed 1/a_i).
+ * Stores per point the inverse pivot of the block-local downward elimination (RD) and the real
+ * diagonal term of T^dagger, per joint line the factored reduced matrix (RS).  Synchronises `stream`
+ * once at the end to report CN_EBREAKDOWN.
+ */
+cn_status cn_factorize(cn_plan *plan, void *stream);
+
+/*
+ * cn_step -- nsteps Crank-Nicolson steps of one system, in place.
+ *   psi : N complex128.  DEVICE pointer normally; PINNED HOST pointer when the plan is out-of-core.
+ * Stages per step: RHS product fused into RD, RU, JD/JU into two slots per joint
+ * line, RS, SS fused with the psi write and with RHS+RD/RU of the next step
+ * (PAPER.md:27, 201).  Asynchronous on `stream` (the out-of-core mode uses internal streams and
+ * returns after the last copy is enqueued; synchronise `stream` to wait).
+ */
+cn_status cn_step(cn_plan *plan, void *psi, int64_t nsteps, void *stream);
+
+/*
+ * cn_batched_sweep -- the same step for nsys independent systems that share the plan's matrix
+ * (operator splitting; config C4).  System k, row j lives at
+ * psi[k * sys_stride + j * elem_stride] (strides in complex elements).  Supported layouts:
+ * elem_stride == 1 (x-sweep, rows contiguous) and sys_stride == 1 (y-sweep, systems interleaved).
+ */
+cn_status cn_batched_sweep(cn_plan *plan, void *psi, int64_t nsys, int64_t elem_stride, int64_t sys_stride,
+                           int64_t nsteps, void *stream);
+
+cn_status cn_destroy(cn_plan *plan);
+
+cn_status cn_plan_get_info(const cn_plan *plan, cn_plan_info *info);
+const char *cn_status_string(cn_status s);
+/* last CUDA runtime error code seen by this plan (0 = cudaSuccess) */
+cn_status cn_last_cuda_error(const cn_plan *plan, int *cuda_err);
+const char *cn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CN_NSHAPE_H */

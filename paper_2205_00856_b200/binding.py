@@ -1,0 +1,199 @@
+"""Thin ctypes binding of include/cn_nshape.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of libcn_nshape.so.  There is no CPU fallback and this
+module never imports `oracle/`: if the shared library is missing or no CUDA device is present the calls
+fail loudly.  PyTorch is used by callers only to hold device memory and streams; this module accepts
+torch tensors (their data_ptr), numpy arrays (host pointers) or raw integer addresses.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(PKG, "libcn_nshape.so")
+
+CN_OK, CN_EINVAL, CN_ENOMEM, CN_ECUDA, CN_ENOTFACTORIZED, CN_EBREAKDOWN = range(6)
+CN_OPT_PATH, CN_OPT_TILE_THREADS, CN_OPT_RS_THREADS, CN_OPT_USE_GRAPH, CN_OPT_RS_LEVELS = 1, 2, 3, 4, 5
+PATH_AUTO, PATH_GENERIC, PATH_TILED = 0, 1, 2
+
+EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", "cn_factorize", "cn_step",
+           "cn_batched_sweep", "cn_destroy", "cn_plan_get_info", "cn_status_string", "cn_last_cuda_error",
+           "cn_version"]
+
+
+class CnError(RuntimeError):
+    def __init__(self, status: int, where: str, cuda_err: int = 0):
+        self.status = status
+        self.cuda_err = cuda_err
+        msg = lib().cn_status_string(status).decode()
+        super().__init__("%s failed: %s%s" % (where, msg, (" [cudaError %d]" % cuda_err) if cuda_err else ""))
+
+
+class cn_plan_info(ctypes.Structure):
+    _fields_ = [("N", ctypes.c_int64), ("P", ctypes.c_int64), ("path", ctypes.c_int32),
+                ("tile_threads", ctypes.c_int32), ("tile_points", ctypes.c_int64), ("rs_levels", ctypes.c_int32),
+                ("out_of_core", ctypes.c_int32), ("device_bytes", ctypes.c_size_t), ("launches", ctypes.c_int64),
+                ("bytes_per_point_step", ctypes.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libcn_nshape.so (built in-tree by build.py / __graft_entry__.build()).  No fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libcn_nshape.so is missing: run `python -m paper_2205_00856_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64, dbl, sz, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_size_t, ctypes.c_int
+        L.cn_plan_create.restype = i32
+        L.cn_plan_create.argtypes = [ctypes.POINTER(vp), i64, i64, dbl, dbl, vp]
+        L.cn_plan_set_device_budget.restype = i32
+        L.cn_plan_set_device_budget.argtypes = [vp, sz]
+        L.cn_plan_set_option.restype = i32
+        L.cn_plan_set_option.argtypes = [vp, i32, i64]
+        L.cn_factorize.restype = i32
+        L.cn_factorize.argtypes = [vp, vp]
+        L.cn_step.restype = i32
+        L.cn_step.argtypes = [vp, vp, i64, vp]
+        L.cn_batched_sweep.restype = i32
+        L.cn_batched_sweep.argtypes = [vp, vp, i64, i64, i64, i64, vp]
+        L.cn_destroy.restype = i32
+        L.cn_destroy.argtypes = [vp]
+        L.cn_plan_get_info.restype = i32
+        L.cn_plan_get_info.argtypes = [vp, ctypes.POINTER(cn_plan_info)]
+        L.cn_status_string.restype = ctypes.c_char_p
+        L.cn_status_string.argtypes = [i32]
+        L.cn_last_cuda_error.restype = i32
+        L.cn_last_cuda_error.argtypes = [vp, ctypes.POINTER(i32)]
+        L.cn_version.restype = ctypes.c_char_p
+        L.cn_version.argtypes = []
+        _lib = L
+    return _lib
+
+
+def _ptr(x) -> int:
+    """Address of a torch tensor / numpy array / int."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return int(x.data_ptr())
+    if hasattr(x, "ctypes"):
+        return int(x.ctypes.data)
+    raise TypeError("expected a torch tensor, a numpy array or an integer address, got %r" % type(x))
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        import torch
+        return int(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return stream
+    return int(stream.cuda_stream)
+
+
+def _check(plan, st: int, where: str):
+    if st != CN_OK:
+        err = ctypes.c_int(0)
+        if plan:
+            lib().cn_last_cuda_error(plan, ctypes.byref(err))
+        raise CnError(st, where, err.value)
+
+
+# ---- the C-ABI, same names ------------------------------------------------------------------------------
+def cn_plan_create(N: int, P: int, dx: float, dt: float, V):
+    """V: N float64 values, numpy (host) or torch CUDA tensor (device); copied by the library."""
+    if hasattr(V, "dtype"):
+        assert str(V.dtype).endswith("float64"), "V must be float64"
+    h = ctypes.c_void_p()
+    st = lib().cn_plan_create(ctypes.byref(h), N, P, dx, dt, _ptr(V))
+    _check(None, st, "cn_plan_create")
+    return h
+
+
+def cn_plan_set_device_budget(plan, nbytes: int):
+    _check(plan, lib().cn_plan_set_device_budget(plan, nbytes), "cn_plan_set_device_budget")
+
+
+def cn_plan_set_option(plan, key: int, value: int):
+    _check(plan, lib().cn_plan_set_option(plan, key, value), "cn_plan_set_option")
+
+
+def cn_factorize(plan, stream=None):
+    _check(plan, lib().cn_factorize(plan, _stream(stream)), "cn_factorize")
+
+
+def cn_step(plan, psi, nsteps: int = 1, stream=None):
+    """psi: N complex128, torch CUDA tensor (or pinned host tensor in out-of-core mode); updated in place."""
+    _check(plan, lib().cn_step(plan, _ptr(psi), nsteps, _stream(stream)), "cn_step")
+
+
+def cn_batched_sweep(plan, psi, nsys: int, elem_stride: int, sys_stride: int, nsteps: int = 1, stream=None):
+    _check(plan, lib().cn_batched_sweep(plan, _ptr(psi), nsys, elem_stride, sys_stride, nsteps, _stream(stream)),
+           "cn_batched_sweep")
+
+
+def cn_destroy(plan):
+    _check(None, lib().cn_destroy(plan), "cn_destroy")
+
+
+def cn_plan_get_info(plan) -> dict:
+    info = cn_plan_info()
+    _check(plan, lib().cn_plan_get_info(plan, ctypes.byref(info)), "cn_plan_get_info")
+    return {k: getattr(info, k) for k, _ in cn_plan_info._fields_}
+
+
+def cn_version() -> str:
+    return lib().cn_version().decode()
+
+
+class Plan:
+    """RAII convenience around the handle; still marshalling only."""
+
+    def __init__(self, N, P, dx, dt, V, path=PATH_AUTO, tile_threads=0, device_budget=0, **opts):
+        self.h = cn_plan_create(N, P, dx, dt, V)
+        self.N, self.P = N, P
+        if path:
+            cn_plan_set_option(self.h, CN_OPT_PATH, path)
+        if tile_threads:
+            cn_plan_set_option(self.h, CN_OPT_TILE_THREADS, tile_threads)
+        if device_budget:
+            cn_plan_set_device_budget(self.h, device_budget)
+        for k, v in opts.items():
+            cn_plan_set_option(self.h, {"rs_threads": CN_OPT_RS_THREADS, "use_graph": CN_OPT_USE_GRAPH,
+                                        "rs_levels": CN_OPT_RS_LEVELS}[k], v)
+
+    def factorize(self, stream=None):
+        cn_factorize(self.h, stream)
+        return self
+
+    def step(self, psi, nsteps=1, stream=None):
+        cn_step(self.h, psi, nsteps, stream)
+
+    def batched_sweep(self, psi, nsys, elem_stride, sys_stride, nsteps=1, stream=None):
+        cn_batched_sweep(self.h, psi, nsys, elem_stride, sys_stride, nsteps, stream)
+
+    def info(self):
+        return cn_plan_get_info(self.h)
+
+    def close(self):
+        if self.h:
+            cn_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()

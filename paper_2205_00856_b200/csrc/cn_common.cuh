@@ -1,0 +1,93 @@
+// Common device helpers: complex128 arithmetic written out in re/im with explicit FMAs
+// (the paper notes the same hand expansion paid off on its GPU), and the
+// first-order linear recurrence scan used by every sweep.
+//
+// Scaled system: every row of Eq. 5 is multiplied by kappa = i / s with
+// s = dt / (4 dx^2).  Because b = c = -i s this makes both off-diagonals of kappa*T exactly 1 and
+// its diagonal mu_j = -gamma_j + i rho,  gamma_j = 2 + 2 dx^2 V_j,  rho = 1 / s = 4 dx^2 / dt.
+// The scaled right-hand side of Eq. 3 is E_j = (gamma_j + i rho) psi_j - psi_{j-1} - psi_{j+1}.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+typedef double2 cplx;
+
+#define CN_DEVINL __device__ __forceinline__
+
+CN_DEVINL cplx cmake(double x, double y) { return make_double2(x, y); }
+CN_DEVINL cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
+CN_DEVINL cplx csub(cplx a, cplx b) { return make_double2(a.x - b.x, a.y - b.y); }
+CN_DEVINL cplx cneg(cplx a) { return make_double2(-a.x, -a.y); }
+CN_DEVINL cplx cmul(cplx a, cplx b)
+{
+    return make_double2(fma(-a.y, b.y, a.x * b.x), fma(a.y, b.x, a.x * b.y));
+}
+// c + a*b
+CN_DEVINL cplx cfma(cplx a, cplx b, cplx c)
+{
+    return make_double2(fma(-a.y, b.y, fma(a.x, b.x, c.x)), fma(a.y, b.x, fma(a.x, b.y, c.y)));
+}
+// c - a*b
+CN_DEVINL cplx cfnma(cplx a, cplx b, cplx c)
+{
+    return make_double2(fma(a.y, b.y, fma(-a.x, b.x, c.x)), fma(-a.y, b.x, fma(-a.x, b.y, c.y)));
+}
+CN_DEVINL cplx crecip(cplx a)
+{
+    // scaled by the larger component so that |a|^2 can neither overflow nor underflow early
+    double m = fmax(fabs(a.x), fabs(a.y));
+    double inv_m = 1.0 / m;
+    double xr = a.x * inv_m, xi = a.y * inv_m;
+    double d = 1.0 / (fma(xr, xr, xi * xi));
+    return make_double2(xr * d * inv_m, -xi * d * inv_m);
+}
+CN_DEVINL bool cfinite_nonzero(cplx a)
+{
+    return isfinite(a.x) && isfinite(a.y) && (a.x != 0.0 || a.y != 0.0);
+}
+
+// E = (gamma + i rho) * p - lo - hi      (scaled Eq. 3)
+CN_DEVINL cplx rhs_E(double gamma, double rho, cplx p, cplx lo, cplx hi)
+{
+    double er = fma(gamma, p.x, fma(-rho, p.y, -(lo.x + hi.x)));
+    double ei = fma(gamma, p.y, fma(rho, p.x, -(lo.y + hi.y)));
+    return make_double2(er, ei);
+}
+
+CN_DEVINL cplx shfl_up_c(cplx v, int d)
+{
+    return make_double2(__shfl_up_sync(0xffffffffu, v.x, d), __shfl_up_sync(0xffffffffu, v.y, d));
+}
+CN_DEVINL cplx shfl_down_c(cplx v, int d)
+{
+    return make_double2(__shfl_down_sync(0xffffffffu, v.x, d), __shfl_down_sync(0xffffffffu, v.y, d));
+}
+CN_DEVINL cplx shfl_c(cplx v, int src)
+{
+    return make_double2(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src));
+}
+
+// ---- scan of affine maps  x -> A x + B  ------------------------------------------------------------
+// A sweep D_i = E_i - q_{i-1} D_{i-1} restricted to one thread's chunk is the affine map
+// "value entering the chunk -> value leaving it".  Composing the maps of consecutive chunks gives
+// every chunk its true inflow.  At a joint line the value is reset, i.e. A = 0, which is what keeps
+// blocks independent ("no communication at this stage").
+//
+// Warp-level inclusive Kogge-Stone over lanes in direction DIR (+1: information flows to higher
+// lanes, -1: to lower lanes).  STEPS = number of doubling steps (5 for a full warp; fewer when a
+// block spans fewer than 32 chunks, because A = 0 at block ends makes later steps no-ops).
+template <int DIR, int STEPS>
+CN_DEVINL void warp_scan_affine(cplx &A, cplx &B, int lane)
+{
+#pragma unroll
+    for (int k = 0; k < STEPS; ++k) {
+        const int d = 1 << k;
+        cplx As = (DIR > 0) ? shfl_up_c(A, d) : shfl_down_c(A, d);
+        cplx Bs = (DIR > 0) ? shfl_up_c(B, d) : shfl_down_c(B, d);
+        bool ok = (DIR > 0) ? (lane >= d) : (lane + d < 32);
+        if (ok) {
+            B = cfma(A, Bs, B);
+            A = cmul(A, As);
+        }
+    }
+}

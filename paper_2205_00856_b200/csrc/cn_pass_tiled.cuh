@@ -1,0 +1,328 @@
+// Tiled pass kernel for sm_100a: the hot path.
+//
+// One CTA owns a tile of TPB*8 consecutive points = a whole number of blocks.  The tile of psi, of the
+// stored inverse pivots q and of gamma is brought in by three TMA tensor loads (cp.async.bulk.tensor,
+// SASS UTMALDG) from 2-D views [N/8][8 points] with the 128-byte (64-byte for gamma) shared-memory
+// swizzle, so that HBM sees only full-line coalesced traffic while thread t can read "its" row of
+// 8 consecutive points conflict-free: that is the transposition from the paper's "conventional layout"
+// to one contiguous chunk per thread.  The new psi leaves through the same swizzled
+// buffer with one TMA tensor store (UTMASTG).
+//
+// Inside a block the RD / RU sweeps are first-order linear recurrences.  A thread
+// sweeps its 8 points serially; the chunks of one block are chained by the affine-map scan of
+// cn_common.cuh (warp shuffles carry the interface values).  A joint line resets the recurrence
+// (A = 0), so blocks stay independent exactly as in the paper.
+//
+//   P1 (finish step k):  E = scaled T^dagger psi (Eq. 3) -> RD with the new support value of the joint
+//                        above as inflow -> RU + SS with the support value of the own joint -> new psi.
+//   P2 (start step k+1): E of the new psi -> RD, RU with zero support values -> JD / JU contributions
+//                        slotD[w], slotU[w-1] (two slots per joint line instead of atomics).
+//
+// Algorithmic HBM bytes per point of a fused pass: psi in 16 + q 16 + gamma 8 + psi out 16 = 56.
+#pragma once
+#include <cuda.h>
+#include "cn_common.cuh"
+
+struct cn_tiled_params {
+    int64_t nchunks; // N / 8
+    int64_t P;
+    double rho;
+    const cplx *psi_raw; // prologue only: old psi for the tile's left halo
+    const cplx *supOld;  // psi^k   at the joint lines (RS output of the previous step)
+    const cplx *supNew;  // psi^k+1 at the joint lines (RS output of this step)
+    cplx *slotD, *slotU;
+    cplx *supInit; // prologue only: receives psi^0 at the joint lines
+};
+
+CN_DEVINL uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+CN_DEVINL void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+CN_DEVINL void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+CN_DEVINL void mbar_wait(uint64_t *bar, uint32_t phase)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(phase)
+            : "memory");
+    } while (!done);
+}
+CN_DEVINL void tma_load_2d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+        : "memory");
+}
+CN_DEVINL void tma_store_2d(const CUtensorMap *map, const void *src, int c0, int c1)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(map),
+                 "r"(smem_u32(src)), "r"(c0), "r"(c1)
+                 : "memory");
+}
+CN_DEVINL void tma_store_commit_wait()
+{
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+CN_DEVINL void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// shared-memory bytes of one CTA
+template <int TPB>
+constexpr size_t tiled_smem_bytes()
+{
+    return 1024 /*alignment slack*/ + (size_t)TPB * (128 + 128 + 64) + 2 * 2 * 32 * sizeof(cplx) + 4 * 32 * sizeof(cplx) + 64;
+}
+
+// TPB threads, 8 points per thread, 2^LOGC chunks (threads) per block.
+template <int TPB, int LOGC, bool P1, bool P2, int MINB>
+__global__ void __launch_bounds__(TPB, MINB)
+k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ CUtensorMap tmQ,
+             const __grid_constant__ CUtensorMap tmGam, const cn_tiled_params prm)
+{
+    constexpr int CPB = 1 << LOGC;          // chunks per block
+    constexpr bool XWARP = (LOGC > 5);      // a block spans several warps
+    constexpr int WSTEPS = XWARP ? 5 : LOGC; // shuffle-scan steps inside a warp
+    constexpr int NW = TPB / 32;
+    static_assert(CPB <= TPB, "a block must fit in one tile");
+
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *base = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    cplx *s_psi = (cplx *)base;
+    cplx *s_q = (cplx *)(base + (size_t)TPB * 128);
+    double2 *s_g = (double2 *)(base + (size_t)TPB * 256);
+    cplx *s_scan = (cplx *)(base + (size_t)TPB * 320);        // [2 buffers][A,B][32]
+    cplx *s_edge = s_scan + 2 * 2 * 32;                        // [4][32] edge exchange between warps
+    uint64_t *bar = (uint64_t *)(s_edge + 4 * 32);
+
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    const int64_t row0 = (int64_t)blockIdx.x * TPB;
+    const int64_t c = row0 + t; // global chunk index
+    const bool active = c < prm.nchunks;
+    const bool isFirst = (c & (CPB - 1)) == 0;
+    const bool isLast = (c & (CPB - 1)) == CPB - 1;
+    const int64_t w = c >> LOGC;
+    const double rho = prm.rho;
+    const cplx zero = cmake(0.0, 0.0);
+
+    if (t == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (t == 0) {
+        mbar_expect_tx(bar, (uint32_t)(TPB * 320));
+#pragma unroll
+        for (int r = 0; r < TPB; r += 256) {
+            const int rows = (TPB - r < 256) ? (TPB - r) : 256;
+            (void)rows;
+            tma_load_2d((uint8_t *)s_psi + (size_t)r * 128, &tmPsi, bar, 0, (int)(row0 + r));
+            tma_load_2d((uint8_t *)s_q + (size_t)r * 128, &tmQ, bar, 0, (int)(row0 + r));
+            tma_load_2d((uint8_t *)s_g + (size_t)r * 64, &tmGam, bar, 0, (int)(row0 + r));
+        }
+    }
+    // while the tile is in flight: the few values that live on the joint lines
+    cplx supN = zero;      // new value of the own joint line (last chunk of a block)
+    cplx jointAbove = zero; // new value of the joint line above the block of this thread
+    if (active) {
+        if (P1) {
+            if (isLast) supN = prm.supNew[w];
+            if (w > 0) jointAbove = prm.supNew[w - 1];
+        }
+    }
+    cplx oldAbove = zero; // OLD psi just above the tile (needed by thread 0 only)
+    if (t == 0 && c > 0) oldAbove = P1 ? prm.supOld[w - 1] : prm.psi_raw[8 * c - 1];
+
+    mbar_wait(bar, 0);
+
+    // ---- registers <- swizzled shared memory ----------------------------------------------------------
+    cplx v[8], qv[8];
+    double g[8];
+    const int sw = t & 7;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        v[j] = s_psi[t * 8 + (j ^ sw)];
+        qv[j] = s_q[t * 8 + (j ^ sw)];
+    }
+    const int sg = (t >> 1) & 3;
+#pragma unroll
+    for (int jj = 0; jj < 4; ++jj) {
+        double2 gg = s_g[t * 4 + (jj ^ sg)];
+        g[2 * jj] = gg.x;
+        g[2 * jj + 1] = gg.y;
+    }
+    cplx vlo, vhi, qm1;
+    if (t > 0) {
+        vlo = s_psi[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
+        qm1 = s_q[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
+    } else {
+        vlo = oldAbove;
+        qm1 = cmake(1.0, 0.0); // the row above a tile is a joint line (or the virtual one)
+    }
+    vhi = (t < TPB - 1) ? s_psi[(t + 1) * 8 + ((t + 1) & 7)] : zero;
+    if (!P1 && isFirst) jointAbove = vlo; // prologue: psi^0 of the joint above
+
+    // chunk multipliers: Qp = prod_{j<7} (-q_j);  RD map A = (-q_{-1}) Qp,  RU map A = Qp (-q_7)
+    cplx Qp = cneg(qv[0]);
+#pragma unroll
+    for (int j = 1; j < 7; ++j) Qp = cmul(Qp, cneg(qv[j]));
+    const cplx fwdA = isLast ? zero : cmul(cneg(qm1), Qp);
+    const cplx bwdA = isLast ? zero : cmul(Qp, cneg(qv[7]));
+
+    // exclusive inflow of a forward (RD) chain; tin = value on the joint line above the block
+    auto scan_fwd = [&](cplx A, cplx B, cplx tin, int buf) -> cplx {
+        warp_scan_affine<+1, WSTEPS>(A, B, lane);
+        cplx carry = tin;
+        if (XWARP) {
+            cplx *sA = s_scan + buf * 64, *sB = sA + 32;
+            if (lane == 31) {
+                sA[warp] = A;
+                sB[warp] = B;
+            }
+            __syncthreads();
+            const int vb = warp & ~((CPB / 32) - 1); // first warp of this block
+            for (int u = vb; u < warp; ++u) carry = cfma(sA[u], carry, sB[u]);
+        }
+        cplx Ae = shfl_up_c(A, 1), Be = shfl_up_c(B, 1);
+        return (lane == 0) ? carry : cfma(Ae, carry, Be);
+    };
+    // exclusive inflow of a backward (RU) chain; nothing enters a block from below (joint resets)
+    auto scan_bwd = [&](cplx A, cplx B, int buf) -> cplx {
+        warp_scan_affine<-1, WSTEPS>(A, B, lane);
+        cplx carry = zero;
+        if (XWARP) {
+            cplx *sA = s_scan + buf * 64, *sB = sA + 32;
+            if (lane == 0) {
+                sA[warp] = A;
+                sB[warp] = B;
+            }
+            __syncthreads();
+            const int ve = (warp & ~((CPB / 32) - 1)) + (CPB / 32) - 1; // last warp of this block
+            for (int u = ve; u > warp; --u) carry = cfma(sA[u], carry, sB[u]);
+        }
+        cplx Ae = shfl_down_c(A, 1), Be = shfl_down_c(B, 1);
+        return (lane == 31) ? carry : cfma(Ae, carry, Be);
+    };
+
+    if (P1) {
+        // ---- Eq. 3 fused into RD ----------------------------------------------------
+        cplx E[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            cplx lo = (j == 0) ? vlo : v[j - 1];
+            cplx hi = (j == 7) ? vhi : v[j + 1];
+            E[j] = rhs_E(g[j], rho, v[j], lo, hi);
+        }
+        if (isLast) E[7] = supN; // the joint line carries its new support value
+        cplx D = zero;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
+        if (isLast) D = supN;
+        cplx in = scan_fwd(fwdA, D, jointAbove, 0);
+        D = in;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
+            E[j] = D; // E now holds d after RD
+        }
+        // ---- RU + SS: x_j = q_j (d_j - x_{j+1}) ---------------------------------------------------------
+        cplx X = zero;
+#pragma unroll
+        for (int j = 7; j >= 0; --j) {
+            X = cmul(qv[j], csub(E[j], X));
+            if (j == 7 && isLast) X = supN;
+        }
+        cplx xin = scan_bwd(bwdA, X, 1);
+        X = xin;
+#pragma unroll
+        for (int j = 7; j >= 0; --j) {
+            X = cmul(qv[j], csub(E[j], X));
+            if (j == 7 && isLast) X = supN;
+            v[j] = X;
+        }
+    }
+
+    if (P1) {
+        // the old psi in shared memory has been read by everybody (halo reads above): overwrite with the new
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s_psi[t * 8 + (j ^ sw)] = v[j];
+        fence_proxy_async();
+        __syncthreads();
+        if (t == 0) {
+#pragma unroll
+            for (int r = 0; r < TPB; r += 256) tma_store_2d(&tmPsi, (uint8_t *)s_psi + (size_t)r * 128, 0, (int)(row0 + r));
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+    }
+
+    if (P2) {
+        // ---- neighbours of the NEW psi ----------------------------------------------------------------
+        cplx xlo = shfl_up_c(v[7], 1), xhi = shfl_down_c(v[0], 1);
+        if (XWARP) {
+            cplx *eLo = s_edge, *eHi = s_edge + 32;
+            if (lane == 31) eLo[warp] = v[7];
+            if (lane == 0) eHi[warp] = v[0];
+            __syncthreads();
+            if (lane == 0 && warp > 0) xlo = eLo[warp - 1];
+            if (lane == 31 && warp < NW - 1) xhi = eHi[warp + 1];
+        }
+        if (isFirst) xlo = jointAbove; // also covers lane 0 when blocks do not span warps
+        cplx E[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            cplx lo = (j == 0) ? xlo : v[j - 1];
+            cplx hi = (j == 7) ? (isLast ? zero : xhi) : v[j + 1];
+            E[j] = rhs_E(g[j], rho, v[j], lo, hi);
+        }
+        const cplx EJ = E[7]; // for a last chunk: E of the joint line without its psi_{J+1} term (JD part)
+        if (isLast) E[7] = zero;
+        cplx D = zero;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
+        if (isLast) D = zero;
+        cplx in = scan_fwd(fwdA, D, zero, 1);
+        D = in;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
+            E[j] = D;
+        }
+        cplx Y = zero, yn = zero;
+#pragma unroll
+        for (int j = 7; j >= 0; --j) {
+            Y = cmul(qv[j], csub(E[j], Y));
+            if (j == 7 && isLast) Y = zero;
+            if (j == 6) yn = Y; // local solution next to the own joint (meaningful for a last chunk)
+        }
+        cplx yin = scan_bwd(bwdA, Y, 0);
+        if (active) {
+            if (isLast) {
+                prm.slotD[w] = csub(EJ, yn);
+                if (w == prm.P - 1) prm.slotU[w] = zero;
+                if (!P1) prm.supInit[w] = v[7];
+            }
+            if (isFirst && w > 0) {
+                cplx y0 = cfma(bwdA, yin, Y); // isLast && isFirst: bwdA = 0 and Y is already exact
+                prm.slotU[w - 1] = cneg(cadd(v[0], y0));
+            }
+        }
+    }
+
+    if (P1) {
+        if (t == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    }
+}

@@ -1,0 +1,160 @@
+"""Parity of the CUDA path (through the C-ABI) with the oracle, element by element, on the same seeded
+inputs.  Tolerances are BASELINE.json's: max |dpsi| <= 1e-10 after the config's step count, relative
+residual <= 1e-12 per solve."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import cn_oracle as O
+from paper_2205_00856_b200 import binding as B
+from paper_2205_00856_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+TOL_PSI = 1e-10
+TOL_RES = 1e-12
+
+
+def torch_():
+    import torch
+    return torch
+
+
+def gpu_step(N, P, dx, dt, V, psi, nsteps, path=B.PATH_AUTO, tile_threads=0, calls=1):
+    torch = torch_()
+    d_psi = torch.from_numpy(np.ascontiguousarray(psi)).cuda()
+    with B.Plan(N, P, dx, dt, np.ascontiguousarray(V), path=path, tile_threads=tile_threads) as plan:
+        plan.factorize()
+        for _ in range(calls):
+            plan.step(d_psi, nsteps)
+        torch.cuda.synchronize()
+        info = plan.info()
+    return d_psi.cpu().numpy(), info
+
+
+def residual(dx, dt, V, old, new):
+    """|| T new - T^dagger old || / || T^dagger old || with T applied as a stencil in numpy (not the oracle)."""
+    s = dt / (4 * dx * dx)
+    a = 1 + 1j * (2 * s + 0.5 * dt * V)
+
+    def apply(diag, off, x):
+        y = diag * x
+        y[1:] += off * x[:-1]
+        y[:-1] += off * x[1:]
+        return y
+    d = apply(np.conj(a), 1j * s, old)
+    r = apply(a, -1j * s, new) - d
+    return np.linalg.norm(r) / np.linalg.norm(d)
+
+
+GENERIC_SHAPES = [(2, 1), (2, 2), (9, 2), (10, 3), (40, 7), (64, 64), (65, 32), (33, 33), (100, 1), (1000, 37),
+                  (4096, 64), (5000, 123), (777, 776)]
+
+
+@pytest.mark.parametrize("N,P", GENERIC_SHAPES)
+def test_generic_path_random(N, P):
+    # ragged blocks, blocks of one interior row, joint-only blocks (m = 1), a single block
+    V, psi = W.random_system(N, seed=17)
+    dx, dt = 0.2, 0.03
+    for nsteps in (1, 4):
+        ref = O.step(dx, dt, V, psi, nsteps)
+        out, info = gpu_step(N, P, dx, dt, V, psi, nsteps, path=B.PATH_GENERIC)
+        assert info["path"] == B.PATH_GENERIC
+        assert np.max(np.abs(out - ref)) <= TOL_PSI, (N, P, nsteps)
+    out1, _ = gpu_step(N, P, dx, dt, V, psi, 1, path=B.PATH_GENERIC)
+    assert residual(dx, dt, V, psi, out1) <= TOL_RES
+
+
+TILED_SHAPES = [
+    # (N, P, tile_threads)   m = N/P must be 8 * 2^k
+    (64, 8, 0), (64, 1, 0), (256, 1, 0), (2048, 1, 0), (4096, 1, 512), (4096, 64, 0), (4096, 64, 128),
+    (4096, 64, 512), (1 << 16, 1 << 13, 0), (1 << 16, 1 << 12, 0), (1 << 16, 1 << 11, 128), (1 << 16, 1 << 10, 0),
+    (1 << 16, 1 << 9, 0), (1 << 16, 1 << 8, 0), (1 << 16, 1 << 7, 512), (1 << 16, 1 << 6, 0), (1 << 16, 1 << 5, 0),
+    (1 << 16, 1 << 4, 512), (6656, 26, 0), (6656, 26, 128), (8 * 1000, 1000, 0), (2048 * 3 + 512, 13, 0),
+    (2048 * 5 + 1024, 11, 0),
+]
+
+
+@pytest.mark.parametrize("N,P,tt", TILED_SHAPES)
+def test_tiled_path_random(N, P, tt):
+    # several tiles and a ragged last tile; every scan depth (block inside a warp, across warps)
+    V, psi = W.random_system(N, seed=23)
+    dx, dt = 0.1, 0.02
+    for nsteps in (1, 3):
+        ref = O.step(dx, dt, V, psi, nsteps)
+        out, info = gpu_step(N, P, dx, dt, V, psi, nsteps, path=B.PATH_TILED, tile_threads=tt)
+        assert info["path"] == B.PATH_TILED
+        err = np.max(np.abs(out - ref))
+        assert err <= TOL_PSI, (N, P, tt, nsteps, err)
+    out1, _ = gpu_step(N, P, dx, dt, V, psi, 1, path=B.PATH_TILED, tile_threads=tt)
+    assert residual(dx, dt, V, psi, out1) <= TOL_RES
+
+
+def test_config_c1_both_paths():
+    cfg = W.CONFIGS["C1"]
+    V, psi = W.potential(cfg), W.psi0(cfg)
+    ref = O.step(cfg.dx, cfg.dt, V, psi, cfg.steps)
+    for path in (B.PATH_GENERIC, B.PATH_TILED, B.PATH_AUTO):
+        out, info = gpu_step(cfg.N, cfg.P, cfg.dx, cfg.dt, V, psi, cfg.steps, path=path)
+        assert np.max(np.abs(out - ref)) <= TOL_PSI
+        assert abs(np.vdot(out, out).real * cfg.dx - 1.0) <= 1e-12
+    # the same 100 steps as 10 calls of 10 (prologue / epilogue per call)
+    out, _ = gpu_step(cfg.N, cfg.P, cfg.dx, cfg.dt, V, psi, 10, calls=10)
+    assert np.max(np.abs(out - ref)) <= TOL_PSI
+
+
+def test_p_invariance_and_linearity():
+    cfg = W.scaled(W.CONFIGS["C2dense"], N=1 << 15)
+    V, psi = W.potential(cfg), W.psi0(cfg)
+    outs = [gpu_step(cfg.N, P, cfg.dx, cfg.dt, V, psi, 5)[0] for P in (1 << 3, 1 << 6, 1 << 9, 1 << 12)]
+    for o in outs[1:]:
+        assert np.max(np.abs(o - outs[0])) <= 1e-13
+    a, _ = gpu_step(cfg.N, 1 << 7, cfg.dx, cfg.dt, V, (2 - 3j) * psi, 5)
+    assert np.max(np.abs(a - (2 - 3j) * outs[0])) <= 1e-12
+
+
+def test_time_reversal_gpu():
+    cfg = W.scaled(W.CONFIGS["C1"], N=1 << 14, P=1 << 6)
+    V, psi = W.potential(cfg), W.psi0(cfg)
+    fwd, _ = gpu_step(cfg.N, cfg.P, cfg.dx, cfg.dt, V, psi, 20)
+    back, _ = gpu_step(cfg.N, cfg.P, cfg.dx, -cfg.dt, V, fwd, 20)
+    assert np.max(np.abs(back - psi)) <= 1e-11
+
+
+def test_cayley_phase_gpu():
+    # closed form straight against the CUDA path (V = 0, sine mode)
+    n, k, dx, dt, steps = 4096, 7, 0.1, 0.01, 200
+    j = np.arange(1, n + 1)
+    v = np.sin(math.pi * k * j / (n + 1)).astype(complex)
+    lam = (1.0 - math.cos(math.pi * k / (n + 1))) / dx ** 2
+    ph = ((1 - 0.5j * lam * dt) / (1 + 0.5j * lam * dt)) ** steps
+    out, _ = gpu_step(n, 32, dx, dt, np.zeros(n), v, steps)
+    assert np.max(np.abs(out - ph * v)) <= 1e-11
+
+
+def test_errors_on_device():
+    torch = torch_()
+    V = np.zeros(64)
+    plan = B.Plan(64, 8, 0.1, 0.01, V)
+    psi = torch.zeros(64, dtype=torch.complex128, device="cuda")
+    with pytest.raises(B.CnError) as ei:
+        plan.step(psi, 1)
+    assert ei.value.status == B.CN_ENOTFACTORIZED
+    plan.factorize()
+    plan.step(psi, 0)
+    with pytest.raises(B.CnError) as ei:
+        B.cn_step(plan.h, psi.data_ptr() + 8, 1)
+    assert ei.value.status == B.CN_EINVAL
+    plan.close()
+    # V given as a device tensor
+    dV = torch.zeros(64, dtype=torch.float64, device="cuda")
+    with B.Plan(64, 8, 0.1, 0.01, dV) as p2:
+        p2.factorize()
+        p2.step(psi, 2)
+    # breakdown: mu = -gamma + i rho hits a non-finite pivot when V is not finite
+    Vbad = np.zeros(64)
+    Vbad[10] = np.inf
+    with B.Plan(64, 8, 0.1, 0.01, Vbad) as p3:
+        with pytest.raises(B.CnError) as ei:
+            p3.factorize()
+        assert ei.value.status == B.CN_EBREAKDOWN
