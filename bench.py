@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the B200-native N-shaped partition Crank-Nicolson stepper.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Metric (BASELINE.json): CN grid-point-steps per second in complex128 on config C2
+(N = 2^24, dx = 0.05, dt = 0.005, soft-Coulomb V), plus the achieved fraction of the HBM roofline.
+
+One bench "step" = one `cn_step(plan, psi, nsteps = CN_PER_STEP)` call through the C-ABI, i.e. one pass of
+the whole hot path (RHS, RD, RU, JD/JU, RS, SS and psi write -- every row of SURVEY 8a) CN_PER_STEP times
+over the resident wave function; K = 10 such steps are the 1000 CN steps of the config.
+`value` has psi, V and the factors resident in HBM; `e2e` is the same call with psi in PINNED HOST memory,
+copied host->device before and device->host after every bench step inside the timed region.
+
+N > 1 (torchrun, one rank per GPU): the path does not shard in this build ("replicas only");
+every rank advances its own replica of the system, no data-path collective; value = sum over ranks.
+
+--impl reference times the ORACLE (plain serial Thomas CN stepper, oracle/) on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2205_00856_b200 import workloads as W  # noqa: E402
+
+CN_PER_STEP = 100            # CN steps per bench step (one cn_step call)
+BYTES_PER_POINT_STEP = 56.0  # algorithmic: psi in 16 + q 16 + gamma 8 + psi out 16
+METRIC = "cn_grid_point_steps_per_sec_complex128"
+UNIT = "Gpoint-steps/s"
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            with open(path) as f:
+                return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic_per_launch():
+    """dram bytes per fused-pass launch from the committed ncu --set full capture, if any (profiles/)."""
+    path = os.path.join(ROOT, "profiles", "pass_kernel_traffic.txt")
+    try:
+        with open(path) as f:
+            for line in f:
+                if line.startswith("dram_bytes_per_launch_at_N_2^24="):
+                    return float(line.split("=")[1])
+    except Exception:
+        pass
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.proc = None
+        self.lines = []
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._pump, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        time.sleep(0.05)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [ln for (ts, ln) in self.lines if t0 <= ts <= t1 + 0.05] or [ln for (_, ln) in self.lines]
+        for ln in rows:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                smax.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def oracle_timed(cfg, V, psi, cn_steps: int):
+    from oracle import cn_oracle as O
+    work = psi.copy()
+    sec = O.step_inplace(cfg.dx, cfg.dt, V, work, cn_steps)
+    return sec, work
+
+
+def run_reference(args):
+    """The oracle as it stands, on the host cores, same metric/config (bounded sample per step)."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    cfg = W.CONFIGS["C2dense"]
+    V, psi = W.potential(cfg), W.psi0(cfg)
+    from oracle import cn_oracle as O
+    cn_per = 2                                # bounded sample: 2 CN steps at full N per bench step (~1 s)
+    work = psi.copy()
+    for _ in range(args.warmup):
+        O.step_inplace(cfg.dx, cfg.dt, V, work, 1)
+    tot = 0.0
+    for _ in range(args.steps):
+        tot += O.step_inplace(cfg.dx, cfg.dt, V, work, cn_per)
+    value = cfg.N * cn_per * args.steps / tot / 1e9
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "C2 (N=2^24, dx=0.05, dt=0.005, soft-Coulomb V, Gaussian x random phase + 1e-3 noise)",
+                   "cn_steps_per_bench_step": cn_per},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": "%d CN steps at full N=2^24 per bench step, serial Thomas, 1 thread" % cn_per},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--P", type=int, default=0, help="partition count (0 = config default)")
+    ap.add_argument("--tile-threads", type=int, default=0)
+    ap.add_argument("--cn-per-step", type=int, default=CN_PER_STEP)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="also time the P sweep 2^8..2^16 (extra JSON key)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2205_00856_b200 import binding as B
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; this library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = W.CONFIGS["C2dense"]
+    P = args.P or cfg.P
+    cn_per = args.cn_per_step
+    V, psi_h = W.potential(cfg), W.psi0(cfg)
+    psi_pin = torch.from_numpy(psi_h).pin_memory()
+    d_psi = psi_pin.cuda()
+    plan = B.Plan(cfg.N, P, cfg.dx, cfg.dt, V, tile_threads=args.tile_threads)
+    t0 = time.time()
+    plan.factorize()
+    torch.cuda.synchronize()
+    factor_ms = 1e3 * (time.time() - t0)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed_region(fn, steps):
+        """EXACTLY `steps` calls of fn between barrier+sync, CUDA events on the launching stream, max over ranks."""
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        w0 = time.time()
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+        barrier()
+        w1 = time.time()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, w0, w1
+
+    # ---- value: everything resident in HBM; event pairs bracket every fused-pass launch (roofline) ---------
+    plan.set_option(B.CN_OPT_PROFILE, 1)
+    for _ in range(args.warmup):
+        plan.step(d_psi, cn_per)
+    torch.cuda.synchronize()
+    plan.profile()  # drop warm-up samples
+    launches0 = plan.info()["launches"]
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.1)
+    ms, w0, w1 = timed_region(lambda: plan.step(d_psi, cn_per), args.steps)
+    clocks = sampler.stop(w0, w1)
+    launches = plan.info()["launches"] - launches0
+    prof = plan.profile()
+    plan.set_option(B.CN_OPT_PROFILE, 0)
+    value = world * cfg.N * cn_per * args.steps / (ms * 1e-3) / 1e9
+
+    # ---- roofline of the dominant kernel (fused pass) -----------------------------------------------------
+    peak, peak_src = measured_peaks()
+    pass_ms = prof["pass_ms"] / max(1, prof["pass_count"])
+    achieved = BYTES_PER_POINT_STEP * cfg.N / (pass_ms * 1e-3) / 1e9 if prof["pass_count"] else None
+    traffic = ncu_traffic_per_launch()
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": (achieved / peak) if achieved else None, "traffic": traffic,
+                "kernel": "k_pass_tiled<P1,P2> (fused SS(k) + RHS/RD/RU/JD/JU(k+1))",
+                "kernel_ms": pass_ms, "launches_timed": prof["pass_count"],
+                "rs_kernel_ms": prof["rs_ms"] / max(1, prof["rs_count"]),
+                "algorithmic_bytes_per_launch": BYTES_PER_POINT_STEP * cfg.N, "peak_source": peak_src,
+                "whole_step_GBps": BYTES_PER_POINT_STEP * cfg.N * cn_per * args.steps / (ms * 1e-3) / 1e9}
+
+    # ---- e2e: psi lives in pinned host memory, H2D + cn_step + D2H inside the timed region ---------------
+    e2e = None
+    if not args.no_e2e:
+        def e2e_step():
+            d_psi.copy_(psi_pin, non_blocking=True)
+            plan.step(d_psi, cn_per)
+            psi_pin.copy_(d_psi, non_blocking=True)
+        for _ in range(2):
+            e2e_step()
+        ms_e, _, _ = timed_region(e2e_step, args.steps)
+        e2e = {"value": world * cfg.N * cn_per * args.steps / (ms_e * 1e-3) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": 16 * cfg.N, "d2h_bytes_per_step": 16 * cfg.N,
+               "ms_per_step": ms_e / args.steps}
+
+    # ---- optional P sweep (config C2: P = 2^8..2^16 against the paper's optimal-P model) -----------------
+    sweep = None
+    if args.sweep and rank == 0:
+        sweep = []
+        for Pk in cfg.P_sweep:
+            pl = B.Plan(cfg.N, Pk, cfg.dx, cfg.dt, V).factorize()
+            info = pl.info()
+            n = 20 if info["path"] == B.PATH_TILED else 2
+            pl.step(d_psi, 2)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            pl.step(d_psi, n)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            sweep.append({"P": Pk, "path": info["path"], "us_per_cn_step": 1e3 * e0.elapsed_time(e1) / n})
+            pl.close()
+
+    # ---- cpu_baseline: the oracle as it stands on this box's host cores, bounded sample (rank 0, N = 1) ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nsamp = 24
+        sec, _ = oracle_timed(cfg, V, psi_h, nsamp)
+        cpu = {"value": cfg.N * nsamp / sec / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "host_cores_available": os.cpu_count(),
+               "sample": "first %d of the 1000 CN steps of C2 at full N=2^24 (serial Thomas, 1 thread)" % nsamp}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "C2 (N=2^24 complex128, dx=0.05, dt=0.005, soft-Coulomb V, Gaussian x random "
+                                   "phase + 1e-3 dense noise)", "N": cfg.N, "P": P, "cn_steps_per_bench_step": cn_per,
+                       "l2_policy": "inputs_larger_than_L2 (psi 268 MB + factors 403 MB per pass vs 126 MB L2)",
+                       "parallelism": "replicas x%d" % world, "path": plan.info()["path"],
+                       "tile_threads": plan.info()["tile_threads"], "factorize_ms": factor_ms},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "cpu_baseline": cpu,
+        }
+        if sweep is not None:
+            line["p_sweep"] = sweep
+        print(json.dumps(line), flush=True)
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

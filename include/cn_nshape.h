@@ -55,7 +55,9 @@ typedef enum {
     CN_OPT_TILE_THREADS = 2,/* threads per CTA of the tiled kernels: 0 = auto, else 64/128/256/512 (8 points per thread) */
     CN_OPT_RS_THREADS = 3,  /* threads of the single-CTA reduced-system kernel (32..1024, power of two) */
     CN_OPT_USE_GRAPH = 4,   /* 1 = replay the per-step launches from a CUDA graph inside cn_step (default 0) */
-    CN_OPT_RS_LEVELS = 5    /* 0 = auto, 1 = single-CTA RS, 2 = two-level (nested, Eq. 6) RS */
+    CN_OPT_RS_LEVELS = 5,   /* 0 = auto, 1 = single-CTA RS, 2 = two-level (nested, Eq. 6) RS */
+    CN_OPT_PROFILE = 6      /* 1 = bracket every fused-pass and RS launch of cn_step with CUDA events on the
+                               launching stream (read back with cn_plan_get_profile); default 0 */
 } cn_option;
 
 typedef struct {
@@ -119,6 +121,12 @@ cn_status cn_batched_sweep(cn_plan *plan, void *psi, int64_t nsys, int64_t elem_
 cn_status cn_destroy(cn_plan *plan);
 
 cn_status cn_plan_get_info(const cn_plan *plan, cn_plan_info *info);
+
+/* Kernel timings gathered since the last call while CN_OPT_PROFILE was on (measurement aid):
+ * out[0] = sum of fused-pass kernel durations in ms, out[1] = their count,
+ * out[2] = sum of RS kernel durations in ms,        out[3] = their count.
+ * HOST pointer to 4 doubles.  Synchronises the recorded events, then resets the counters. */
+cn_status cn_plan_get_profile(cn_plan *plan, double *out);
 const char *cn_status_string(cn_status s);
 /* last CUDA runtime error code seen by this plan (0 = cudaSuccess) */
 cn_status cn_last_cuda_error(const cn_plan *plan, int *cuda_err);

@@ -14,12 +14,12 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(PKG, "libcn_nshape.so")
 
 CN_OK, CN_EINVAL, CN_ENOMEM, CN_ECUDA, CN_ENOTFACTORIZED, CN_EBREAKDOWN = range(6)
-CN_OPT_PATH, CN_OPT_TILE_THREADS, CN_OPT_RS_THREADS, CN_OPT_USE_GRAPH, CN_OPT_RS_LEVELS = 1, 2, 3, 4, 5
+CN_OPT_PATH, CN_OPT_TILE_THREADS, CN_OPT_RS_THREADS, CN_OPT_USE_GRAPH, CN_OPT_RS_LEVELS, CN_OPT_PROFILE = 1, 2, 3, 4, 5, 6
 PATH_AUTO, PATH_GENERIC, PATH_TILED = 0, 1, 2
 
 EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", "cn_factorize", "cn_step",
-           "cn_batched_sweep", "cn_destroy", "cn_plan_get_info", "cn_status_string", "cn_last_cuda_error",
-           "cn_version"]
+           "cn_batched_sweep", "cn_destroy", "cn_plan_get_info", "cn_plan_get_profile", "cn_status_string",
+           "cn_last_cuda_error", "cn_version"]
 
 
 class CnError(RuntimeError):
@@ -65,6 +65,8 @@ def lib():
         L.cn_destroy.argtypes = [vp]
         L.cn_plan_get_info.restype = i32
         L.cn_plan_get_info.argtypes = [vp, ctypes.POINTER(cn_plan_info)]
+        L.cn_plan_get_profile.restype = i32
+        L.cn_plan_get_profile.argtypes = [vp, ctypes.POINTER(dbl)]
         L.cn_status_string.restype = ctypes.c_char_p
         L.cn_status_string.argtypes = [i32]
         L.cn_last_cuda_error.restype = i32
@@ -148,6 +150,12 @@ def cn_plan_get_info(plan) -> dict:
     return {k: getattr(info, k) for k, _ in cn_plan_info._fields_}
 
 
+def cn_plan_get_profile(plan) -> dict:
+    out = (ctypes.c_double * 4)()
+    _check(plan, lib().cn_plan_get_profile(plan, out), "cn_plan_get_profile")
+    return {"pass_ms": out[0], "pass_count": int(out[1]), "rs_ms": out[2], "rs_count": int(out[3])}
+
+
 def cn_version() -> str:
     return lib().cn_version().decode()
 
@@ -166,7 +174,7 @@ class Plan:
             cn_plan_set_device_budget(self.h, device_budget)
         for k, v in opts.items():
             cn_plan_set_option(self.h, {"rs_threads": CN_OPT_RS_THREADS, "use_graph": CN_OPT_USE_GRAPH,
-                                        "rs_levels": CN_OPT_RS_LEVELS}[k], v)
+                                        "rs_levels": CN_OPT_RS_LEVELS, "profile": CN_OPT_PROFILE}[k], v)
 
     def factorize(self, stream=None):
         cn_factorize(self.h, stream)
@@ -180,6 +188,12 @@ class Plan:
 
     def info(self):
         return cn_plan_get_info(self.h)
+
+    def set_option(self, key, value):
+        cn_plan_set_option(self.h, key, value)
+
+    def profile(self):
+        return cn_plan_get_profile(self.h)
 
     def close(self):
         if self.h:

@@ -8,6 +8,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "../../include/cn_nshape.h"
 #include "cn_common.cuh"
@@ -33,7 +34,11 @@ struct cn_plan {
     int *derr = nullptr;
     size_t device_bytes = 0;
     // configuration
-    int opt_path = 0, opt_tile_threads = 0, opt_rs_threads = 1024, opt_graph = 0, opt_rs_levels = 0;
+    int opt_path = 0, opt_tile_threads = 0, opt_rs_threads = 1024, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0;
+    // profiling (CN_OPT_PROFILE): event pairs around fused-pass (kind 0) and RS (kind 1) launches
+    struct ev_pair { cudaEvent_t a, b; int kind; };
+    std::vector<ev_pair> ev_pool;
+    size_t ev_used = 0;
     size_t budget = 0;
     // derived at factorize
     bool factorized = false;
@@ -132,6 +137,10 @@ extern "C" cn_status cn_destroy(cn_plan *plan)
     if (!plan) return CN_EINVAL;
     free_factors(plan);
     if (plan->dV) cudaFree(plan->dV);
+    for (auto &e : plan->ev_pool) {
+        cudaEventDestroy(e.a);
+        cudaEventDestroy(e.b);
+    }
     delete plan;
     return CN_OK;
 }
@@ -168,6 +177,9 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
     case CN_OPT_RS_LEVELS:
         if (value < 0 || value > 2) return CN_EINVAL;
         plan->opt_rs_levels = (int)value;
+        return CN_OK;
+    case CN_OPT_PROFILE:
+        plan->opt_profile = value ? 1 : 0;
         return CN_OK;
     }
     return CN_EINVAL;
@@ -348,11 +360,47 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     return CN_OK;
 }
 
+// ---- profiling aid ---------------------------------------------------------------------------------------
+static int prof_begin(cn_plan *p, int kind, cudaStream_t stream)
+{
+    if (!p->opt_profile) return -1;
+    if (p->ev_used == p->ev_pool.size()) {
+        if (p->ev_pool.size() >= 8192) return -1; // enough samples; later launches go unbracketed
+        cn_plan::ev_pair e;
+        if (cudaEventCreate(&e.a) != cudaSuccess || cudaEventCreate(&e.b) != cudaSuccess) return -1;
+        p->ev_pool.push_back(e);
+    }
+    int i = (int)p->ev_used++;
+    p->ev_pool[i].kind = kind;
+    cudaEventRecord(p->ev_pool[i].a, stream);
+    return i;
+}
+static void prof_end(cn_plan *p, int i, cudaStream_t stream)
+{
+    if (i >= 0) cudaEventRecord(p->ev_pool[i].b, stream);
+}
+
+extern "C" cn_status cn_plan_get_profile(cn_plan *p, double *out)
+{
+    if (!p || !out) return CN_EINVAL;
+    out[0] = out[1] = out[2] = out[3] = 0.0;
+    for (size_t i = 0; i < p->ev_used; ++i) {
+        float ms = 0.f;
+        CN_CUDA(p, cudaEventSynchronize(p->ev_pool[i].b));
+        CN_CUDA(p, cudaEventElapsedTime(&ms, p->ev_pool[i].a, p->ev_pool[i].b));
+        out[2 * p->ev_pool[i].kind] += ms;
+        out[2 * p->ev_pool[i].kind + 1] += 1.0;
+    }
+    p->ev_used = 0;
+    return CN_OK;
+}
+
 // ---- one pass + RS ------------------------------------------------------------------------------------
 // mode 0: prologue (P2 only), 1: fused (P1 + P2), 2: epilogue (P1 only)
 static cn_status launch_pass(cn_plan *p, cplx *psi, int mode, int cur, cudaStream_t stream)
 {
     const cplx *supOld = p->sup[cur ^ 1], *supNew = p->sup[cur];
+    const int pi = (mode == 1) ? prof_begin(p, 0, stream) : -1;
     if (p->path == 2) {
         cn_tiled_params prm;
         prm.nchunks = p->N / 8;
@@ -381,6 +429,7 @@ static cn_status launch_pass(cn_plan *p, cplx *psi, int mode, int cur, cudaStrea
             k_pass_generic<true, false><<<grid, T, 0, stream>>>(g, p->rho, psi, p->q, p->gam, p->work, supOld, supNew,
                                                                p->slotD, p->slotU, p->sup[0]);
     }
+    prof_end(p, pi, stream);
     p->launches += 1;
     CN_CUDA(p, cudaGetLastError());
     return CN_OK;
@@ -390,7 +439,9 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
 {
     int T = p->opt_rs_threads;
     while (T > 32 && (int64_t)T / 2 >= p->P) T /= 2;
+    const int pi = prof_begin(p, 1, stream);
     k_rs_single<<<1, T, 0, stream>>>(p->P, p->slotD, p->slotU, p->lw, p->rq, p->uw, p->sup[out]);
+    prof_end(p, pi, stream);
     p->launches += 1;
     CN_CUDA(p, cudaGetLastError());
     return CN_OK;
