@@ -53,11 +53,16 @@ typedef enum {
     CN_OPT_PATH = 1,        /* 0 = auto (default), 1 = force the generic thread-per-block kernels,
                                2 = force the tiled TMA kernels (CN_EINVAL at factorize if the shape does not fit) */
     CN_OPT_TILE_THREADS = 2,/* threads per CTA of the tiled kernels: 0 = auto, else 64/128/256/512 (8 points per thread) */
-    CN_OPT_RS_THREADS = 3,  /* threads of the single-CTA reduced-system kernel (32..1024, power of two) */
+    CN_OPT_RS_TOPMAX = 3,   /* largest reduced system solved by the single-CTA RS kernel (1..8192, default 4096);
+                               a larger one is partitioned again into groups of 256 joint lines (next RS level) */
     CN_OPT_USE_GRAPH = 4,   /* 1 = replay the per-step launches from a CUDA graph inside cn_step (default 0) */
-    CN_OPT_RS_LEVELS = 5,   /* 0 = auto, 1 = single-CTA RS, 2 = two-level (nested, Eq. 6) RS */
-    CN_OPT_PROFILE = 6      /* 1 = bracket every fused-pass and RS launch of cn_step with CUDA events on the
+    CN_OPT_RS_LEVELS = 5,   /* 0 = auto (levels added while the system exceeds RS_TOPMAX), k >= 1 = exactly k nested
+                               levels where possible (Eq. 6; CN_EINVAL at factorize if the last
+                               level exceeds 8192 rows), -1 = paper-literal serial RS by one thread */
+    CN_OPT_PROFILE = 6,     /* 1 = bracket every fused-pass and RS launch of cn_step with CUDA events on the
                                launching stream (read back with cn_plan_get_profile); default 0 */
+    CN_OPT_PDL = 7          /* 1 (default) = launch the per-step kernels with programmatic dependent launch so that
+                               each kernel's independent prefetch overlaps the tail of its predecessor; 0 = plain */
 } cn_option;
 
 typedef struct {

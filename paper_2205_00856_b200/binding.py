@@ -14,7 +14,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(PKG, "libcn_nshape.so")
 
 CN_OK, CN_EINVAL, CN_ENOMEM, CN_ECUDA, CN_ENOTFACTORIZED, CN_EBREAKDOWN = range(6)
-CN_OPT_PATH, CN_OPT_TILE_THREADS, CN_OPT_RS_THREADS, CN_OPT_USE_GRAPH, CN_OPT_RS_LEVELS, CN_OPT_PROFILE = 1, 2, 3, 4, 5, 6
+CN_OPT_PATH, CN_OPT_TILE_THREADS, CN_OPT_RS_TOPMAX, CN_OPT_USE_GRAPH, CN_OPT_RS_LEVELS, CN_OPT_PROFILE, CN_OPT_PDL = 1, 2, 3, 4, 5, 6, 7
 PATH_AUTO, PATH_GENERIC, PATH_TILED = 0, 1, 2
 
 EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", "cn_factorize", "cn_step",
@@ -173,8 +173,9 @@ class Plan:
         if device_budget:
             cn_plan_set_device_budget(self.h, device_budget)
         for k, v in opts.items():
-            cn_plan_set_option(self.h, {"rs_threads": CN_OPT_RS_THREADS, "use_graph": CN_OPT_USE_GRAPH,
-                                        "rs_levels": CN_OPT_RS_LEVELS, "profile": CN_OPT_PROFILE}[k], v)
+            cn_plan_set_option(self.h, {"rs_topmax": CN_OPT_RS_TOPMAX, "use_graph": CN_OPT_USE_GRAPH,
+                                        "rs_levels": CN_OPT_RS_LEVELS, "profile": CN_OPT_PROFILE,
+                                        "pdl": CN_OPT_PDL}[k], v)
 
     def factorize(self, stream=None):
         cn_factorize(self.h, stream)

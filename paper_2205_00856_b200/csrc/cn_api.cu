@@ -28,13 +28,24 @@ struct cn_plan {
     double *dV = nullptr;
     cplx *q = nullptr;
     double *gam = nullptr;
-    cplx *lw = nullptr, *rq = nullptr, *uw = nullptr;
+    cplx *lw = nullptr, *rq = nullptr, *uw = nullptr; // LU factors of the LAST RS level
     cplx *slotD = nullptr, *slotU = nullptr, *sup[2] = {nullptr, nullptr};
     cplx *work = nullptr;
     int *derr = nullptr;
     size_t device_bytes = 0;
+    std::vector<void *> owned; // every device allocation of the factorization (freed by free_factors)
+    // RS levels: lv[0] is the reduced system on the P joint lines, lv[i+1] the reduced
+    // system of lv[i] partitioned into groups of CN_RS_G rows; the last level is solved by one CTA
+    struct rs_level {
+        int64_t n = 0;
+        cplx *sub = nullptr, *diag = nullptr, *sup = nullptr; // matrix of this level
+        cplx *l = nullptr, *rp = nullptr, *u = nullptr;       // group-local factors (all but the last level)
+        cplx *rD = nullptr, *rU = nullptr, *X = nullptr;      // two rhs slots per row, solution (levels >= 1)
+    };
+    std::vector<rs_level> lv;
     // configuration
-    int opt_path = 0, opt_tile_threads = 0, opt_rs_threads = 1024, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0;
+    int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0;
+    int opt_pdl = 1;
     // profiling (CN_OPT_PROFILE): event pairs around fused-pass (kind 0) and RS (kind 1) launches
     struct ev_pair { cudaEvent_t a, b; int kind; };
     std::vector<ev_pair> ev_pool;
@@ -44,6 +55,7 @@ struct cn_plan {
     bool factorized = false;
     int path = 0; // 1 generic, 2 tiled
     int tpb = 0, logc = 0;
+    int grid_tiled = 0; // persistent grid of the tiled pass kernel
     // tensor maps
     encode_tiled_fn encode = nullptr;
     CUtensorMap tmQ, tmGam, tmPsi;
@@ -76,14 +88,16 @@ static cn_status dev_alloc(cn_plan *p, T **ptr, size_t count)
         return (e == cudaErrorMemoryAllocation) ? CN_ENOMEM : CN_ECUDA;
     }
     p->device_bytes += bytes;
+    p->owned.push_back((void *)*ptr);
     return CN_OK;
 }
 
 static void free_factors(cn_plan *p)
 {
-    void *ptrs[] = {p->q, p->gam, p->lw, p->rq, p->uw, p->slotD, p->slotU, p->sup[0], p->sup[1], p->work, p->derr};
-    for (void *x : ptrs)
-        if (x) cudaFree(x);
+    for (void *x : p->owned) cudaFree(x);
+    p->owned.clear();
+    p->lv.clear();
+    p->device_bytes = p->dV ? sizeof(double) * (size_t)p->N : 0;
     p->q = nullptr; p->gam = nullptr; p->lw = p->rq = p->uw = nullptr;
     p->slotD = p->slotU = nullptr; p->sup[0] = p->sup[1] = nullptr; p->work = nullptr; p->derr = nullptr;
     p->factorized = false;
@@ -124,7 +138,8 @@ extern "C" cn_status cn_plan_create(cn_plan **out, int64_t N, int64_t P, double 
     p->rho = 4.0 * dx * dx / dt; // 1 / s
     p->two_dx2 = 2.0 * dx * dx;
     cn_status st = dev_alloc(p, &p->dV, (size_t)N);
-    if (st != CN_OK) { int e = p->last_cuda; delete p; (void)e; return st; }
+    if (st != CN_OK) { delete p; return st; }
+    p->owned.clear(); // V lives as long as the plan; `owned` lists what cn_factorize allocates
     // V may be a host or a device pointer; cudaMemcpyDefault resolves it (UVA)
     cudaError_t e = cudaMemcpy(p->dV, V, sizeof(double) * (size_t)N, cudaMemcpyDefault);
     if (e != cudaSuccess) { cudaFree(p->dV); delete p; return CN_ECUDA; }
@@ -167,16 +182,21 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
         plan->opt_tile_threads = (int)value;
         plan->factorized = false;
         return CN_OK;
-    case CN_OPT_RS_THREADS:
-        if (value < 32 || value > 1024 || (value & (value - 1))) return CN_EINVAL;
-        plan->opt_rs_threads = (int)value;
+    case CN_OPT_RS_TOPMAX:
+        if (value < 1 || value > 8 * CN_RS_TOP_THREADS) return CN_EINVAL;
+        plan->opt_rs_topmax = (int)value;
+        plan->factorized = false;
+        return CN_OK;
+    case CN_OPT_PDL:
+        plan->opt_pdl = value ? 1 : 0;
         return CN_OK;
     case CN_OPT_USE_GRAPH:
         plan->opt_graph = value ? 1 : 0;
         return CN_OK;
     case CN_OPT_RS_LEVELS:
-        if (value < 0 || value > 2) return CN_EINVAL;
+        if (value < -1 || value > 8) return CN_EINVAL;
         plan->opt_rs_levels = (int)value;
+        plan->factorized = false;
         return CN_OK;
     case CN_OPT_PROFILE:
         plan->opt_profile = value ? 1 : 0;
@@ -193,7 +213,7 @@ extern "C" cn_status cn_plan_get_info(const cn_plan *plan, cn_plan_info *info)
     info->path = plan->path;
     info->tile_threads = plan->tpb;
     info->tile_points = (int64_t)plan->tpb * 8;
-    info->rs_levels = 1;
+    info->rs_levels = (plan->opt_rs_levels < 0) ? -1 : (int32_t)plan->lv.size();
     info->out_of_core = 0;
     info->device_bytes = plan->device_bytes;
     info->launches = plan->launches;
@@ -311,9 +331,6 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     cn_status st;
     if ((st = dev_alloc(p, &p->q, (size_t)N)) != CN_OK) return st;
     if ((st = dev_alloc(p, &p->gam, (size_t)N)) != CN_OK) return st;
-    if ((st = dev_alloc(p, &p->lw, (size_t)P)) != CN_OK) return st;
-    if ((st = dev_alloc(p, &p->rq, (size_t)P)) != CN_OK) return st;
-    if ((st = dev_alloc(p, &p->uw, (size_t)P)) != CN_OK) return st;
     if ((st = dev_alloc(p, &p->slotD, (size_t)P)) != CN_OK) return st;
     if ((st = dev_alloc(p, &p->slotU, (size_t)P)) != CN_OK) return st;
     if ((st = dev_alloc(p, &p->sup[0], (size_t)P)) != CN_OK) return st;
@@ -322,11 +339,54 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     if (p->path == 1)
         if ((st = dev_alloc(p, &p->work, (size_t)N)) != CN_OK) return st;
 
-    // temporaries of the reduced matrix (freed below)
+    // RS levels: lv[0] has P rows; add levels of ceil(n / G) rows until the last one fits the single CTA
+    {
+        const int64_t topmax = (p->opt_rs_levels < 0) ? INT64_MAX : p->opt_rs_topmax;
+        int64_t n = P;
+        for (;;) {
+            cn_plan::rs_level L;
+            L.n = n;
+            p->lv.push_back(L);
+            const int nl = (int)p->lv.size();
+            const bool want_more = (p->opt_rs_levels > 0) ? (nl < p->opt_rs_levels) : (n > topmax);
+            if (!want_more || n <= 2) break;
+            n = (n + CN_RS_G - 1) / CN_RS_G;
+        }
+        if (p->opt_rs_levels >= 0 && p->lv.back().n > 8 * CN_RS_TOP_THREADS) return CN_EINVAL;
+    }
+    const int nlv = (int)p->lv.size();
+    for (int i = 0; i < nlv; ++i) {
+        cn_plan::rs_level &L = p->lv[i];
+        const size_t n = (size_t)L.n;
+        if ((st = dev_alloc(p, &L.sub, n)) != CN_OK) return st;
+        if ((st = dev_alloc(p, &L.diag, n)) != CN_OK) return st;
+        if ((st = dev_alloc(p, &L.sup, n)) != CN_OK) return st;
+        if (i < nlv - 1) {
+            if ((st = dev_alloc(p, &L.l, n)) != CN_OK) return st;
+            if ((st = dev_alloc(p, &L.rp, n)) != CN_OK) return st;
+            if ((st = dev_alloc(p, &L.u, n)) != CN_OK) return st;
+        }
+        if (i == 0) {
+            L.rD = p->slotD;
+            L.rU = p->slotU;
+        } else {
+            if ((st = dev_alloc(p, &L.rD, n)) != CN_OK) return st;
+            if ((st = dev_alloc(p, &L.rU, n)) != CN_OK) return st;
+            if ((st = dev_alloc(p, &L.X, n)) != CN_OK) return st;
+            CN_CUDA(p, cudaMemsetAsync(L.rU, 0, sizeof(cplx) * n, stream)); // rU[last] stays 0
+        }
+    }
+    const size_t ntop = (size_t)p->lv.back().n;
+    if ((st = dev_alloc(p, &p->lw, ntop)) != CN_OK) return st;
+    if ((st = dev_alloc(p, &p->rq, ntop)) != CN_OK) return st;
+    if ((st = dev_alloc(p, &p->uw, ntop)) != CN_OK) return st;
+
+    // temporaries of the factorization (freed below)
     cplx *red = nullptr;
-    CN_CUDA(p, cudaMalloc((void **)&red, sizeof(cplx) * 4 * (size_t)P));
+    CN_CUDA(p, cudaMalloc((void **)&red, sizeof(cplx) * 6 * (size_t)P));
     cplx *redSubD = red, *redDiagD = red + P, *redSupU = red + 2 * P, *redDiagU = red + 3 * P;
-    CN_CUDA(p, cudaMemsetAsync(red, 0, sizeof(cplx) * 4 * (size_t)P, stream));
+    cplx *tmpA = red + 4 * P, *tmpB = red + 5 * P;
+    CN_CUDA(p, cudaMemsetAsync(red, 0, sizeof(cplx) * 6 * (size_t)P, stream));
     CN_CUDA(p, cudaMemsetAsync(p->derr, 0, sizeof(int), stream));
     CN_CUDA(p, cudaMemsetAsync(p->slotU, 0, sizeof(cplx) * (size_t)P, stream));
 
@@ -334,9 +394,21 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     const int T = 128;
     k_factor_blocks<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(g, p->two_dx2, p->rho, p->dV, p->q, p->gam, redSubD,
                                                                   redDiagD, redSupU, redDiagU, p->derr);
-    k_factor_reduced<<<1, 32, 0, stream>>>(g, p->rho, p->gam, redSubD, redDiagD, redSupU, redDiagU, p->lw, p->rq, p->uw,
-                                           p->derr);
+    k_rs_assemble0<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(P, N, p->rho, p->gam, redSubD, redDiagD, redSupU,
+                                                                 redDiagU, p->lv[0].sub, p->lv[0].diag, p->lv[0].sup);
     p->launches += 2;
+    for (int i = 0; i + 1 < nlv; ++i) {
+        cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
+        k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, tmpA,
+                                                                         U.sub, U.diag, tmpB, U.sup, p->derr);
+        k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB);
+        p->launches += 2;
+    }
+    {
+        cn_plan::rs_level &L = p->lv.back();
+        k_rs_factor_top<<<1, 32, 0, stream>>>(L.n, L.sub, L.diag, L.sup, p->lw, p->rq, p->uw, p->derr);
+        p->launches += 1;
+    }
     int herr = 0;
     cudaError_t e = cudaMemcpyAsync(&herr, p->derr, sizeof(int), cudaMemcpyDeviceToHost, stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
@@ -354,7 +426,18 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
             if (!k) return CN_EINVAL;
             CN_CUDA(p, cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             (int)tiled_smem(p->tpb)));
+            CN_CUDA(p, cudaFuncSetAttribute((const void *)k, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
         }
+        // persistent grid: one CTA per resident slot (148 SMs x resident CTAs per SM), never more than tiles
+        int dev = 0, sms = 0, per_sm = 0;
+        CN_CUDA(p, cudaGetDevice(&dev));
+        CN_CUDA(p, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        CN_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)tiled_kernel(p->tpb, p->logc, 1),
+                                                                 p->tpb, tiled_smem(p->tpb)));
+        if (per_sm < 1) return CN_ECUDA;
+        const int64_t tiles = (N / 8 + p->tpb - 1) / p->tpb;
+        const int64_t slots = (int64_t)sms * per_sm;
+        p->grid_tiled = (int)(tiles < slots ? tiles : slots);
     }
     p->factorized = true;
     return CN_OK;
@@ -396,11 +479,31 @@ extern "C" cn_status cn_plan_get_profile(cn_plan *p, double *out)
 }
 
 // ---- one pass + RS ------------------------------------------------------------------------------------
+// every kernel of the per-step chain goes through here; pdl = programmatic stream serialization (cn_common.cuh)
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_k(void (*k)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t stream,
+                            bool pdl, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, k, args...);
+}
+
 // mode 0: prologue (P2 only), 1: fused (P1 + P2), 2: epilogue (P1 only)
 static cn_status launch_pass(cn_plan *p, cplx *psi, int mode, int cur, cudaStream_t stream)
 {
     const cplx *supOld = p->sup[cur ^ 1], *supNew = p->sup[cur];
     const int pi = (mode == 1) ? prof_begin(p, 0, stream) : -1;
+    const bool pdl = p->opt_pdl && mode != 0 && !p->opt_profile;
+    cudaError_t e;
     if (p->path == 2) {
         cn_tiled_params prm;
         prm.nchunks = p->N / 8;
@@ -413,37 +516,65 @@ static cn_status launch_pass(cn_plan *p, cplx *psi, int mode, int cur, cudaStrea
         prm.slotU = p->slotU;
         prm.supInit = p->sup[0];
         tiled_kernel_t k = tiled_kernel(p->tpb, p->logc, mode);
-        const int64_t tiles = (prm.nchunks + p->tpb - 1) / p->tpb;
-        k<<<(unsigned)tiles, p->tpb, tiled_smem(p->tpb), stream>>>(p->tmPsi, p->tmQ, p->tmGam, prm);
+        e = launch_k(k, (unsigned)p->grid_tiled, (unsigned)p->tpb, tiled_smem(p->tpb), stream, pdl, p->tmPsi, p->tmQ,
+                     p->tmGam, prm);
     } else {
         cn_geom g{p->N, p->P};
         const int T = 64;
         const unsigned grid = (unsigned)((p->P + T - 1) / T);
-        if (mode == 0)
-            k_pass_generic<false, true><<<grid, T, 0, stream>>>(g, p->rho, psi, p->q, p->gam, p->work, supOld, supNew,
-                                                               p->slotD, p->slotU, p->sup[0]);
-        else if (mode == 1)
-            k_pass_generic<true, true><<<grid, T, 0, stream>>>(g, p->rho, psi, p->q, p->gam, p->work, supOld, supNew,
-                                                              p->slotD, p->slotU, p->sup[0]);
-        else
-            k_pass_generic<true, false><<<grid, T, 0, stream>>>(g, p->rho, psi, p->q, p->gam, p->work, supOld, supNew,
-                                                               p->slotD, p->slotU, p->sup[0]);
+        auto k = (mode == 0) ? k_pass_generic<false, true> : (mode == 1 ? k_pass_generic<true, true> : k_pass_generic<true, false>);
+        e = launch_k(k, grid, T, 0, stream, pdl, g, p->rho, psi, (const cplx *)p->q, (const double *)p->gam, p->work,
+                     supOld, supNew, p->slotD, p->slotU, p->sup[0]);
     }
     prof_end(p, pi, stream);
     p->launches += 1;
-    CN_CUDA(p, cudaGetLastError());
+    if (e != cudaSuccess) return cuda_fail(p, e);
     return CN_OK;
 }
 
+template <int K>
+static cudaError_t launch_top_k(cn_plan *p, const cn_plan::rs_level &L, cplx *X, cudaStream_t stream, bool pdl)
+{
+    int T = CN_RS_TOP_THREADS;
+    while (T > 32 && (int64_t)(T / 2) * K >= L.n) T /= 2;
+    return launch_k(k_rs_top<K>, 1u, (unsigned)T, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU,
+                    (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw, X);
+}
+
+// RS of one step: (RD+RU+JD+JU) level by level, RS of the last level, SS level by level (Eq. 6)
 static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
 {
-    int T = p->opt_rs_threads;
-    while (T > 32 && (int64_t)T / 2 >= p->P) T /= 2;
+    const bool pdl = p->opt_pdl && !p->opt_profile;
+    const int nlv = (int)p->lv.size();
     const int pi = prof_begin(p, 1, stream);
-    k_rs_single<<<1, T, 0, stream>>>(p->P, p->slotD, p->slotU, p->lw, p->rq, p->uw, p->sup[out]);
+    cudaError_t e = cudaSuccess;
+    p->lv[0].X = p->sup[out];
+    for (int i = 0; i + 1 < nlv && e == cudaSuccess; ++i) {
+        const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
+        e = launch_k(k_rs_reduce, (unsigned)U.n, (unsigned)CN_RS_G, 0, stream, pdl, L.n, (const cplx *)L.rD,
+                     (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
+                     (const cplx *)L.sup, U.rD, U.rU);
+        p->launches += 1;
+    }
+    if (e == cudaSuccess) {
+        const cn_plan::rs_level &L = p->lv.back();
+        if (p->opt_rs_levels < 0)
+            e = launch_k(k_rs_serial, 1u, 32u, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU,
+                         (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw, L.X);
+        else if (L.n <= CN_RS_TOP_THREADS) e = launch_top_k<1>(p, L, L.X, stream, pdl);
+        else if (L.n <= 2 * CN_RS_TOP_THREADS) e = launch_top_k<2>(p, L, L.X, stream, pdl);
+        else if (L.n <= 4 * CN_RS_TOP_THREADS) e = launch_top_k<4>(p, L, L.X, stream, pdl);
+        else e = launch_top_k<8>(p, L, L.X, stream, pdl);
+        p->launches += 1;
+    }
+    for (int i = nlv - 2; i >= 0 && e == cudaSuccess; --i) {
+        const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
+        e = launch_k(k_rs_subst, (unsigned)U.n, (unsigned)CN_RS_G, 0, stream, pdl, L.n, (const cplx *)L.rD,
+                     (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X);
+        p->launches += 1;
+    }
     prof_end(p, pi, stream);
-    p->launches += 1;
-    CN_CUDA(p, cudaGetLastError());
+    if (e != cudaSuccess) return cuda_fail(p, e);
     return CN_OK;
 }
 

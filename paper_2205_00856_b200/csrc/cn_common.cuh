@@ -54,6 +54,14 @@ CN_DEVINL cplx rhs_E(double gamma, double rho, cplx p, cplx lo, cplx hi)
     return make_double2(er, ei);
 }
 
+// Programmatic dependent launch (sm_90+): every kernel of the per-step chain is launched with
+// programmatic stream serialization, fetches what does not depend on its predecessor, then waits for the
+// predecessor to COMPLETE (memory flushed) with pdl_wait().  Because every kernel of the chain executes
+// pdl_wait() before it finishes, completion is transitive: after pdl_wait() all earlier kernels are done.
+// Without the launch attribute both instructions are no-ops.
+CN_DEVINL void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+CN_DEVINL void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 CN_DEVINL cplx shfl_up_c(cplx v, int d)
 {
     return make_double2(__shfl_up_sync(0xffffffffu, v.x, d), __shfl_up_sync(0xffffffffu, v.y, d));

@@ -20,6 +20,8 @@ __global__ void k_pass_generic(cn_geom g, double rho, cplx *__restrict__ psi, co
                                const cplx *__restrict__ supOld, const cplx *__restrict__ supNew,
                                cplx *__restrict__ slotD, cplx *__restrict__ slotU, cplx *__restrict__ supInit)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= g.P) return;
     const int64_t f = g.off(w), J = g.off(w + 1) - 1;

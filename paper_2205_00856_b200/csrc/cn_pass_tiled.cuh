@@ -80,14 +80,16 @@ CN_DEVINL void tma_store_commit_wait()
 }
 CN_DEVINL void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// shared-memory bytes of one CTA
+// shared-memory bytes of one CTA: one in-flight input tile (psi, q, gamma), one output staging tile, scan scratch
 template <int TPB>
 constexpr size_t tiled_smem_bytes()
 {
-    return 1024 /*alignment slack*/ + (size_t)TPB * (128 + 128 + 64) + 2 * 2 * 32 * sizeof(cplx) + 4 * 32 * sizeof(cplx) + 64;
+    return (size_t)TPB * (128 + 128 + 64 + 128) + (size_t)(TPB / 32) * (2 * 2 + 2) * sizeof(cplx) + 16;
 }
 
-// TPB threads, 8 points per thread, 2^LOGC chunks (threads) per block.
+// TPB threads, 8 points per thread, 2^LOGC chunks (threads) per block.  PERSISTENT: CTA b handles tiles
+// b, b + gridDim.x, ...; the TMA loads of the next tile are issued as soon as the current tile has been
+// copied to registers, so they overlap the whole computation of the current tile.
 template <int TPB, int LOGC, bool P1, bool P2, int MINB>
 __global__ void __launch_bounds__(TPB, MINB)
 k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ CUtensorMap tmQ,
@@ -97,232 +99,256 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
     constexpr bool XWARP = (LOGC > 5);      // a block spans several warps
     constexpr int WSTEPS = XWARP ? 5 : LOGC; // shuffle-scan steps inside a warp
     constexpr int NW = TPB / 32;
+    constexpr int WPB = XWARP ? (CPB / 32) : 1; // warps per block
     static_assert(CPB <= TPB, "a block must fit in one tile");
 
-    extern __shared__ uint8_t smem_raw[];
-    uint8_t *base = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-    cplx *s_psi = (cplx *)base;
-    cplx *s_q = (cplx *)(base + (size_t)TPB * 128);
-    double2 *s_g = (double2 *)(base + (size_t)TPB * 256);
-    cplx *s_scan = (cplx *)(base + (size_t)TPB * 320);        // [2 buffers][A,B][32]
-    cplx *s_edge = s_scan + 2 * 2 * 32;                        // [4][32] edge exchange between warps
-    uint64_t *bar = (uint64_t *)(s_edge + 4 * 32);
+    extern __shared__ __align__(1024) uint8_t smem[];
+    cplx *const s_psi = (cplx *)smem;
+    cplx *const s_q = (cplx *)(smem + (size_t)TPB * 128);
+    double2 *const s_g = (double2 *)(smem + (size_t)TPB * 256);
+    cplx *const s_out = (cplx *)(smem + (size_t)TPB * 320);
+    cplx *const s_scan = (cplx *)(smem + (size_t)TPB * 448); // [2 buffers][A,B][NW]
+    cplx *const s_edge = s_scan + 2 * 2 * NW;                // [2][NW] edge exchange between warps
+    uint64_t *const bar = (uint64_t *)(s_edge + 2 * NW);
 
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    const int64_t row0 = (int64_t)blockIdx.x * TPB;
-    const int64_t c = row0 + t; // global chunk index
-    const bool active = c < prm.nchunks;
-    const bool isFirst = (c & (CPB - 1)) == 0;
-    const bool isLast = (c & (CPB - 1)) == CPB - 1;
-    const int64_t w = c >> LOGC;
     const double rho = prm.rho;
     const cplx zero = cmake(0.0, 0.0);
+    const int64_t ntiles = (prm.nchunks + TPB - 1) / TPB;
 
-    if (t == 0) {
-        mbar_init(bar, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncthreads();
-    if (t == 0) {
+    auto issue_loads = [&](int64_t tile) {
+        const int64_t r0 = tile * TPB;
         mbar_expect_tx(bar, (uint32_t)(TPB * 320));
 #pragma unroll
         for (int r = 0; r < TPB; r += 256) {
-            const int rows = (TPB - r < 256) ? (TPB - r) : 256;
-            (void)rows;
-            tma_load_2d((uint8_t *)s_psi + (size_t)r * 128, &tmPsi, bar, 0, (int)(row0 + r));
-            tma_load_2d((uint8_t *)s_q + (size_t)r * 128, &tmQ, bar, 0, (int)(row0 + r));
-            tma_load_2d((uint8_t *)s_g + (size_t)r * 64, &tmGam, bar, 0, (int)(row0 + r));
+            tma_load_2d((uint8_t *)s_psi + (size_t)r * 128, &tmPsi, bar, 0, (int)(r0 + r));
+            tma_load_2d((uint8_t *)s_q + (size_t)r * 128, &tmQ, bar, 0, (int)(r0 + r));
+            tma_load_2d((uint8_t *)s_g + (size_t)r * 64, &tmGam, bar, 0, (int)(r0 + r));
         }
+    };
+
+    if (t == 0) {
+        if ((smem_u32(smem) & 1023u) != 0) __trap(); // the swizzle patterns below assume a 1 KiB aligned base
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        if ((int64_t)blockIdx.x < ntiles) issue_loads(blockIdx.x); // psi: written two kernels ago, complete
     }
-    // while the tile is in flight: the few values that live on the joint lines
-    cplx supN = zero;      // new value of the own joint line (last chunk of a block)
-    cplx jointAbove = zero; // new value of the joint line above the block of this thread
-    if (active) {
-        if (P1) {
+    pdl_wait();              // the RS kernel before this one has delivered supNew
+    pdl_launch_dependents(); // the next RS kernel may become resident as soon as CTAs retire
+    __syncthreads();
+
+    uint32_t phase = 0;
+    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int64_t row0 = tile * TPB;
+        const int64_t c = row0 + t; // global chunk index
+        const bool active = c < prm.nchunks;
+        const bool isFirst = (c & (CPB - 1)) == 0;
+        const bool isLast = (c & (CPB - 1)) == CPB - 1;
+        const int64_t w = c >> LOGC;
+
+        // the few values that live on the joint lines (issued before waiting for the tile)
+        cplx supN = zero;       // new value of the own joint line (last chunk of a block)
+        cplx jointAbove = zero; // new value of the joint line above the block of this thread
+        if (P1 && active) {
             if (isLast) supN = prm.supNew[w];
             if (w > 0) jointAbove = prm.supNew[w - 1];
         }
-    }
-    cplx oldAbove = zero; // OLD psi just above the tile (needed by thread 0 only)
-    if (t == 0 && c > 0) oldAbove = P1 ? prm.supOld[w - 1] : prm.psi_raw[8 * c - 1];
+        cplx oldAbove = zero; // OLD psi just above the tile (needed by thread 0 only)
+        if (t == 0 && c > 0) oldAbove = P1 ? prm.supOld[w - 1] : prm.psi_raw[8 * c - 1];
 
-    mbar_wait(bar, 0);
+        mbar_wait(bar, phase);
+        phase ^= 1;
 
-    // ---- registers <- swizzled shared memory ----------------------------------------------------------
-    cplx v[8], qv[8];
-    double g[8];
-    const int sw = t & 7;
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-        v[j] = s_psi[t * 8 + (j ^ sw)];
-        qv[j] = s_q[t * 8 + (j ^ sw)];
-    }
-    const int sg = (t >> 1) & 3;
-#pragma unroll
-    for (int jj = 0; jj < 4; ++jj) {
-        double2 gg = s_g[t * 4 + (jj ^ sg)];
-        g[2 * jj] = gg.x;
-        g[2 * jj + 1] = gg.y;
-    }
-    cplx vlo, vhi, qm1;
-    if (t > 0) {
-        vlo = s_psi[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
-        qm1 = s_q[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
-    } else {
-        vlo = oldAbove;
-        qm1 = cmake(1.0, 0.0); // the row above a tile is a joint line (or the virtual one)
-    }
-    vhi = (t < TPB - 1) ? s_psi[(t + 1) * 8 + ((t + 1) & 7)] : zero;
-    if (!P1 && isFirst) jointAbove = vlo; // prologue: psi^0 of the joint above
-
-    // chunk multipliers: Qp = prod_{j<7} (-q_j);  RD map A = (-q_{-1}) Qp,  RU map A = Qp (-q_7)
-    cplx Qp = cneg(qv[0]);
-#pragma unroll
-    for (int j = 1; j < 7; ++j) Qp = cmul(Qp, cneg(qv[j]));
-    const cplx fwdA = isLast ? zero : cmul(cneg(qm1), Qp);
-    const cplx bwdA = isLast ? zero : cmul(Qp, cneg(qv[7]));
-
-    // exclusive inflow of a forward (RD) chain; tin = value on the joint line above the block
-    auto scan_fwd = [&](cplx A, cplx B, cplx tin, int buf) -> cplx {
-        warp_scan_affine<+1, WSTEPS>(A, B, lane);
-        cplx carry = tin;
-        if (XWARP) {
-            cplx *sA = s_scan + buf * 64, *sB = sA + 32;
-            if (lane == 31) {
-                sA[warp] = A;
-                sB[warp] = B;
-            }
-            __syncthreads();
-            const int vb = warp & ~((CPB / 32) - 1); // first warp of this block
-            for (int u = vb; u < warp; ++u) carry = cfma(sA[u], carry, sB[u]);
-        }
-        cplx Ae = shfl_up_c(A, 1), Be = shfl_up_c(B, 1);
-        return (lane == 0) ? carry : cfma(Ae, carry, Be);
-    };
-    // exclusive inflow of a backward (RU) chain; nothing enters a block from below (joint resets)
-    auto scan_bwd = [&](cplx A, cplx B, int buf) -> cplx {
-        warp_scan_affine<-1, WSTEPS>(A, B, lane);
-        cplx carry = zero;
-        if (XWARP) {
-            cplx *sA = s_scan + buf * 64, *sB = sA + 32;
-            if (lane == 0) {
-                sA[warp] = A;
-                sB[warp] = B;
-            }
-            __syncthreads();
-            const int ve = (warp & ~((CPB / 32) - 1)) + (CPB / 32) - 1; // last warp of this block
-            for (int u = ve; u > warp; --u) carry = cfma(sA[u], carry, sB[u]);
-        }
-        cplx Ae = shfl_down_c(A, 1), Be = shfl_down_c(B, 1);
-        return (lane == 31) ? carry : cfma(Ae, carry, Be);
-    };
-
-    if (P1) {
-        // ---- Eq. 3 fused into RD ----------------------------------------------------
-        cplx E[8];
+        // ---- registers <- swizzled shared memory ------------------------------------------------------
+        cplx v[8], qv[8];
+        double g[8];
+        const int sw = t & 7;
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-            cplx lo = (j == 0) ? vlo : v[j - 1];
-            cplx hi = (j == 7) ? vhi : v[j + 1];
-            E[j] = rhs_E(g[j], rho, v[j], lo, hi);
+            v[j] = s_psi[t * 8 + (j ^ sw)];
+            qv[j] = s_q[t * 8 + (j ^ sw)];
         }
-        if (isLast) E[7] = supN; // the joint line carries its new support value
-        cplx D = zero;
+        const int sg = (t >> 1) & 3;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
-        if (isLast) D = supN;
-        cplx in = scan_fwd(fwdA, D, jointAbove, 0);
-        D = in;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
-            E[j] = D; // E now holds d after RD
+        for (int jj = 0; jj < 4; ++jj) {
+            double2 gg = s_g[t * 4 + (jj ^ sg)];
+            g[2 * jj] = gg.x;
+            g[2 * jj + 1] = gg.y;
         }
-        // ---- RU + SS: x_j = q_j (d_j - x_{j+1}) ---------------------------------------------------------
-        cplx X = zero;
-#pragma unroll
-        for (int j = 7; j >= 0; --j) {
-            X = cmul(qv[j], csub(E[j], X));
-            if (j == 7 && isLast) X = supN;
+        cplx vlo = oldAbove, vhi = zero, qm1 = cmake(1.0, 0.0); // the row above a tile is a joint line
+        if (t > 0) {
+            vlo = s_psi[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
+            qm1 = s_q[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
         }
-        cplx xin = scan_bwd(bwdA, X, 1);
-        X = xin;
-#pragma unroll
-        for (int j = 7; j >= 0; --j) {
-            X = cmul(qv[j], csub(E[j], X));
-            if (j == 7 && isLast) X = supN;
-            v[j] = X;
-        }
-    }
+        if (t < TPB - 1) vhi = s_psi[(t + 1) * 8 + ((t + 1) & 7)];
+        if (!P1 && isFirst) jointAbove = vlo; // prologue: psi^0 of the joint above
 
-    if (P1) {
-        // the old psi in shared memory has been read by everybody (halo reads above): overwrite with the new
+        // everybody has its copy: refill the input buffers with the next tile while this one is computed
         __syncthreads();
-#pragma unroll
-        for (int j = 0; j < 8; ++j) s_psi[t * 8 + (j ^ sw)] = v[j];
-        fence_proxy_async();
-        __syncthreads();
-        if (t == 0) {
-#pragma unroll
-            for (int r = 0; r < TPB; r += 256) tma_store_2d(&tmPsi, (uint8_t *)s_psi + (size_t)r * 128, 0, (int)(row0 + r));
-            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-        }
-    }
+        if (t == 0 && tile + gridDim.x < ntiles) issue_loads(tile + gridDim.x);
 
-    if (P2) {
-        // ---- neighbours of the NEW psi ----------------------------------------------------------------
-        cplx xlo = shfl_up_c(v[7], 1), xhi = shfl_down_c(v[0], 1);
-        if (XWARP) {
-            cplx *eLo = s_edge, *eHi = s_edge + 32;
-            if (lane == 31) eLo[warp] = v[7];
-            if (lane == 0) eHi[warp] = v[0];
+        // chunk multipliers: Qp = prod_{j<7} (-q_j);  RD map A = (-q_{-1}) Qp,  RU map A = Qp (-q_7)
+        cplx Qp = cneg(qv[0]);
+#pragma unroll
+        for (int j = 1; j < 7; ++j) Qp = cmul(Qp, cneg(qv[j]));
+        const cplx fwdA = isLast ? zero : cmul(cneg(qm1), Qp);
+        const cplx bwdA = isLast ? zero : cmul(Qp, cneg(qv[7]));
+
+        // exclusive inflow of a forward (RD) chain; tin = value on the joint line above the block.
+        // Across the warps of one block the per-warp maps are composed by a second shuffle scan that every
+        // warp of the block runs redundantly on the WPB aggregates (no serial chain, one barrier).
+        auto scan_fwd = [&](cplx A, cplx B, cplx tin, int buf) -> cplx {
+            warp_scan_affine<+1, WSTEPS>(A, B, lane);
+            cplx carry = tin;
+            if (XWARP) {
+                cplx *sA = s_scan + buf * 2 * NW, *sB = sA + NW;
+                if (lane == 31) {
+                    sA[warp] = A;
+                    sB[warp] = B;
+                }
+                __syncthreads();
+                const int vb = warp & ~(WPB - 1); // first warp of this block
+                cplx wA = cmake(1.0, 0.0), wB = zero;
+                if (lane < WPB) {
+                    wA = sA[vb + lane];
+                    wB = sB[vb + lane];
+                }
+                warp_scan_affine<+1, (LOGC > 5 ? LOGC - 5 : 0)>(wA, wB, lane);
+                const int src = warp - vb - 1; // composite of warps vb .. warp-1
+                cplx cA = shfl_c(wA, src < 0 ? 0 : src), cB = shfl_c(wB, src < 0 ? 0 : src);
+                if (src >= 0) carry = cfma(cA, tin, cB);
+            }
+            cplx Ae = shfl_up_c(A, 1), Be = shfl_up_c(B, 1);
+            cplx r = cfma(Ae, carry, Be);
+            return (lane == 0) ? carry : r;
+        };
+        // exclusive inflow of a backward (RU) chain; nothing enters a block from below (joint resets)
+        auto scan_bwd = [&](cplx A, cplx B, int buf) -> cplx {
+            warp_scan_affine<-1, WSTEPS>(A, B, lane);
+            cplx carry = zero;
+            if (XWARP) {
+                cplx *sA = s_scan + buf * 2 * NW, *sB = sA + NW;
+                if (lane == 0) {
+                    sA[warp] = A;
+                    sB[warp] = B;
+                }
+                __syncthreads();
+                const int vb = warp & ~(WPB - 1);
+                cplx wA = cmake(1.0, 0.0), wB = zero;
+                if (lane < WPB) {
+                    wA = sA[vb + lane];
+                    wB = sB[vb + lane];
+                }
+                warp_scan_affine<-1, (LOGC > 5 ? LOGC - 5 : 0)>(wA, wB, lane);
+                const int src = warp - vb + 1; // composite of warps warp+1 .. last, applied to 0
+                cplx cB = shfl_c(wB, src > 31 ? 31 : src);
+                if (src < WPB) carry = cB;
+            }
+            cplx Ae = shfl_down_c(A, 1), Be = shfl_down_c(B, 1);
+            cplx r = cfma(Ae, carry, Be);
+            return (lane == 31) ? carry : r;
+        };
+
+        if (P1) {
+            // ---- Eq. 3 fused into RD -------------------------------------------------
+            cplx E[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                cplx lo = (j == 0) ? vlo : v[j - 1];
+                cplx hi = (j == 7) ? vhi : v[j + 1];
+                E[j] = rhs_E(g[j], rho, v[j], lo, hi);
+            }
+            cplx D = zero;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
+            if (isLast) D = supN; // the joint line carries its new support value
+            cplx in = scan_fwd(fwdA, D, jointAbove, 0);
+            D = in;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
+                E[j] = D; // E now holds d after RD
+            }
+            // ---- RU + SS: x_j = q_j (d_j - x_{j+1}) -----------------------------------------------------
+            cplx X = cmul(qv[7], E[7]);
+            if (isLast) X = supN;
+#pragma unroll
+            for (int j = 6; j >= 0; --j) X = cmul(qv[j], csub(E[j], X));
+            cplx xin = scan_bwd(bwdA, X, 1);
+            X = cmul(qv[7], csub(E[7], xin));
+            if (isLast) X = supN;
+            v[7] = X;
+#pragma unroll
+            for (int j = 6; j >= 0; --j) {
+                X = cmul(qv[j], csub(E[j], X));
+                v[j] = X;
+            }
+            // ---- new psi -> swizzled staging tile -> one TMA tensor store ---------------------------------
+            if (t == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); // previous store drained
             __syncthreads();
-            if (lane == 0 && warp > 0) xlo = eLo[warp - 1];
-            if (lane == 31 && warp < NW - 1) xhi = eHi[warp + 1];
-        }
-        if (isFirst) xlo = jointAbove; // also covers lane 0 when blocks do not span warps
-        cplx E[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            cplx lo = (j == 0) ? xlo : v[j - 1];
-            cplx hi = (j == 7) ? (isLast ? zero : xhi) : v[j + 1];
-            E[j] = rhs_E(g[j], rho, v[j], lo, hi);
-        }
-        const cplx EJ = E[7]; // for a last chunk: E of the joint line without its psi_{J+1} term (JD part)
-        if (isLast) E[7] = zero;
-        cplx D = zero;
+            for (int j = 0; j < 8; ++j) s_out[t * 8 + (j ^ sw)] = v[j];
+            fence_proxy_async();
+            __syncthreads();
+            if (t == 0) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
-        if (isLast) D = zero;
-        cplx in = scan_fwd(fwdA, D, zero, 1);
-        D = in;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
-            E[j] = D;
-        }
-        cplx Y = zero, yn = zero;
-#pragma unroll
-        for (int j = 7; j >= 0; --j) {
-            Y = cmul(qv[j], csub(E[j], Y));
-            if (j == 7 && isLast) Y = zero;
-            if (j == 6) yn = Y; // local solution next to the own joint (meaningful for a last chunk)
-        }
-        cplx yin = scan_bwd(bwdA, Y, 0);
-        if (active) {
-            if (isLast) {
-                prm.slotD[w] = csub(EJ, yn);
-                if (w == prm.P - 1) prm.slotU[w] = zero;
-                if (!P1) prm.supInit[w] = v[7];
-            }
-            if (isFirst && w > 0) {
-                cplx y0 = cfma(bwdA, yin, Y); // isLast && isFirst: bwdA = 0 and Y is already exact
-                prm.slotU[w - 1] = cneg(cadd(v[0], y0));
+                for (int r = 0; r < TPB; r += 256)
+                    tma_store_2d(&tmPsi, (uint8_t *)s_out + (size_t)r * 128, 0, (int)(row0 + r));
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
             }
         }
-    }
 
-    if (P1) {
-        if (t == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        if (P2) {
+            // ---- neighbours of the NEW psi ------------------------------------------------------------
+            cplx xlo = shfl_up_c(v[7], 1), xhi = shfl_down_c(v[0], 1);
+            if (XWARP) {
+                cplx *eLo = s_edge, *eHi = s_edge + NW;
+                if (lane == 31) eLo[warp] = v[7];
+                if (lane == 0) eHi[warp] = v[0];
+                __syncthreads();
+                if (lane == 0 && warp > 0) xlo = eLo[warp - 1];
+                if (lane == 31 && warp < NW - 1) xhi = eHi[warp + 1];
+            }
+            if (isFirst) xlo = jointAbove; // also covers lane 0 when blocks do not span warps
+            if (isLast) xhi = zero;
+            cplx E[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                cplx lo = (j == 0) ? xlo : v[j - 1];
+                cplx hi = (j == 7) ? xhi : v[j + 1];
+                E[j] = rhs_E(g[j], rho, v[j], lo, hi);
+            }
+            const cplx EJ = E[7]; // for a last chunk: E of the joint line without its psi_{J+1} term (JD part)
+            cplx D = zero;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
+            if (isLast) D = zero;
+            cplx in = scan_fwd(fwdA, D, zero, 1);
+            D = in;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
+                E[j] = D;
+            }
+            cplx Y = cmul(qv[7], E[7]);
+            if (isLast) Y = zero;
+            Y = cmul(qv[6], csub(E[6], Y));
+            const cplx yn = Y; // local solution next to the own joint (meaningful for a last chunk)
+#pragma unroll
+            for (int j = 5; j >= 0; --j) Y = cmul(qv[j], csub(E[j], Y));
+            cplx yin = scan_bwd(bwdA, Y, 0);
+            if (active) {
+                if (isLast) {
+                    prm.slotD[w] = csub(EJ, yn);
+                    if (w == prm.P - 1) prm.slotU[w] = zero;
+                    if (!P1) prm.supInit[w] = v[7];
+                }
+                if (isFirst && w > 0) {
+                    cplx y0 = cfma(bwdA, yin, Y); // isLast && isFirst: bwdA = 0 and Y is already exact
+                    prm.slotU[w - 1] = cneg(cadd(v[0], y0));
+                }
+            }
+        }
     }
+    if (P1 && t == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }

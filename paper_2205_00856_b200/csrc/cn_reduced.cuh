@@ -1,74 +1,313 @@
 // RS stage: solve the reduced tridiagonal system on the joint lines.
 //
 // The paper solves it serially ("implemented serially", beta * n_bl in its model) and
-// notes that it can itself be parallelised.  Here the pre-factored system is
-// solved by ONE CTA: every thread owns a contiguous chunk of joint lines, sweeps it serially, and the
-// chunks are chained by the affine-map scan of cn_common.cuh, so the serial depth is P / threads.
+// notes that the reduced system can itself be solved by the same partition method, level after level
+// (Eq. 6:  N[M_0] = sum (RD+RU+JU+JD)[M_i] + RS[M_last] + sum SS[M_i]).
+// Here:
+//   * k_rs_top<K>     -- RS[M_last]: the pre-factored system of the last level is solved by ONE CTA;
+//                        every thread owns K consecutive rows held in registers, the threads are chained
+//                        by the affine-map scan of cn_common.cuh (serial depth K instead of n).
+//   * k_rs_reduce     -- (RD+RU+JD+JU)[M_i], i >= 1, d-side only: one CTA per group of G joint lines of
+//                        level i, one row per thread; emits two slots per joint line of level i+1.
+//   * k_rs_subst      -- SS[M_i], i >= 1: one CTA per group, given the two support values of level i+1.
+//   * k_rs_serial     -- the paper-literal variant (one thread, plain Thomas on the joint lines), kept
+//                        for the P sweep (CN_OPT_RS_LEVELS = -1).
+// All matrix-side quantities (local pivots, fill-in, the next level's matrix) are produced once by the
+// factor kernels at the end of this file.
+//
+// A level is a general complex tridiagonal system (sub_i, diag_i, sup_i), i = 0..n-1.  Group g owns rows
+// [g G, min((g+1) G, n)); its LAST row is the joint line of the next level, the rows before it are its
+// interior.  Stored per interior row:  l_i = sub_i * rp_{i-1}  (rp := 1 above the first interior row, so
+// that "D above the group := support value of the joint above" works as in the pass kernels),
+// rp_i = 1 / pivot_i,  u_i = sup_i * rp_i.
 #pragma once
 #include "cn_common.cuh"
 
-// Exclusive scan over the threads of a CTA.  (A, B) is this thread's chunk map; returns the value
-// entering this thread's chunk, given `tin` entering the first chunk in direction DIR.
-// sA, sB: shared arrays of >= 32 cplx, not in use by anyone else until the trailing barrier.
+#define CN_RS_G 256          // joint lines per group (= threads per CTA of the group kernels)
+#define CN_RS_TOP_THREADS 1024
+
+// Exclusive scan of affine maps over all threads of a CTA (blockDim.x a multiple of 32, <= 1024).
+// (A, B) is this thread's map in direction DIR; returns the value ENTERING this thread when `tin` enters
+// the first thread of the direction.  sA, sB: 32 cplx each, free again after the next barrier of the caller.
 template <int DIR>
-CN_DEVINL cplx block_scan_affine_excl(cplx A, cplx B, cplx tin, cplx *sA, cplx *sB)
+CN_DEVINL cplx cta_scan_excl(cplx A, cplx B, cplx tin, cplx *sA, cplx *sB)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     warp_scan_affine<DIR, 5>(A, B, lane);
     if (lane == (DIR > 0 ? 31 : 0)) {
         sA[warp] = A;
         sB[warp] = B;
     }
     __syncthreads();
-    cplx carry = tin;
-    if (DIR > 0) {
-        for (int v = 0; v < warp; ++v) carry = cfma(sA[v], carry, sB[v]);
-    } else {
-        for (int v = nwarps - 1; v > warp; --v) carry = cfma(sA[v], carry, sB[v]);
+    cplx wA = cmake(1.0, 0.0), wB = cmake(0.0, 0.0);
+    if (lane < nwarps) {
+        wA = sA[lane];
+        wB = sB[lane];
     }
+    warp_scan_affine<DIR, 5>(wA, wB, lane);
+    const int src = (DIR > 0) ? warp - 1 : warp + 1; // inclusive composite of all warps before this one
+    const bool has = (DIR > 0) ? (src >= 0) : (src < nwarps);
+    const int srcc = has ? src : lane;
+    cplx cA = shfl_c(wA, srcc), cB = shfl_c(wB, srcc);
+    cplx carry = has ? cfma(cA, tin, cB) : tin;
     cplx Ae = (DIR > 0) ? shfl_up_c(A, 1) : shfl_down_c(A, 1);
     cplx Be = (DIR > 0) ? shfl_up_c(B, 1) : shfl_down_c(B, 1);
     const bool first = (DIR > 0) ? (lane == 0) : (lane == 31);
-    cplx in = first ? carry : cfma(Ae, carry, Be);
-    __syncthreads();
-    return in;
+    cplx r = cfma(Ae, carry, Be);
+    return first ? carry : r;
 }
 
-// R_w = slotD[w] + slotU[w]  (the two extra elements per joint line of PAPER.md:102, summed here)
-__global__ void __launch_bounds__(1024, 1)
-k_rs_single(int64_t P, const cplx *__restrict__ slotD, const cplx *__restrict__ slotU,
-            const cplx *__restrict__ lw, const cplx *__restrict__ rq, const cplx *__restrict__ uw,
-            cplx *__restrict__ sup)
+// ---- RS[M_last]: one CTA, K rows per thread in registers ---------------------------------------------
+// R_w = rD[w] + rU[w]  (the two extra elements per joint line of PAPER.md:102, summed here)
+// forward   R'_w = R_w - lw_w R'_{w-1},   back substitution  X_w = rq_w R'_w - uw_w X_{w+1}
+template <int K>
+__global__ void __launch_bounds__(CN_RS_TOP_THREADS, 1)
+k_rs_top(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ lw,
+         const cplx *__restrict__ rq, const cplx *__restrict__ uw, cplx *__restrict__ X)
 {
-    __shared__ cplx sA[32], sB[32];
-    const int T = blockDim.x, t = threadIdx.x;
-    const int64_t K = (P + T - 1) / T;
-    const int64_t w0 = (int64_t)t * K, w1 = (w0 + K < P) ? (w0 + K) : P;
+    __shared__ cplx sA[2][32], sB[2][32];
+    const int t = threadIdx.x;
+    const int64_t w0 = (int64_t)t * K;
     const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
+    cplx l[K], r[K], u[K], R[K];
+    // the factors do not depend on the preceding kernel: fetch them before waiting for it
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const bool in = w0 + k < n;
+        l[k] = in ? lw[w0 + k] : zero;
+        r[k] = in ? rq[w0 + k] : zero;
+        u[k] = in ? uw[w0 + k] : zero;
+    }
+    pdl_wait();
+#pragma unroll
+    for (int k = 0; k < K; ++k) R[k] = (w0 + k < n) ? cadd(rD[w0 + k], rU[w0 + k]) : zero;
+    pdl_launch_dependents();
 
-    // forward elimination  R'_w = R_w - lw_w R'_{w-1}   (e_d / f_d on the joint lines)
     cplx A = one, B = zero;
-    for (int64_t w = w0; w < w1; ++w) {
-        cplx l = lw[w];
-        B = cfnma(l, B, cadd(slotD[w], slotU[w]));
-        A = cmul(cneg(l), A);
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        B = cfnma(l[k], B, R[k]);
+        A = cmul(cneg(l[k]), A);
     }
-    cplx in = block_scan_affine_excl<+1>(A, B, zero, sA, sB);
-    for (int64_t w = w0; w < w1; ++w) {
-        in = cfnma(lw[w], in, cadd(slotD[w], slotU[w]));
-        sup[w] = in; // R'_w, same thread reads it back below
+    cplx in = cta_scan_excl<+1>(A, B, zero, sA[0], sB[0]);
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        in = cfnma(l[k], in, R[k]);
+        R[k] = cmul(r[k], in); // rq_w R'_w
     }
-    // back substitution  Psi_w = rq_w R'_w - uw_w Psi_{w+1}
     A = one;
     B = zero;
-    for (int64_t w = w1 - 1; w >= w0; --w) {
-        cplx u = uw[w];
-        B = cfnma(u, B, cmul(rq[w], sup[w]));
-        A = cmul(cneg(u), A);
+#pragma unroll
+    for (int k = K - 1; k >= 0; --k) {
+        B = cfnma(u[k], B, R[k]);
+        A = cmul(cneg(u[k]), A);
     }
-    in = block_scan_affine_excl<-1>(A, B, zero, sA, sB);
-    for (int64_t w = w1 - 1; w >= w0; --w) {
-        in = cfnma(uw[w], in, cmul(rq[w], sup[w]));
-        sup[w] = in;
+    in = cta_scan_excl<-1>(A, B, zero, sA[1], sB[1]);
+#pragma unroll
+    for (int k = K - 1; k >= 0; --k) {
+        in = cfnma(u[k], in, R[k]);
+        if (w0 + k < n) X[w0 + k] = in;
     }
+}
+
+// ---- paper-literal serial RS: plain Thomas back/forward substitution by one thread ----------------------
+__global__ void k_rs_serial(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
+                            const cplx *__restrict__ lw, const cplx *__restrict__ rq, const cplx *__restrict__ uw,
+                            cplx *__restrict__ X)
+{
+    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+    pdl_wait();
+    pdl_launch_dependents();
+    cplx prev = cmake(0.0, 0.0);
+    for (int64_t w = 0; w < n; ++w) {
+        prev = cfnma(lw[w], prev, cadd(rD[w], rU[w]));
+        X[w] = prev;
+    }
+    prev = cmake(0.0, 0.0);
+    for (int64_t w = n - 1; w >= 0; --w) {
+        prev = cfnma(uw[w], prev, cmul(rq[w], X[w]));
+        X[w] = prev;
+    }
+}
+
+// ---- (RD+RU+JD+JU)[M_i], d-side: group g of level i -> slots of joint line g of level i+1 ----------------
+__global__ void __launch_bounds__(CN_RS_G, 4)
+k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
+            const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ sub,
+            const cplx *__restrict__ sup, cplx *__restrict__ outD, cplx *__restrict__ outU)
+{
+    __shared__ cplx sA[2][32], sB[2][32], sY;
+    const int t = threadIdx.x;
+    const int64_t g = blockIdx.x, g0 = g * CN_RS_G;
+    const int ng = (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G);
+    const int64_t i = g0 + t;
+    const bool interior = t < ng - 1, joint = t == ng - 1;
+    const cplx zero = cmake(0.0, 0.0);
+    cplx li = zero, rpi = zero, ui = zero, subJ = zero, supAbove = zero;
+    if (interior) {
+        li = l[i];
+        rpi = rp[i];
+        ui = u[i];
+    }
+    if (joint) subJ = sub[i];
+    if (t == 0 && g > 0) supAbove = sup[g0 - 1];
+    pdl_wait();
+    cplx R = (t < ng) ? cadd(rD[i], rU[i]) : zero;
+    pdl_launch_dependents();
+    // RD: D_i = R_i - l_i D_{i-1}, nothing enters the group (zero support values)
+    cplx A = cneg(li), B = interior ? R : zero;
+    cplx in = cta_scan_excl<+1>(A, B, zero, sA[0], sB[0]);
+    cplx D = cfma(A, in, B);
+    // RU + local solution: y_i = rp_i D_i - u_i y_{i+1}, y_joint = 0
+    A = cneg(ui);
+    B = cmul(rpi, D);
+    in = cta_scan_excl<-1>(A, B, zero, sA[1], sB[1]);
+    cplx y = cfma(A, in, B);
+    if (t == ng - 2) sY = y;
+    __syncthreads();
+    if (joint) outD[g] = (ng >= 2) ? cfnma(subJ, sY, R) : R;              // JD
+    if (t == 0 && g > 0) outU[g - 1] = (ng >= 2) ? cneg(cmul(supAbove, y)) : zero; // JU
+}
+
+// ---- SS[M_i]: group g of level i from the support values of level i+1 ------------------------------------
+__global__ void __launch_bounds__(CN_RS_G, 4)
+k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
+           const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ Xup,
+           cplx *__restrict__ X)
+{
+    __shared__ cplx sA[2][32], sB[2][32];
+    const int t = threadIdx.x;
+    const int64_t g = blockIdx.x, g0 = g * CN_RS_G;
+    const int ng = (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G);
+    const int64_t i = g0 + t;
+    const bool interior = t < ng - 1, joint = t == ng - 1;
+    const cplx zero = cmake(0.0, 0.0);
+    cplx li = zero, rpi = zero, ui = zero;
+    if (interior) {
+        li = l[i];
+        rpi = rp[i];
+        ui = u[i];
+    }
+    cplx R = interior ? cadd(rD[i], rU[i]) : zero; // written two kernels ago: complete
+    pdl_wait();
+    const cplx XL = (g > 0) ? Xup[g - 1] : zero, XJ = Xup[g];
+    pdl_launch_dependents();
+    cplx A = cneg(li), B = R;
+    if (t == 0 && interior) B = cfnma(li, XL, R); // the joint above carries its support value
+    cplx in = cta_scan_excl<+1>(A, B, zero, sA[0], sB[0]);
+    cplx D = cfma(A, in, B);
+    A = cneg(ui);
+    B = joint ? XJ : cmul(rpi, D);
+    in = cta_scan_excl<-1>(A, B, zero, sA[1], sB[1]);
+    cplx x = cfma(A, in, B);
+    if (t < ng) X[i] = x;
+}
+
+// ======================================= factor side (once per plan) =======================================
+
+// level-0 reduced matrix from the block corner entries produced by k_factor_blocks (cn_factor.cuh)
+__global__ void k_rs_assemble0(int64_t P, int64_t N, double rho, const double *__restrict__ gam,
+                               const cplx *__restrict__ redSubD, const cplx *__restrict__ redDiagD,
+                               const cplx *__restrict__ redSupU, const cplx *__restrict__ redDiagU,
+                               cplx *__restrict__ sub, cplx *__restrict__ diag, cplx *__restrict__ sup)
+{
+    int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= P) return;
+    const int64_t J = ((N % P == 0) ? (w + 1) * (N / P) : (int64_t)(((__int128)(w + 1) * N) / P)) - 1;
+    cplx d = cmake(-gam[J] + redDiagD[w].x, rho + redDiagD[w].y);
+    cplx s = cmake(0.0, 0.0);
+    if (w < P - 1) {
+        d = cadd(d, redDiagU[w]);
+        s = redSupU[w];
+    }
+    sub[w] = (w > 0) ? redSubD[w] : cmake(0.0, 0.0);
+    diag[w] = d;
+    sup[w] = s;
+}
+
+// one thread per group of a non-last level: local LU of the interior rows, responses to unit support
+// values, and from them the rows of the next level's matrix (the JD / JU matrix side)
+__global__ void k_rs_factor_level(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
+                                  const cplx *__restrict__ sup, cplx *__restrict__ l, cplx *__restrict__ rp,
+                                  cplx *__restrict__ u, cplx *__restrict__ tmp, cplx *__restrict__ sub2,
+                                  cplx *__restrict__ diag2, cplx *__restrict__ diag2U, cplx *__restrict__ sup2,
+                                  int *__restrict__ err)
+{
+    const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
+    const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= ngroups) return;
+    const int64_t g0 = g * CN_RS_G;
+    const int64_t J = ((g0 + CN_RS_G < n) ? (g0 + CN_RS_G) : n) - 1;
+    const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
+    bool bad = false;
+    cplx prp = one, psup = zero, Dal = one; // Dal: forward sweep of the response to X_{g-1} = 1
+    for (int64_t i = g0; i < J; ++i) {
+        cplx li = cmul(sub[i], prp);
+        cplx piv = cfnma(li, psup, diag[i]);
+        if (!cfinite_nonzero(piv)) bad = true;
+        cplx r = crecip(piv);
+        l[i] = li;
+        rp[i] = r;
+        u[i] = cmul(sup[i], r);
+        Dal = cneg(cmul(li, Dal));
+        tmp[i] = Dal;
+        prp = r;
+        psup = sup[i];
+    }
+    l[J] = zero;
+    rp[J] = zero;
+    u[J] = zero;
+    const bool has = J > g0;
+    // alpha_i: response to (X_{g-1}, X_g) = (1, 0);  beta_i: response to (0, 1)
+    cplx al = zero, be = one, alLast = zero, beLast = zero;
+    for (int64_t i = J - 1; i >= g0; --i) {
+        al = cfnma(u[i], al, cmul(rp[i], tmp[i]));
+        be = cneg(cmul(u[i], be));
+        if (i == J - 1) {
+            alLast = al;
+            beLast = be;
+        }
+    }
+    // row J of this level:  sub_J x_{J-1} + diag_J x_J + sup_J x_{J+1} = R_J
+    sub2[g] = (g == 0) ? zero : (has ? cmul(sub[J], alLast) : sub[J]);
+    diag2[g] = has ? cfma(sub[J], beLast, diag[J]) : diag[J];
+    if (g > 0) {
+        const cplx sa = sup[g0 - 1];
+        diag2U[g - 1] = has ? cmul(sa, al) : zero;
+        sup2[g - 1] = has ? cmul(sa, be) : sa;
+    }
+    if (g == ngroups - 1) {
+        diag2U[g] = zero;
+        sup2[g] = zero;
+    }
+    if (bad) atomicExch(err, 1);
+}
+
+// diag += diagU (the two-writer accumulation of the next level's diagonal)
+__global__ void k_rs_add(int64_t n, cplx *__restrict__ diag, const cplx *__restrict__ diagU)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) diag[i] = cadd(diag[i], diagU[i]);
+}
+
+// serial LU of the last level's matrix: lw_w = sub_w * rq_{w-1}, rq_w = 1 / pivot_w, uw_w = sup_w * rq_w
+__global__ void k_rs_factor_top(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
+                                const cplx *__restrict__ sup, cplx *__restrict__ lw, cplx *__restrict__ rq,
+                                cplx *__restrict__ uw, int *__restrict__ err)
+{
+    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+    cplx rqprev = cmake(0.0, 0.0), supprev = cmake(0.0, 0.0);
+    bool bad = false;
+    for (int64_t w = 0; w < n; ++w) {
+        cplx lq = (w > 0) ? cmul(sub[w], rqprev) : cmake(0.0, 0.0);
+        cplx piv = cfnma(lq, supprev, diag[w]);
+        if (!cfinite_nonzero(piv)) bad = true;
+        cplx r = crecip(piv);
+        lw[w] = lq;
+        rq[w] = r;
+        uw[w] = cmul(sup[w], r);
+        rqprev = r;
+        supprev = sup[w];
+    }
+    if (bad) atomicExch(err, 1);
 }

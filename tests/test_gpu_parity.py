@@ -20,10 +20,10 @@ def torch_():
     return torch
 
 
-def gpu_step(N, P, dx, dt, V, psi, nsteps, path=B.PATH_AUTO, tile_threads=0, calls=1):
+def gpu_step(N, P, dx, dt, V, psi, nsteps, path=B.PATH_AUTO, tile_threads=0, calls=1, **opts):
     torch = torch_()
     d_psi = torch.from_numpy(np.ascontiguousarray(psi)).cuda()
-    with B.Plan(N, P, dx, dt, np.ascontiguousarray(V), path=path, tile_threads=tile_threads) as plan:
+    with B.Plan(N, P, dx, dt, np.ascontiguousarray(V), path=path, tile_threads=tile_threads, **opts) as plan:
         plan.factorize()
         for _ in range(calls):
             plan.step(d_psi, nsteps)
@@ -87,6 +87,38 @@ def test_tiled_path_random(N, P, tt):
         err = np.max(np.abs(out - ref))
         assert err <= TOL_PSI, (N, P, tt, nsteps, err)
     out1, _ = gpu_step(N, P, dx, dt, V, psi, 1, path=B.PATH_TILED, tile_threads=tt)
+    assert residual(dx, dt, V, psi, out1) <= TOL_RES
+
+
+RS_CASES = [
+    # (N, P, opts): nested RS levels, ragged last group, single-row groups, serial RS
+    (1 << 13, 1 << 10, dict(rs_topmax=64)),            # 1024 -> 4 groups of 256
+    (8 * 1000, 1000, dict(rs_topmax=64)),               # ragged last group (232 rows)
+    (8 * 1025, 1025, dict(rs_topmax=64)),               # last group is a single joint row
+    (8 * 513, 513, dict(rs_topmax=2)),                  # 513 -> 3 -> 1 : three levels
+    (1 << 16, 1 << 13, dict(rs_levels=1)),              # single CTA, K = 8
+    (1 << 15, 3000, dict(rs_levels=1)),                 # single CTA, K = 4, generic path (ragged blocks)
+    (1 << 16, 1 << 13, dict(rs_levels=2)),
+    (1 << 17, 1 << 14, dict()),                         # auto: 16384 > 4096 -> two levels
+    (1 << 13, 1 << 10, dict(rs_levels=-1)),             # paper-literal serial RS
+    (1 << 13, 1 << 10, dict(pdl=0)),
+    (5000, 700, dict(rs_topmax=16)),                    # generic path + nested RS
+]
+
+
+@pytest.mark.parametrize("N,P,opts", RS_CASES)
+def test_rs_levels(N, P, opts):
+    cfg = W.scaled(W.CONFIGS["C2dense"], N=N)
+    V, psi = W.potential(cfg), W.psi0(cfg)
+    # strongly implicit step (s = dt / 4 dx^2 = 12.5) so that the reduced system is NOT nearly diagonal
+    dx, dt = 0.01, 0.005
+    ref = O.step(dx, dt, V, psi, 3)
+    out, info = gpu_step(N, P, dx, dt, V, psi, 3, **opts)
+    err = np.max(np.abs(out - ref))
+    assert err <= TOL_PSI, (N, P, opts, info, err)
+    if "rs_levels" in opts and opts["rs_levels"] > 0:
+        assert info["rs_levels"] == opts["rs_levels"]
+    out1, _ = gpu_step(N, P, dx, dt, V, psi, 1, **opts)
     assert residual(dx, dt, V, psi, out1) <= TOL_RES
 
 
