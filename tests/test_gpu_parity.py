@@ -190,3 +190,21 @@ def test_errors_on_device():
         with pytest.raises(B.CnError) as ei:
             p3.factorize()
         assert ei.value.status == B.CN_EBREAKDOWN
+
+
+@pytest.mark.parametrize("name", ["C2dense", "C2"])
+def test_config_c2_full_size(name):
+    """BASELINE configs[1] at full N = 2^24 in the launch configuration bench.py times (default P, tiled path,
+    nested RS, PDL): every element against the oracle after 20 of the 1000 steps (the oracle needs ~0.3 s per
+    step at this size), plus the size-independent properties: norm and the residual of one solve."""
+    cfg = W.CONFIGS[name]
+    V, psi = W.potential(cfg), W.psi0(cfg)
+    nsteps = 20
+    ref = O.step(cfg.dx, cfg.dt, V, psi, nsteps)
+    out, info = gpu_step(cfg.N, cfg.P, cfg.dx, cfg.dt, V, psi, nsteps)
+    assert info["path"] == B.PATH_TILED and info["rs_levels"] >= 2
+    err = np.max(np.abs(out - ref))
+    assert err <= TOL_PSI, err
+    assert abs(np.vdot(out, out).real * cfg.dx - 1.0) <= 1e-12
+    out1, _ = gpu_step(cfg.N, cfg.P, cfg.dx, cfg.dt, V, psi, 1)
+    assert residual(cfg.dx, cfg.dt, V, psi, out1) <= TOL_RES
