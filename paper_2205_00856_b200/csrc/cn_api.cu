@@ -16,6 +16,7 @@
 #include "cn_pass_generic.cuh"
 #include "cn_pass_tiled.cuh"
 #include "cn_reduced.cuh"
+#include "cn_batched.cuh"
 
 typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -31,6 +32,7 @@ struct cn_plan {
     cplx *lw = nullptr, *rq = nullptr, *uw = nullptr; // LU factors of the LAST RS level
     cplx *slotD = nullptr, *slotU = nullptr, *sup[2] = {nullptr, nullptr};
     cplx *work = nullptr;
+    cplx *qB = nullptr; // whole-system inverse pivots for cn_batched_sweep (N <= CN_BATCHED_NMAX)
     int *derr = nullptr;
     size_t device_bytes = 0;
     std::vector<void *> owned; // every device allocation of the factorization (freed by free_factors)
@@ -60,6 +62,12 @@ struct cn_plan {
     encode_tiled_fn encode = nullptr;
     CUtensorMap tmQ, tmGam, tmPsi;
     const void *tmPsiFor = nullptr;
+    // batched sweep: tensor map of the last (psi, nsys, strides) and the persistent grid of its kernel
+    CUtensorMap tmBatch;
+    const void *tmBatchFor = nullptr;
+    int64_t tmBatchKey[3] = {0, 0, 0};
+    int batchGrid = 0;
+    int sms = 0;
     // bookkeeping
     int last_cuda = 0;
     int64_t launches = 0;
@@ -100,8 +108,10 @@ static void free_factors(cn_plan *p)
     p->device_bytes = p->dV ? sizeof(double) * (size_t)p->N : 0;
     p->q = nullptr; p->gam = nullptr; p->lw = p->rq = p->uw = nullptr;
     p->slotD = p->slotU = nullptr; p->sup[0] = p->sup[1] = nullptr; p->work = nullptr; p->derr = nullptr;
+    p->qB = nullptr;
     p->factorized = false;
     p->tmPsiFor = nullptr;
+    p->tmBatchFor = nullptr;
 }
 
 extern "C" const char *cn_version(void) { return "cn_nshape 0.1 (sm_100a)"; }
@@ -338,6 +348,8 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     if ((st = dev_alloc(p, &p->derr, 1)) != CN_OK) return st;
     if (p->path == 1)
         if ((st = dev_alloc(p, &p->work, (size_t)N)) != CN_OK) return st;
+    if (N <= CN_BATCHED_NMAX)
+        if ((st = dev_alloc(p, &p->qB, (size_t)N)) != CN_OK) return st;
 
     // RS levels: lv[0] has P rows; add levels of ceil(n / G) rows until the last one fits the single CTA
     {
@@ -397,6 +409,10 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     k_rs_assemble0<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(P, N, p->rho, p->gam, redSubD, redDiagD, redSupU,
                                                                  redDiagU, p->lv[0].sub, p->lv[0].diag, p->lv[0].sup);
     p->launches += 2;
+    if (p->qB) { // one block per system: the factors of cn_batched_sweep
+        k_factor_whole<<<1, 32, 0, stream>>>(N, p->rho, p->gam, p->qB, p->derr);
+        p->launches += 1;
+    }
     for (int i = 0; i + 1 < nlv; ++i) {
         cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
         k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, tmpA,
@@ -438,6 +454,11 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
         const int64_t tiles = (N / 8 + p->tpb - 1) / p->tpb;
         const int64_t slots = (int64_t)sms * per_sm;
         p->grid_tiled = (int)(tiles < slots ? tiles : slots);
+    }
+    {
+        int dev = 0;
+        CN_CUDA(p, cudaGetDevice(&dev));
+        CN_CUDA(p, cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, dev));
     }
     p->factorized = true;
     return CN_OK;
@@ -604,10 +625,218 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
     return launch_pass(p, psi, 2, cur, stream);
 }
 
-extern "C" cn_status cn_batched_sweep(cn_plan *p, void *psi, int64_t nsys, int64_t elem_stride, int64_t sys_stride,
-                                      int64_t nsteps, void *stream)
+// ---- batched sweep (config C4) --------------------------------------------------------------------------
+typedef void (*bx_kernel_t)(const CUtensorMap, const cn_bx_params);
+typedef void (*by_kernel_t)(const CUtensorMap, const cn_by_params);
+
+static bx_kernel_t bx_kernel(int logc, int cl)
 {
-    (void)psi; (void)nsys; (void)elem_stride; (void)sys_stride; (void)nsteps; (void)stream;
-    if (!p) return CN_EINVAL;
-    return CN_EINVAL; // implemented in a later commit of this round
+    if (cl == 1) {
+        switch (logc) {
+        case 3: return k_batched_x<3, 1>;
+        case 4: return k_batched_x<4, 1>;
+        case 5: return k_batched_x<5, 1>;
+        case 6: return k_batched_x<6, 1>;
+        case 7: return k_batched_x<7, 1>;
+        case 8: return k_batched_x<8, 1>;
+        }
+        return nullptr;
+    }
+    if (logc != 8) return nullptr;
+    if (cl == 2) return k_batched_x<8, 2>;
+    if (cl == 4) return k_batched_x<8, 4>;
+    if (cl == 8) return k_batched_x<8, 8>;
+    return nullptr;
+}
+
+static by_kernel_t by_kernel(int logg, int cl, size_t *smem)
+{
+#define CN_BY(L, C)                          \
+    {                                        \
+        *smem = batched_y_smem_bytes<L>();   \
+        return k_batched_y<L, C>;            \
+    }
+    if (cl == 1) {
+        switch (logg) {
+        case 2: CN_BY(2, 1)
+        case 3: CN_BY(3, 1)
+        case 4: CN_BY(4, 1)
+        case 5: CN_BY(5, 1)
+        case 6: CN_BY(6, 1)
+        }
+        return nullptr;
+    }
+    if (logg != 6) return nullptr;
+    if (cl == 2) CN_BY(6, 2)
+    if (cl == 4) CN_BY(6, 4)
+    if (cl == 8) CN_BY(6, 8)
+#undef CN_BY
+    return nullptr;
+}
+
+// launch with a cluster dimension (and programmatic stream serialization) on a persistent grid
+template <typename K, typename... Args>
+static cudaError_t launch_cluster(K k, unsigned grid, unsigned block, size_t smem, unsigned cl, cudaStream_t stream,
+                                  bool pdl, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[2];
+    int na = 0;
+    if (cl > 1) {
+        at[na].id = cudaLaunchAttributeClusterDimension;
+        at[na].val.clusterDim.x = cl;
+        at[na].val.clusterDim.y = 1;
+        at[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    if (pdl) {
+        at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    cfg.attrs = at;
+    cfg.numAttrs = na;
+    return cudaLaunchKernelEx(&cfg, k, args...);
+}
+
+// persistent grid (in CTAs) of a kernel launched in clusters of `cl`
+template <typename K>
+static cn_status persistent_grid(cn_plan *p, K k, unsigned block, size_t smem, unsigned cl, int64_t work, int *grid)
+{
+    CN_CUDA(p, cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int64_t slots = 0;
+    if (cl > 1) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(cl * 1024, 1, 1);
+        cfg.blockDim = dim3(block, 1, 1);
+        cfg.dynamicSmemBytes = smem;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = cl;
+        at[0].val.clusterDim.y = 1;
+        at[0].val.clusterDim.z = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        int ncl = 0;
+        CN_CUDA(p, cudaOccupancyMaxActiveClusters(&ncl, (const void *)k, &cfg));
+        slots = ncl;
+    } else {
+        int per_sm = 0;
+        CN_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)k, (int)block, smem));
+        slots = (int64_t)per_sm * p->sms;
+    }
+    if (slots < 1) return CN_ECUDA;
+    const int64_t n = work < slots ? work : slots;
+    *grid = (int)(n * cl);
+    return CN_OK;
+}
+
+extern "C" cn_status cn_batched_sweep(cn_plan *p, void *psi_, int64_t nsys, int64_t es, int64_t ss, int64_t nsteps,
+                                      void *stream_)
+{
+    if (!p || !psi_ || nsys < 1 || nsteps < 0 || es < 1 || ss < 1) return CN_EINVAL;
+    if (((uintptr_t)psi_ & 15) != 0) return CN_EINVAL;
+    const int64_t N = p->N;
+    const bool xs = (es == 1 && (ss >= N || nsys == 1)), ys = (ss == 1 && es >= nsys && !xs);
+    if (!xs && !ys) return CN_EINVAL;
+    if (!p->factorized) return CN_ENOTFACTORIZED;
+    if (!p->qB) return CN_EINVAL; // N > CN_BATCHED_NMAX
+    if (nsteps == 0) return CN_OK;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    cplx *psi = (cplx *)psi_;
+    const bool pdl = p->opt_pdl != 0;
+    cn_status st;
+
+    // shape of the fast kernels: N = 8 * 2^k (x) / 16 * 2^k (y), at most 8 CTAs of a cluster per system
+    int lg = -1;
+    if ((N & (N - 1)) == 0)
+        for (lg = 0; (1LL << lg) < N; ++lg) {}
+    int path = 0, logp = 0, cl = 1; // 0 generic, 1 x, 2 y
+    if (p->opt_path != 1 && lg >= 6 && lg <= 14 && nsys < (1LL << 31) && ss < (1LL << 36) && es < (1LL << 36)) {
+        if (xs && lg <= 14) {
+            path = 1;
+            logp = lg - 3;
+            if (logp > 8) {
+                cl = 1 << (logp - 8);
+                logp = 8;
+            }
+        } else if (ys && lg <= 13 && nsys >= 8) {
+            path = 2;
+            logp = lg - 4;
+            if (logp > 6) {
+                cl = 1 << (logp - 6);
+                logp = 6;
+            }
+        }
+    }
+    const bool fresh = !(p->tmBatchFor == psi_ && p->tmBatchKey[0] == nsys && p->tmBatchKey[1] == es &&
+                         p->tmBatchKey[2] == ss);
+    cudaError_t e = cudaSuccess;
+    if (path == 1) {
+        bx_kernel_t k = bx_kernel(logp, cl);
+        if (!k) return CN_EINVAL;
+        const int cpb = 1 << logp, spt = CN_BX_TPB / cpb;
+        if (fresh) {
+            if ((st = get_encoder(p)) != CN_OK) return st;
+            cuuint64_t dims[3] = {16, (cuuint64_t)(N / 8), (cuuint64_t)nsys};
+            cuuint64_t strides[2] = {128, (cuuint64_t)ss * 16};
+            cuuint32_t box[3] = {16, (cuuint32_t)cpb, (cuuint32_t)(cl > 1 ? 1 : spt)};
+            cuuint32_t estr[3] = {1, 1, 1};
+            if (nsys == 1) strides[1] = (cuuint64_t)N * 16;
+            CUresult r = p->encode(&p->tmBatch, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, psi_, dims, strides, box, estr,
+                                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                   CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) return cuda_fail(p, cudaErrorInvalidValue);
+            const int64_t ntiles = cl > 1 ? nsys : (nsys + spt - 1) / spt;
+            if ((st = persistent_grid(p, k, CN_BX_TPB, batched_x_smem_bytes(), cl, ntiles, &p->batchGrid)) != CN_OK)
+                return st;
+        }
+        cn_bx_params prm{nsys, ss, p->rho, psi, p->qB, p->gam};
+        for (int64_t s = 0; s < nsteps && e == cudaSuccess; ++s) {
+            e = launch_cluster(k, (unsigned)p->batchGrid, CN_BX_TPB, batched_x_smem_bytes(), (unsigned)cl, stream, pdl,
+                               p->tmBatch, prm);
+            p->launches += 1;
+        }
+    } else if (path == 2) {
+        size_t smem = 0;
+        by_kernel_t k = by_kernel(logp, cl, &smem);
+        if (!k) return CN_EINVAL;
+        const int tpb = 8 << logp, rc = 16 << logp;
+        if (fresh) {
+            if ((st = get_encoder(p)) != CN_OK) return st;
+            cuuint64_t dims[2] = {(cuuint64_t)(2 * nsys), (cuuint64_t)N};
+            cuuint64_t strides[1] = {(cuuint64_t)es * 16};
+            cuuint32_t box[2] = {16, (cuuint32_t)(rc < 256 ? rc : 256)};
+            cuuint32_t estr[2] = {1, 1};
+            CUresult r = p->encode(&p->tmBatch, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, psi_, dims, strides, box, estr,
+                                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                   CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) return cuda_fail(p, cudaErrorInvalidValue);
+            if ((st = persistent_grid(p, k, tpb, smem, cl, (nsys + 7) / 8, &p->batchGrid)) != CN_OK) return st;
+        }
+        cn_by_params prm{nsys, es, p->rho, psi, p->qB, p->gam};
+        for (int64_t s = 0; s < nsteps && e == cudaSuccess; ++s) {
+            e = launch_cluster(k, (unsigned)p->batchGrid, (unsigned)tpb, smem, (unsigned)cl, stream, pdl, p->tmBatch, prm);
+            p->launches += 1;
+        }
+    } else {
+        const int T = 64;
+        for (int64_t s = 0; s < nsteps && e == cudaSuccess; ++s) {
+            e = launch_k(k_batched_generic, (unsigned)((nsys + T - 1) / T), T, 0, stream, pdl, N, nsys, es, ss, p->rho, psi,
+                         (const cplx *)p->qB, (const double *)p->gam);
+            p->launches += 1;
+        }
+    }
+    if (path != 0 && fresh) {
+        p->tmBatchFor = psi_;
+        p->tmBatchKey[0] = nsys;
+        p->tmBatchKey[1] = es;
+        p->tmBatchKey[2] = ss;
+    }
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    return CN_OK;
 }

@@ -1,0 +1,604 @@
+// Many-systems sweep (config C4; operator splitting reduces N-D to series of 1-D problems, PAPER.md:74,
+// 209-211): nsys independent tridiagonal systems that SHARE the plan's matrix, advanced by one CN step.
+//
+// Every system is solved entirely on chip, so psi crosses HBM once in and once out (32 B per point).  The
+// partition of a system is mapped onto the machine's own levels, the paper's nested scheme
+// (Eq. 6) applied downwards:
+//     level 0   one thread  = one block of 8 (x-sweep) or 16 (y-sweep) consecutive rows, in registers
+//     level 1   one warp    = the blocks of its lanes, interface values carried by warp shuffles
+//     level 2   one CTA     = its warps, interface values through shared memory
+//     level 3   one cluster = up to 8 CTAs, interface values through distributed shared memory
+// At every level the d-side of a sweep restricted to a part is the affine map "value entering the part ->
+// value leaving it" (cn_common.cuh); composing the maps of the parts before a part gives its inflow, which is
+// the RS + SS of that level.  Because the matrix is shared, the stored factors are the inverse pivots of
+// the downward elimination of the WHOLE system (one block per system), kept in registers
+// (x) or shared memory (y) for the lifetime of the persistent CTA: they never touch HBM again.
+//
+//   k_batched_x  rows of a system are contiguous (elem_stride == 1).  psi tiles move by TMA tensor loads /
+//                stores with the 128-byte swizzle (the transposition to one chunk per thread, as in
+//                cn_pass_tiled.cuh).
+//   k_batched_y  systems are interleaved (sys_stride == 1, rows elem_stride apart): a strip of 8 adjacent
+//                systems is 128 B wide; thread (g, c) owns 16 rows of column c, so global accesses are
+//                whole lines without any transposition.  The strip arrives by TMA (prefetched one strip
+//                ahead), the new psi leaves by 128-bit stores straight from registers.
+//   k_batched_generic  any N, any strides: one thread per system, in-place serial sweeps (correctness path).
+#pragma once
+#include <cuda.h>
+#include "cn_common.cuh"
+#include "cn_pass_tiled.cuh"
+
+// ---- cluster helpers ---------------------------------------------------------------------------------
+CN_DEVINL uint32_t cluster_ctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+CN_DEVINL void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+CN_DEVINL void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+// store a complex value into the shared memory of CTA `rank` of this cluster at the address `p` has here
+CN_DEVINL void dsmem_store(cplx *p, uint32_t rank, cplx v)
+{
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(p)), "r"(rank));
+    asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(remote), "d"(v.x), "d"(v.y) : "memory");
+}
+
+CN_DEVINL void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+CN_DEVINL void tma_store_3d(const CUtensorMap *map, const void *src, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];" ::"l"(map),
+                 "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
+}
+
+struct cn_bx_params {
+    int64_t nsys;
+    int64_t sys_stride; // complex elements between systems
+    double rho;
+    const cplx *psi_raw; // halo rows at CTA edges inside a cluster
+    const cplx *qB;      // inverse pivots of the whole-system downward elimination
+    const double *gam;
+};
+
+#define CN_BX_TPB 256
+#define CN_BATCHED_NMAX (1 << 20) // largest N for which cn_factorize also keeps whole-system pivots
+
+constexpr size_t batched_x_smem_bytes()
+{
+    return (size_t)CN_BX_TPB * 256 + (size_t)(CN_BX_TPB / 32) * 4 * sizeof(cplx) + 4 * 8 * sizeof(cplx) + 16;
+}
+
+// 256 threads x 8 points.  LOGC = log2(chunks per system) when a system fits one CTA (CL == 1, several
+// systems per tile); CL > 1: one system = CL CTAs of a cluster (LOGC == 8, every CTA chains all its chunks).
+template <int LOGC, int CL>
+__global__ void __launch_bounds__(CN_BX_TPB, 2)
+k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
+{
+    constexpr int TPB = CN_BX_TPB;
+    constexpr int CPS = (1 << LOGC) * CL;     // chunks per system
+    constexpr int CPB = 1 << LOGC;            // chunks chained inside this CTA
+    constexpr int SPT = TPB / CPB;            // systems per tile (CL == 1)
+    constexpr bool XWARP = (LOGC > 5);
+    constexpr int WSTEPS = XWARP ? 5 : LOGC;
+    constexpr int NW = TPB / 32;
+    constexpr int WPB = XWARP ? (CPB / 32) : 1;
+    static_assert(CL == 1 || LOGC == 8, "a cluster chains whole CTAs");
+
+    extern __shared__ __align__(1024) uint8_t smem[];
+    cplx *const s_psi = (cplx *)smem;
+    cplx *const s_out = (cplx *)(smem + (size_t)TPB * 128);
+    cplx *const s_scan = (cplx *)(smem + (size_t)TPB * 256); // [2 dirs][A,B][NW]
+    cplx *const s_mail = s_scan + 4 * NW;                    // [2 dirs][A,B][8 ranks]
+    uint64_t *const bar = (uint64_t *)(s_mail + 4 * 8);
+
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    const uint32_t rank = (CL > 1) ? cluster_ctarank() : 0u;
+    const int64_t cid = blockIdx.x / CL, ncl = gridDim.x / CL;
+    const int64_t ntiles = (CL > 1) ? prm.nsys : (prm.nsys + SPT - 1) / SPT;
+    const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
+    const double rho = prm.rho;
+    const int pos = (CL > 1) ? (int)rank * TPB + t : (t & (CPB - 1)); // chunk position inside its system
+    const bool sysFirst = pos == 0, sysLast = pos == CPS - 1;
+
+    auto issue_load = [&](int64_t tile) {
+        mbar_expect_tx(bar, (uint32_t)(TPB * 128));
+        if (CL > 1) tma_load_3d(s_psi, &tmPsi, bar, 0, (int)rank * TPB, (int)tile);
+        else tma_load_3d(s_psi, &tmPsi, bar, 0, 0, (int)(tile * SPT));
+    };
+
+    // ---- per-thread constants of the shared matrix: live in registers for the whole kernel -----------
+    cplx qv[8];
+    double g[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        qv[j] = prm.qB[8 * pos + j];
+        g[j] = prm.gam[8 * pos + j];
+    }
+    const cplx qm1 = sysFirst ? zero : prm.qB[8 * pos - 1];
+    cplx Qp = cneg(qv[0]);
+#pragma unroll
+    for (int j = 1; j < 7; ++j) Qp = cmul(Qp, cneg(qv[j]));
+    const cplx fwdA = sysFirst ? zero : cmul(cneg(qm1), Qp); // nothing enters a system from above
+    const cplx bwdA = sysLast ? zero : cmul(Qp, cneg(qv[7])); // ... nor from below (Dirichlet)
+
+    if (t == 0) {
+        if ((smem_u32(smem) & 1023u) != 0) __trap();
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    pdl_wait(); // psi is the output of the preceding sweep
+    pdl_launch_dependents();
+    if (t == 0 && cid < ntiles) issue_load(cid);
+    if (CL > 1) {
+        cluster_arrive();
+        cluster_wait();
+    } else {
+        __syncthreads();
+    }
+
+    // exclusive map of the chunks of this CTA before (DIR > 0) / after (DIR < 0) this thread: (Aex, Bex);
+    // also leaves the aggregate of the whole CTA in (aggA, aggB)
+    auto scan_cta = [&](auto dirtag, cplx A, cplx B, cplx &Aex, cplx &Bex, cplx &aggA, cplx &aggB) {
+        constexpr int DIR = decltype(dirtag)::value;
+        warp_scan_affine<DIR, WSTEPS>(A, B, lane);
+        cplx cA = one, cB = zero; // composite of the warps of this block before this warp
+        if (XWARP) {
+            cplx *sA = s_scan + (DIR > 0 ? 0 : 2 * NW), *sB = sA + NW;
+            if (lane == (DIR > 0 ? 31 : 0)) {
+                sA[warp] = A;
+                sB[warp] = B;
+            }
+            __syncthreads();
+            const int vb = warp & ~(WPB - 1);
+            cplx wA = one, wB = zero;
+            if (lane < WPB) {
+                wA = sA[vb + lane];
+                wB = sB[vb + lane];
+            }
+            warp_scan_affine<DIR, (LOGC > 5 ? LOGC - 5 : 0)>(wA, wB, lane);
+            aggA = shfl_c(wA, DIR > 0 ? WPB - 1 : 0);
+            aggB = shfl_c(wB, DIR > 0 ? WPB - 1 : 0);
+            const int src = (DIR > 0) ? warp - vb - 1 : warp - vb + 1;
+            const bool has = (DIR > 0) ? (src >= 0) : (src < WPB);
+            cplx xA = shfl_c(wA, has ? src : 0), xB = shfl_c(wB, has ? src : 0);
+            if (has) {
+                cA = xA;
+                cB = xB;
+            }
+        }
+        cplx Ae = (DIR > 0) ? shfl_up_c(A, 1) : shfl_down_c(A, 1);
+        cplx Be = (DIR > 0) ? shfl_up_c(B, 1) : shfl_down_c(B, 1);
+        const bool first = (DIR > 0) ? (lane == 0) : (lane == 31);
+        // (Ae, Be) after the warp composite (cA, cB):  x -> Ae (cA x + cB) + Be
+        Aex = first ? cA : cmul(Ae, cA);
+        Bex = first ? cB : cfma(Ae, cB, Be);
+    };
+
+    // inflow of this CTA from the other CTAs of its cluster (level 3); every thread returns the same value
+    auto cluster_inflow = [&](auto dirtag, cplx aggA, cplx aggB) -> cplx {
+        constexpr int DIR = decltype(dirtag)::value;
+        if (CL == 1) return zero;
+        cplx *mA = s_mail + (DIR > 0 ? 0 : 16), *mB = mA + 8;
+        if (warp == 0 && lane < CL) {
+            const bool wants = (DIR > 0) ? ((uint32_t)lane > rank) : ((uint32_t)lane < rank);
+            if (wants) {
+                dsmem_store(mA + rank, (uint32_t)lane, aggA);
+                dsmem_store(mB + rank, (uint32_t)lane, aggB);
+            }
+        }
+        cluster_arrive();
+        cluster_wait();
+        cplx in = zero;
+        if (DIR > 0) {
+            for (int u = 0; u < (int)rank; ++u) in = cfma(mA[u], in, mB[u]);
+        } else {
+            for (int u = CL - 1; u > (int)rank; --u) in = cfma(mA[u], in, mB[u]);
+        }
+        return in;
+    };
+
+    uint32_t phase = 0;
+    for (int64_t tile = cid; tile < ntiles; tile += ncl) {
+        // halo rows at the CTA edges inside a cluster: old psi straight from global memory (the neighbour CTA
+        // stores its new rows only after the second cluster barrier of this tile)
+        cplx vlo = zero, vhi = zero;
+        if (CL > 1) {
+            const cplx *row = prm.psi_raw + tile * prm.sys_stride;
+            if (t == 0 && rank > 0) vlo = row[8 * pos - 1];
+            if (t == TPB - 1 && rank < CL - 1) vhi = row[8 * pos + 8];
+        }
+        mbar_wait(bar, phase);
+        phase ^= 1;
+
+        cplx v[8];
+        const int sw = t & 7;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) v[j] = s_psi[t * 8 + (j ^ sw)];
+        if (t > 0 && !sysFirst) vlo = s_psi[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
+        if (t < TPB - 1 && !sysLast) vhi = s_psi[(t + 1) * 8 + ((t + 1) & 7)];
+        __syncthreads();
+        if (t == 0 && tile + ncl < ntiles) issue_load(tile + ncl);
+
+        // ---- Eq. 3 fused into the downward sweep -------------------------------------
+        cplx E[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            cplx lo = (j == 0) ? vlo : v[j - 1];
+            cplx hi = (j == 7) ? vhi : v[j + 1];
+            E[j] = rhs_E(g[j], rho, v[j], lo, hi);
+        }
+        cplx D = zero;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
+        cplx Aex, Bex, aggA, aggB;
+        scan_cta(std::integral_constant<int, +1>{}, fwdA, D, Aex, Bex, aggA, aggB);
+        cplx cin = cluster_inflow(std::integral_constant<int, +1>{}, aggA, aggB);
+        D = sysFirst ? zero : cfma(Aex, cin, Bex);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
+            E[j] = D;
+        }
+        // ---- upward sweep + substitution: x_j = q_j (d_j - x_{j+1}) ------------------------------------
+        cplx X = zero;
+#pragma unroll
+        for (int j = 7; j >= 0; --j) X = cmul(qv[j], csub(E[j], X));
+        scan_cta(std::integral_constant<int, -1>{}, bwdA, X, Aex, Bex, aggA, aggB);
+        cin = cluster_inflow(std::integral_constant<int, -1>{}, aggA, aggB);
+        X = sysLast ? zero : cfma(Aex, cin, Bex);
+#pragma unroll
+        for (int j = 7; j >= 0; --j) {
+            X = cmul(qv[j], csub(E[j], X));
+            v[j] = X;
+        }
+        // ---- new psi -> swizzled staging tile -> one TMA tensor store -------------------------------------
+        if (t == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s_out[t * 8 + (j ^ sw)] = v[j];
+        fence_proxy_async();
+        __syncthreads();
+        if (t == 0) {
+            if (CL > 1) tma_store_3d(&tmPsi, s_out, 0, (int)rank * TPB, (int)tile);
+            else tma_store_3d(&tmPsi, s_out, 0, 0, (int)(tile * SPT));
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+    }
+    if (t == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    if (CL > 1) { // nobody leaves while a neighbour may still address its shared memory
+        cluster_arrive();
+        cluster_wait();
+    }
+}
+
+// =========================================== y-sweep ===================================================
+struct cn_by_params {
+    int64_t nsys;  // number of systems (columns)
+    int64_t pitch; // complex elements between consecutive rows of a system (elem_stride)
+    double rho;
+    cplx *psi;
+    const cplx *qB;
+    const double *gam;
+};
+
+// padded index of the per-row constants in shared memory: one pad slot per 16 rows, so that the four row
+// groups of a warp (16 rows apart) broadcast from different banks
+CN_DEVINL int by_pad(int l) { return l + (l >> 4); }
+
+template <int LOGG>
+struct by_layout {
+    static constexpr int G = 1 << LOGG, RC = 16 * G, NW = (G / 4 > 0) ? G / 4 : 1;
+    static constexpr size_t off_q = (size_t)RC * 128;                         // after psi [RC rows][8 columns]
+    static constexpr size_t n_q = RC + RC / 16 + 2;                           // logical index row + 1, padded
+    static constexpr size_t off_g = off_q + n_q * 16;
+    static constexpr size_t n_g = (RC + RC / 16 + 2) & ~(size_t)1;
+    static constexpr size_t off_agg = off_g + n_g * 8;                        // [2 dirs][A[NW], B[NW][8]]
+    static constexpr size_t off_mail = off_agg + (size_t)2 * (NW + NW * 8) * 16; // [2 dirs][8 ranks][A, B[8]]
+    static constexpr size_t off_bar = off_mail + (size_t)2 * 8 * 9 * 16;
+    static constexpr size_t bytes = off_bar + 16;
+};
+template <int LOGG>
+constexpr size_t batched_y_smem_bytes()
+{
+    return by_layout<LOGG>::bytes;
+}
+
+// Thread (g, c): rows 16 g .. 16 g + 15 of this CTA's part of column c of the strip.  lane = c + 8 (g & 3),
+// warp = g >> 2.  G = 2^LOGG row groups per CTA, TPB = 8 G threads, CL CTAs per system (CL > 1 needs LOGG == 6).
+template <int LOGG, int CL>
+__global__ void __launch_bounds__(8 << LOGG, 1)
+k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
+{
+    constexpr int G = 1 << LOGG, TPB = 8 * G, RC = 16 * G;
+    constexpr int NW = (G / 4 > 0) ? G / 4 : 1;
+    constexpr int KW = (NW + 3) / 4; // warps covered by one lane role in the cross-warp scan
+    constexpr int BOXR = RC < 256 ? RC : 256;
+    static_assert(LOGG >= 2 && LOGG <= 6, "32..512 threads");
+    static_assert(CL == 1 || LOGG == 6, "a cluster chains whole CTAs");
+
+    typedef by_layout<LOGG> LY;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    cplx *const s_psi = (cplx *)smem;
+    cplx *const s_q = (cplx *)(smem + LY::off_q);
+    double *const s_g = (double *)(smem + LY::off_g);
+    cplx *const s_agg = (cplx *)(smem + LY::off_agg);
+    cplx *const s_mail = (cplx *)(smem + LY::off_mail);
+    uint64_t *const bar = (uint64_t *)(smem + LY::off_bar);
+
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    const int c = lane & 7, gl = lane >> 3, g = 4 * warp + gl;
+    const uint32_t rank = (CL > 1) ? cluster_ctarank() : 0u;
+    const int64_t cid = blockIdx.x / CL, ncl = gridDim.x / CL;
+    const int64_t nstrips = (prm.nsys + 7) / 8;
+    const int64_t grow0 = (int64_t)rank * RC + 16 * g; // first row of this thread inside its system
+    const bool sysFirst = (rank == 0 && g == 0), sysLast = (rank == CL - 1 && g == G - 1);
+    const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
+    const double rho = prm.rho;
+
+    auto issue_load = [&](int64_t strip) {
+        mbar_expect_tx(bar, (uint32_t)(RC * 128));
+#pragma unroll
+        for (int r = 0; r < RC; r += BOXR)
+            tma_load_2d((uint8_t *)s_psi + (size_t)r * 128, &tmPsi, bar, (int)(strip * 16), (int)(rank * RC + r));
+    };
+
+    // ---- constants of the shared matrix for this CTA's rows: shared memory, loaded once ---------------
+    for (int l = t; l <= RC; l += TPB) { // logical index l = local row + 1
+        const int64_t row = (int64_t)rank * RC + l - 1;
+        s_q[by_pad(l)] = (row >= 0) ? prm.qB[row] : zero;
+        if (l < RC) s_g[by_pad(l)] = prm.gam[row + 1];
+    }
+    if (t == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    pdl_wait();
+    pdl_launch_dependents();
+    if (t == 0 && cid < nstrips) issue_load(cid);
+    if (CL > 1) {
+        cluster_arrive();
+        cluster_wait();
+    } else {
+        __syncthreads();
+    }
+    // chunk multipliers (constant): fwdA = prod_{j<16} (-q_{row0+j-1}), bwdA = prod_{j<16} (-q_{row0+j})
+    cplx fwdA, bwdA;
+    {
+        cplx pm = one; // prod_{j=0..14} (-q_{row0+j})
+#pragma unroll
+        for (int j = 0; j < 15; ++j) pm = cmul(pm, cneg(s_q[by_pad(16 * g + j + 1)]));
+        fwdA = sysFirst ? zero : cmul(cneg(s_q[by_pad(16 * g)]), pm);
+        bwdA = sysLast ? zero : cmul(pm, cneg(s_q[by_pad(16 * g + 16)]));
+    }
+
+    // exclusive map (Aex, Bex) of the row groups of this CTA before (DIR > 0) / after (DIR < 0) this thread in
+    // its column, and the aggregate of the whole CTA for this column
+    auto scan_cta = [&](auto dirtag, cplx A, cplx B, cplx &Aex, cplx &Bex, cplx &aggA, cplx &aggB) {
+        constexpr int DIR = decltype(dirtag)::value;
+        // level 1: the four row groups of a warp (lanes 8 apart)
+#pragma unroll
+        for (int d = 8; d < 32; d <<= 1) {
+            cplx As = (DIR > 0) ? shfl_up_c(A, d) : shfl_down_c(A, d);
+            cplx Bs = (DIR > 0) ? shfl_up_c(B, d) : shfl_down_c(B, d);
+            const bool ok = (DIR > 0) ? (lane >= d) : (lane + d < 32);
+            if (ok) {
+                B = cfma(A, Bs, B);
+                A = cmul(A, As);
+            }
+        }
+        cplx cA = one, cB = zero; // composite of the warps before this warp in chain order
+        aggA = A;
+        aggB = B;
+        if (NW > 1) {
+            // level 2: warps.  chain position of warp w: w (DIR > 0) or NW-1-w (DIR < 0)
+            cplx *sA = s_agg + (DIR > 0 ? 0 : (NW + NW * 8)), *sB = sA + NW;
+            if (gl == (DIR > 0 ? 3 : 0)) {
+                if (c == 0) sA[warp] = A;
+                sB[warp * 8 + c] = B;
+            }
+            __syncthreads();
+            const int role = (DIR > 0) ? gl : 3 - gl;    // this lane composes chain positions [role KW, role KW + KW)
+            cplx a = one, b = zero;
+#pragma unroll
+            for (int i = 0; i < KW; ++i) {
+                const int p = role * KW + i;
+                if (p < NW) {
+                    const int w = (DIR > 0) ? p : NW - 1 - p;
+                    const cplx Au = sA[w], Bu = sB[w * 8 + c];
+                    b = cfma(Au, b, Bu);
+                    a = cmul(Au, a);
+                }
+            }
+#pragma unroll
+            for (int d = 8; d < 32; d <<= 1) { // inclusive over roles
+                cplx as = (DIR > 0) ? shfl_up_c(a, d) : shfl_down_c(a, d);
+                cplx bs = (DIR > 0) ? shfl_up_c(b, d) : shfl_down_c(b, d);
+                const bool ok = (DIR > 0) ? (lane >= d) : (lane + d < 32);
+                if (ok) {
+                    b = cfma(a, bs, b);
+                    a = cmul(a, as);
+                }
+            }
+            const int lastRoleLane = c + 8 * ((DIR > 0) ? 3 : 0);
+            aggA = shfl_c(a, lastRoleLane);
+            aggB = shfl_c(b, lastRoleLane);
+            // exclusive over roles, then the warps of the own role before the own warp
+            const int mypos = (DIR > 0) ? warp : NW - 1 - warp;
+            const int grole = mypos / KW, irole = mypos % KW;
+            cplx ea = (DIR > 0) ? shfl_up_c(a, 8) : shfl_down_c(a, 8);
+            cplx eb = (DIR > 0) ? shfl_up_c(b, 8) : shfl_down_c(b, 8);
+            if (role == 0) {
+                ea = one;
+                eb = zero;
+            }
+            const int srcLane = c + 8 * ((DIR > 0) ? grole : 3 - grole);
+            cA = shfl_c(ea, srcLane);
+            cB = shfl_c(eb, srcLane);
+#pragma unroll
+            for (int i = 0; i < KW - 1; ++i) {
+                if (i < irole) {
+                    const int p = grole * KW + i;
+                    const int w = (DIR > 0) ? p : NW - 1 - p;
+                    const cplx Au = sA[w], Bu = sB[w * 8 + c];
+                    cB = cfma(Au, cB, Bu);
+                    cA = cmul(Au, cA);
+                }
+            }
+        } else {
+            const int lastLane = c + 8 * ((DIR > 0) ? 3 : 0);
+            aggA = shfl_c(A, lastLane);
+            aggB = shfl_c(B, lastLane);
+        }
+        cplx Ae = (DIR > 0) ? shfl_up_c(A, 8) : shfl_down_c(A, 8);
+        cplx Be = (DIR > 0) ? shfl_up_c(B, 8) : shfl_down_c(B, 8);
+        const bool first = (DIR > 0) ? (gl == 0) : (gl == 3);
+        Aex = first ? cA : cmul(Ae, cA);
+        Bex = first ? cB : cfma(Ae, cB, Be);
+    };
+
+    auto cluster_inflow = [&](auto dirtag, cplx aggA, cplx aggB) -> cplx {
+        constexpr int DIR = decltype(dirtag)::value;
+        if (CL == 1) return zero;
+        cplx *m = s_mail + (DIR > 0 ? 0 : 8 * 9); // [rank][A, B[8]]
+        if (warp == 0) {
+            // lane (c, gl): destination ranks gl, gl + 4
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                const uint32_t dst = (uint32_t)gl + 4 * k;
+                const bool wants = dst < (uint32_t)CL && ((DIR > 0) ? (dst > rank) : (dst < rank));
+                if (wants) {
+                    if (c == 0) dsmem_store(m + rank * 9, dst, aggA);
+                    dsmem_store(m + rank * 9 + 1 + c, dst, aggB);
+                }
+            }
+        }
+        cluster_arrive();
+        cluster_wait();
+        cplx in = zero;
+        if (DIR > 0) {
+            for (int u = 0; u < (int)rank; ++u) in = cfma(m[u * 9], in, m[u * 9 + 1 + c]);
+        } else {
+            for (int u = CL - 1; u > (int)rank; --u) in = cfma(m[u * 9], in, m[u * 9 + 1 + c]);
+        }
+        return in;
+    };
+
+    uint32_t phase = 0;
+    for (int64_t strip = cid; strip < nstrips; strip += ncl) {
+        const int64_t col = strip * 8 + c;
+        const bool colOK = col < prm.nsys;
+        cplx *const gcol = prm.psi + col;
+        // halo rows at the CTA edges inside a cluster: old psi from global memory (the neighbour CTA stores its
+        // new rows only after the second cluster barrier of this strip)
+        cplx vlo = zero, vhi = zero;
+        if (CL > 1 && colOK) {
+            if (g == 0 && rank > 0) vlo = gcol[(grow0 - 1) * prm.pitch];
+            if (g == G - 1 && rank < CL - 1) vhi = gcol[(grow0 + 16) * prm.pitch];
+        }
+        mbar_wait(bar, phase);
+        phase ^= 1;
+        cplx v[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) v[j] = s_psi[(16 * g + j) * 8 + c];
+        if (g > 0) vlo = s_psi[(16 * g - 1) * 8 + c];
+        if (g < G - 1) vhi = s_psi[(16 * g + 16) * 8 + c];
+        __syncthreads();
+        if (t == 0 && strip + ncl < nstrips) issue_load(strip + ncl);
+
+        // ---- Eq. 3 in place: v_j <- E_j ------------------------------------------------------------------
+        {
+            cplx prev = vlo;
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                const cplx cur = v[j];
+                const cplx hi = (j == 15) ? vhi : v[j + 1];
+                v[j] = rhs_E(s_g[by_pad(16 * g + j)], rho, cur, prev, hi);
+                prev = cur;
+            }
+        }
+        // ---- downward sweep ----------------------------------------------------------------------------
+        cplx D = zero;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) D = cfnma(s_q[by_pad(16 * g + j)], D, v[j]);
+        cplx Aex, Bex, aggA, aggB;
+        scan_cta(std::integral_constant<int, +1>{}, fwdA, D, Aex, Bex, aggA, aggB);
+        cplx cin = cluster_inflow(std::integral_constant<int, +1>{}, aggA, aggB);
+        D = sysFirst ? zero : cfma(Aex, cin, Bex);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            D = cfnma(s_q[by_pad(16 * g + j)], D, v[j]);
+            v[j] = D;
+        }
+        // ---- upward sweep + substitution -----------------------------------------------------------------
+        cplx X = zero;
+#pragma unroll
+        for (int j = 15; j >= 0; --j) X = cmul(s_q[by_pad(16 * g + j + 1)], csub(v[j], X));
+        scan_cta(std::integral_constant<int, -1>{}, bwdA, X, Aex, Bex, aggA, aggB);
+        cin = cluster_inflow(std::integral_constant<int, -1>{}, aggA, aggB);
+        X = sysLast ? zero : cfma(Aex, cin, Bex);
+#pragma unroll
+        for (int j = 15; j >= 0; --j) {
+            X = cmul(s_q[by_pad(16 * g + j + 1)], csub(v[j], X));
+            v[j] = X;
+        }
+        if (colOK) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) gcol[(grow0 + j) * prm.pitch] = v[j];
+        }
+    }
+    if (CL > 1) {
+        cluster_arrive();
+        cluster_wait();
+    }
+}
+
+// ---- correctness path: one thread per system, in place, any N and any strides -------------------------
+__global__ void k_batched_generic(int64_t N, int64_t nsys, int64_t es, int64_t ss, double rho, cplx *__restrict__ psi,
+                                  const cplx *__restrict__ qB, const double *__restrict__ gam)
+{
+    pdl_wait();
+    pdl_launch_dependents();
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nsys) return;
+    cplx *p = psi + k * ss;
+    const cplx zero = cmake(0.0, 0.0);
+    cplx lo = zero, cur = p[0], D = zero, qprev = zero;
+    for (int64_t i = 0; i < N; ++i) {
+        cplx hi = (i + 1 < N) ? p[(i + 1) * es] : zero;
+        cplx E = rhs_E(gam[i], rho, cur, lo, hi);
+        D = cfnma(qprev, D, E); // RD on d (Eq. 11); D overwrites psi_i, no longer needed
+        p[i * es] = D;
+        qprev = qB[i];
+        lo = cur;
+        cur = hi;
+    }
+    cplx x = zero;
+    for (int64_t i = N - 1; i >= 0; --i) {
+        x = cmul(qB[i], csub(p[i * es], x));
+        p[i * es] = x;
+    }
+}
+
+// whole-system inverse pivots (one block per system): p_0 = mu_0, p_i = mu_i - q_{i-1}, q_i = 1 / p_i
+__global__ void k_factor_whole(int64_t N, double rho, const double *__restrict__ gam, cplx *__restrict__ qB,
+                               int *__restrict__ err)
+{
+    if (blockIdx.x != 0 || threadIdx.x != 0) return;
+    cplx qprev = cmake(0.0, 0.0);
+    bool bad = false;
+    for (int64_t i = 0; i < N; ++i) {
+        cplx p = cmake(-gam[i] - qprev.x, rho - qprev.y);
+        if (!cfinite_nonzero(p)) bad = true;
+        qprev = crecip(p);
+        qB[i] = qprev;
+    }
+    if (bad) atomicExch(err, 1);
+}
