@@ -34,6 +34,19 @@ struct cn_plan {
     cplx *work = nullptr;
     cplx *qB = nullptr; // whole-system inverse pivots for cn_batched_sweep (N <= CN_BATCHED_NMAX)
     int *derr = nullptr;
+    // out-of-core mode (cn_ooc: psi in pinned host memory, streamed part by part)
+    double *hV = nullptr;      // pinned host copy of V when it may not stay on the device
+    bool ooc = false;
+    int64_t partPts = 0;       // points per streamed part (a multiple of the tile and of the block size)
+    int64_t nparts = 0;
+    static const int NB = 3;   // parts in flight: copy in | compute | copy out
+    cplx *bPsi[NB] = {nullptr, nullptr, nullptr}, *bQ[NB] = {nullptr, nullptr, nullptr};
+    double *bV[NB] = {nullptr, nullptr, nullptr}; // V on arrival, gamma after k_factor_part (in place)
+    CUtensorMap tmPsiB[NB], tmQB[NB], tmGamB[NB];
+    double *gamJ = nullptr;    // gamma on the joint lines (the only per-point factor data kept, O(P))
+    cudaStream_t sIn = nullptr, sCmp = nullptr, sOut = nullptr;
+    cudaEvent_t evIn[NB] = {}, evCmp[NB] = {}, evFree[NB] = {}, evFork = nullptr, evJoin[3] = {};
+    std::vector<cudaEvent_t> evHost; // per part: its new psi has landed in host memory
     size_t device_bytes = 0;
     std::vector<void *> owned; // every device allocation of the factorization (freed by free_factors)
     // RS levels: lv[0] is the reduced system on the P joint lines, lv[i+1] the reduced
@@ -106,9 +119,12 @@ static void free_factors(cn_plan *p)
     p->owned.clear();
     p->lv.clear();
     p->device_bytes = p->dV ? sizeof(double) * (size_t)p->N : 0;
+    p->ooc = false;
     p->q = nullptr; p->gam = nullptr; p->lw = p->rq = p->uw = nullptr;
     p->slotD = p->slotU = nullptr; p->sup[0] = p->sup[1] = nullptr; p->work = nullptr; p->derr = nullptr;
     p->qB = nullptr;
+    p->gamJ = nullptr;
+    for (int b = 0; b < cn_plan::NB; ++b) { p->bPsi[b] = nullptr; p->bQ[b] = nullptr; p->bV[b] = nullptr; }
     p->factorized = false;
     p->tmPsiFor = nullptr;
     p->tmBatchFor = nullptr;
@@ -162,6 +178,18 @@ extern "C" cn_status cn_destroy(cn_plan *plan)
     if (!plan) return CN_EINVAL;
     free_factors(plan);
     if (plan->dV) cudaFree(plan->dV);
+    if (plan->hV) cudaFreeHost(plan->hV);
+    if (plan->sIn) cudaStreamDestroy(plan->sIn);
+    if (plan->sCmp) cudaStreamDestroy(plan->sCmp);
+    if (plan->sOut) cudaStreamDestroy(plan->sOut);
+    for (int b = 0; b < cn_plan::NB; ++b) {
+        if (plan->evIn[b]) cudaEventDestroy(plan->evIn[b]);
+        if (plan->evCmp[b]) cudaEventDestroy(plan->evCmp[b]);
+        if (plan->evFree[b]) cudaEventDestroy(plan->evFree[b]);
+        if (plan->evJoin[b]) cudaEventDestroy(plan->evJoin[b]);
+    }
+    if (plan->evFork) cudaEventDestroy(plan->evFork);
+    for (auto &e : plan->evHost) cudaEventDestroy(e);
     for (auto &e : plan->ev_pool) {
         cudaEventDestroy(e.a);
         cudaEventDestroy(e.b);
@@ -170,11 +198,31 @@ extern "C" cn_status cn_destroy(cn_plan *plan)
     return CN_OK;
 }
 
+// device bytes the in-core path needs: V, q, gamma (psi is the caller's) + the O(P) reduced-system arrays
+static size_t incore_bytes(const cn_plan *p)
+{
+    return (size_t)p->N * (8 + 16 + 8) + (size_t)p->P * 16 * 14;
+}
+
 extern "C" cn_status cn_plan_set_device_budget(cn_plan *plan, size_t bytes)
 {
     if (!plan) return CN_EINVAL;
+    free_factors(plan);
     plan->budget = bytes;
-    plan->factorized = false;
+    const bool want_host = bytes != 0 && incore_bytes(plan) > bytes;
+    const size_t vb = sizeof(double) * (size_t)plan->N;
+    if (want_host && !plan->hV) { // V leaves the device: keep a pinned host copy to stream from
+        CN_CUDA(plan, cudaMallocHost((void **)&plan->hV, vb));
+        CN_CUDA(plan, cudaMemcpy(plan->hV, plan->dV, vb, cudaMemcpyDeviceToHost));
+        cudaFree(plan->dV);
+        plan->dV = nullptr;
+    } else if (!want_host && plan->hV) {
+        CN_CUDA(plan, cudaMalloc((void **)&plan->dV, vb));
+        CN_CUDA(plan, cudaMemcpy(plan->dV, plan->hV, vb, cudaMemcpyHostToDevice));
+        cudaFreeHost(plan->hV);
+        plan->hV = nullptr;
+    }
+    plan->device_bytes = plan->dV ? vb : 0;
     return CN_OK;
 }
 
@@ -222,9 +270,9 @@ extern "C" cn_status cn_plan_get_info(const cn_plan *plan, cn_plan_info *info)
     info->N = plan->N; info->P = plan->P;
     info->path = plan->path;
     info->tile_threads = plan->tpb;
-    info->tile_points = (int64_t)plan->tpb * 8;
+    info->tile_points = plan->ooc ? plan->partPts : (int64_t)plan->tpb * 8;
     info->rs_levels = (plan->opt_rs_levels < 0) ? -1 : (int32_t)plan->lv.size();
-    info->out_of_core = 0;
+    info->out_of_core = plan->ooc ? 1 : 0;
     info->device_bytes = plan->device_bytes;
     info->launches = plan->launches;
     info->bytes_per_point_step = 56.0;
@@ -244,9 +292,9 @@ static cn_status get_encoder(cn_plan *p)
 }
 
 // 2-D view [rows = N/8][inner doubles] of a contiguous array; inner = 16 (complex) or 8 (real)
-static cn_status make_map(cn_plan *p, CUtensorMap *map, const void *base, int inner, int box_rows)
+static cn_status make_map(cn_plan *p, CUtensorMap *map, const void *base, int inner, int box_rows, int64_t rows = 0)
 {
-    cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)(p->N / 8)};
+    cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)(rows ? rows : p->N / 8)};
     cuuint64_t strides[1] = {(cuuint64_t)inner * 8};
     cuuint32_t box[2] = {(cuuint32_t)inner, (cuuint32_t)box_rows};
     cuuint32_t estr[2] = {1, 1};
@@ -311,6 +359,71 @@ static size_t tiled_smem(int tpb)
     return tpb == 128 ? tiled_smem_bytes<128>() : (tpb == 256 ? tiled_smem_bytes<256>() : tiled_smem_bytes<512>());
 }
 
+
+// ---- out-of-core mode (config C5) -----------------------------------------------------
+// psi stays in the caller's PINNED HOST memory and V in the plan's pinned copy.  The system is streamed in parts
+// of partPts points (whole blocks, whole tiles): copy in (psi 16 B + V 8 B per point) | k_factor_part + fused pass
+// | copy out (16 B per point) on three streams over NB rotating device buffers.  Only the joint-line arrays (slots,
+// support values, reduced-system factors: O(P)) persist on the device between passes.
+static cn_status ooc_setup(cn_plan *p, int64_t m)
+{
+    const int64_t N = p->N, P = p->P;
+    cn_status st;
+    // what is already owned (joint-line arrays) + the transient of the factorization; the rest: NB parts of 40 B per point
+    const size_t fixed = p->device_bytes + (size_t)P * 16 * 6;
+    const int64_t unit = ((int64_t)p->tpb * 8 > m) ? (int64_t)p->tpb * 8 : m; // both are powers of two times 8
+    if (p->budget <= fixed) return CN_ENOMEM;
+    int64_t pts = (int64_t)((p->budget - fixed) / (cn_plan::NB * 40));
+    if (pts > (1LL << 23)) pts = 1LL << 23; // 128 MB of psi per copy is plenty to reach the link rate
+    pts = pts / unit * unit;
+    if (pts < unit) return CN_ENOMEM;
+    if (pts > N) pts = (N + unit - 1) / unit * unit;
+    p->partPts = pts;
+    p->nparts = (N + pts - 1) / pts;
+    if ((st = get_encoder(p)) != CN_OK) return st;
+    const int box_rows = p->tpb < 256 ? p->tpb : 256;
+    for (int b = 0; b < cn_plan::NB; ++b) {
+        if ((st = dev_alloc(p, &p->bPsi[b], (size_t)pts)) != CN_OK) return st;
+        if ((st = dev_alloc(p, &p->bQ[b], (size_t)pts)) != CN_OK) return st;
+        if ((st = dev_alloc(p, &p->bV[b], (size_t)pts)) != CN_OK) return st;
+        if ((st = make_map(p, &p->tmPsiB[b], p->bPsi[b], 16, box_rows, pts / 8)) != CN_OK) return st;
+        if ((st = make_map(p, &p->tmQB[b], p->bQ[b], 16, box_rows, pts / 8)) != CN_OK) return st;
+        if ((st = make_map(p, &p->tmGamB[b], p->bV[b], 8, box_rows, pts / 8)) != CN_OK) return st;
+        if (!p->evIn[b]) {
+            CN_CUDA(p, cudaEventCreateWithFlags(&p->evIn[b], cudaEventDisableTiming));
+            CN_CUDA(p, cudaEventCreateWithFlags(&p->evCmp[b], cudaEventDisableTiming));
+            CN_CUDA(p, cudaEventCreateWithFlags(&p->evFree[b], cudaEventDisableTiming));
+            CN_CUDA(p, cudaEventCreateWithFlags(&p->evJoin[b], cudaEventDisableTiming));
+        }
+    }
+    if (!p->sIn) {
+        CN_CUDA(p, cudaStreamCreateWithFlags(&p->sIn, cudaStreamNonBlocking));
+        CN_CUDA(p, cudaStreamCreateWithFlags(&p->sCmp, cudaStreamNonBlocking));
+        CN_CUDA(p, cudaStreamCreateWithFlags(&p->sOut, cudaStreamNonBlocking));
+        CN_CUDA(p, cudaEventCreateWithFlags(&p->evFork, cudaEventDisableTiming));
+    }
+    while ((int64_t)p->evHost.size() < p->nparts) {
+        cudaEvent_t e;
+        CN_CUDA(p, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        p->evHost.push_back(e);
+    }
+    for (int mode = 0; mode < 3; ++mode) {
+        tiled_kernel_t k = tiled_kernel(p->tpb, p->logc, mode);
+        if (!k) return CN_EINVAL;
+        CN_CUDA(p, cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tiled_smem(p->tpb)));
+        CN_CUDA(p, cudaFuncSetAttribute((const void *)k, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+    }
+    int dev = 0, sms = 0, per_sm = 0;
+    CN_CUDA(p, cudaGetDevice(&dev));
+    CN_CUDA(p, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CN_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)tiled_kernel(p->tpb, p->logc, 1), p->tpb,
+                                                             tiled_smem(p->tpb)));
+    if (per_sm < 1) return CN_ECUDA;
+    const int64_t tiles = (pts / 8 + p->tpb - 1) / p->tpb, slots = (int64_t)sms * per_sm;
+    p->grid_tiled = (int)(tiles < slots ? tiles : slots);
+    return CN_OK;
+}
+
 // ---- factorize ----------------------------------------------------------------------------------------
 extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
 {
@@ -339,8 +452,14 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     p->logc = logc;
 
     cn_status st;
-    if ((st = dev_alloc(p, &p->q, (size_t)N)) != CN_OK) return st;
-    if ((st = dev_alloc(p, &p->gam, (size_t)N)) != CN_OK) return st;
+    p->ooc = (p->hV != nullptr); // V was moved to the host by cn_plan_set_device_budget: stream everything
+    if (p->ooc && p->path != 2) return CN_EINVAL; // the streamed mode exists for the tiled kernels only
+    if (!p->ooc) {
+        if ((st = dev_alloc(p, &p->q, (size_t)N)) != CN_OK) return st;
+        if ((st = dev_alloc(p, &p->gam, (size_t)N)) != CN_OK) return st;
+    } else {
+        if ((st = dev_alloc(p, &p->gamJ, (size_t)P)) != CN_OK) return st;
+    }
     if ((st = dev_alloc(p, &p->slotD, (size_t)P)) != CN_OK) return st;
     if ((st = dev_alloc(p, &p->slotU, (size_t)P)) != CN_OK) return st;
     if ((st = dev_alloc(p, &p->sup[0], (size_t)P)) != CN_OK) return st;
@@ -348,7 +467,7 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     if ((st = dev_alloc(p, &p->derr, 1)) != CN_OK) return st;
     if (p->path == 1)
         if ((st = dev_alloc(p, &p->work, (size_t)N)) != CN_OK) return st;
-    if (N <= CN_BATCHED_NMAX)
+    if (N <= CN_BATCHED_NMAX && !p->ooc)
         if ((st = dev_alloc(p, &p->qB, (size_t)N)) != CN_OK) return st;
 
     // RS levels: lv[0] has P rows; add levels of ceil(n / G) rows until the last one fits the single CTA
@@ -404,9 +523,26 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
 
     cn_geom g{N, P};
     const int T = 128;
-    k_factor_blocks<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(g, p->two_dx2, p->rho, p->dV, p->q, p->gam, redSubD,
-                                                                  redDiagD, redSupU, redDiagU, p->derr);
-    k_rs_assemble0<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(P, N, p->rho, p->gam, redSubD, redDiagD, redSupU,
+    if (!p->ooc) {
+        k_factor_blocks<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(g, p->two_dx2, p->rho, p->dV, p->q, p->gam, redSubD,
+                                                                      redDiagD, redSupU, redDiagU, p->derr);
+    } else {
+        // stream V through the device once, part by part: only the corner entries of every block's inverse and
+        // gamma on the joint lines stay (O(P)); q and gamma are recomputed per part in every pass of cn_step
+        if ((st = ooc_setup(p, m)) != CN_OK) { cudaFree(red); return st; }
+        for (int64_t i = 0; i < p->nparts; ++i) {
+            const int b = (int)(i % cn_plan::NB);
+            const int64_t r0 = i * p->partPts, n = (N - r0 < p->partPts) ? (N - r0) : p->partPts;
+            CN_CUDA(p, cudaMemcpyAsync(p->bV[b], p->hV + r0, sizeof(double) * (size_t)n, cudaMemcpyHostToDevice, stream));
+            const int64_t nb = n / m;
+            k_factor_part<<<(unsigned)((nb + T - 1) / T), T, 0, stream>>>(nb, m, r0 / m, p->two_dx2, p->rho, p->bV[b], p->bQ[b],
+                                                                         p->bV[b], redSubD, redDiagD, redSupU, redDiagU,
+                                                                         p->derr);
+            k_joint_gamma<<<(unsigned)((nb + T - 1) / T), T, 0, stream>>>(nb, m, r0 / m, p->bV[b], p->gamJ);
+            p->launches += 2;
+        }
+    }
+    k_rs_assemble0<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(P, N, p->rho, p->gam, p->gamJ, redSubD, redDiagD, redSupU,
                                                                  redDiagU, p->lv[0].sub, p->lv[0].diag, p->lv[0].sup);
     p->launches += 2;
     if (p->qB) { // one block per system: the factors of cn_batched_sweep
@@ -432,7 +568,7 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     if (e != cudaSuccess) return cuda_fail(p, e);
     if (herr) return CN_EBREAKDOWN;
 
-    if (p->path == 2) {
+    if (p->path == 2 && !p->ooc) {
         if ((st = get_encoder(p)) != CN_OK) return st;
         const int box_rows = p->tpb < 256 ? p->tpb : 256;
         if ((st = make_map(p, &p->tmQ, p->q, 16, box_rows)) != CN_OK) return st;
@@ -528,6 +664,7 @@ static cn_status launch_pass(cn_plan *p, cplx *psi, int mode, int cur, cudaStrea
     if (p->path == 2) {
         cn_tiled_params prm;
         prm.nchunks = p->N / 8;
+        prm.chunk0 = 0;
         prm.P = p->P;
         prm.rho = p->rho;
         prm.psi_raw = psi;
@@ -599,6 +736,85 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
     return CN_OK;
 }
 
+// one pass over all parts: mode 0 prologue (no copy out), 1 fused, 2 epilogue; `first` = psi on the host is the caller's
+static cn_status ooc_pass(cn_plan *p, cplx *hpsi, int mode, int cur, bool first)
+{
+    const int64_t N = p->N, m = N / p->P;
+    const int T = 128;
+    tiled_kernel_t k = tiled_kernel(p->tpb, p->logc, mode);
+    for (int64_t i = 0; i < p->nparts; ++i) {
+        const int b = (int)(i % cn_plan::NB);
+        const int64_t r0 = i * p->partPts, n = (N - r0 < p->partPts) ? (N - r0) : p->partPts;
+        // copy in: the buffer must be free, and the part's new psi of the previous pass must have landed
+        CN_CUDA(p, cudaStreamWaitEvent(p->sIn, p->evFree[b], 0));
+        if (!first) CN_CUDA(p, cudaStreamWaitEvent(p->sIn, p->evHost[i], 0));
+        CN_CUDA(p, cudaMemcpyAsync(p->bPsi[b], hpsi + r0, sizeof(cplx) * (size_t)n, cudaMemcpyHostToDevice, p->sIn));
+        CN_CUDA(p, cudaMemcpyAsync(p->bV[b], p->hV + r0, sizeof(double) * (size_t)n, cudaMemcpyHostToDevice, p->sIn));
+        CN_CUDA(p, cudaEventRecord(p->evIn[b], p->sIn));
+        // compute: factors of the part (recomputed instead of stored), then the pass
+        CN_CUDA(p, cudaStreamWaitEvent(p->sCmp, p->evIn[b], 0));
+        const int64_t nb = n / m;
+        k_factor_part<<<(unsigned)((nb + T - 1) / T), T, 0, p->sCmp>>>(nb, m, r0 / m, p->two_dx2, p->rho, p->bV[b], p->bQ[b],
+                                                                      p->bV[b], nullptr, nullptr, nullptr, nullptr, p->derr);
+        cn_tiled_params prm;
+        prm.nchunks = n / 8;
+        prm.chunk0 = r0 / 8;
+        prm.P = p->P;
+        prm.rho = p->rho;
+        prm.psi_raw = p->bPsi[b];
+        prm.supOld = p->sup[cur ^ 1];
+        prm.supNew = p->sup[cur];
+        prm.slotD = p->slotD;
+        prm.slotU = p->slotU;
+        prm.supInit = p->sup[0];
+        const int64_t tiles = (n / 8 + p->tpb - 1) / p->tpb;
+        const unsigned grid = (unsigned)(tiles < p->grid_tiled ? tiles : p->grid_tiled);
+        cudaError_t e = launch_k(k, grid, (unsigned)p->tpb, tiled_smem(p->tpb), p->sCmp, false, p->tmPsiB[b], p->tmQB[b],
+                                 p->tmGamB[b], prm);
+        p->launches += 2;
+        if (e != cudaSuccess) return cuda_fail(p, e);
+        CN_CUDA(p, cudaEventRecord(p->evCmp[b], p->sCmp));
+        if (mode != 0) {
+            CN_CUDA(p, cudaStreamWaitEvent(p->sOut, p->evCmp[b], 0));
+            CN_CUDA(p, cudaMemcpyAsync(hpsi + r0, p->bPsi[b], sizeof(cplx) * (size_t)n, cudaMemcpyDeviceToHost, p->sOut));
+            CN_CUDA(p, cudaEventRecord(p->evFree[b], p->sOut));
+            CN_CUDA(p, cudaEventRecord(p->evHost[i], p->sOut));
+        } else {
+            CN_CUDA(p, cudaEventRecord(p->evFree[b], p->sCmp));
+        }
+    }
+    return CN_OK;
+}
+
+static cn_status ooc_step(cn_plan *p, cplx *hpsi, int64_t nsteps, cudaStream_t stream)
+{
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, hpsi) != cudaSuccess || pa.type != cudaMemoryTypeHost) {
+        (void)cudaGetLastError();
+        return CN_EINVAL; // out-of-core mode streams psi from PINNED host memory
+    }
+    cn_status st;
+    CN_CUDA(p, cudaEventRecord(p->evFork, stream));
+    CN_CUDA(p, cudaStreamWaitEvent(p->sIn, p->evFork, 0));
+    CN_CUDA(p, cudaStreamWaitEvent(p->sCmp, p->evFork, 0));
+    CN_CUDA(p, cudaStreamWaitEvent(p->sOut, p->evFork, 0));
+    if ((st = ooc_pass(p, hpsi, 0, /*cur=*/1, true)) != CN_OK) return st;
+    if ((st = launch_rs(p, 1, p->sCmp)) != CN_OK) return st;
+    int cur = 1;
+    for (int64_t k = 1; k < nsteps; ++k) {
+        if ((st = ooc_pass(p, hpsi, 1, cur, k == 1)) != CN_OK) return st;
+        if ((st = launch_rs(p, cur ^ 1, p->sCmp)) != CN_OK) return st;
+        cur ^= 1;
+    }
+    if ((st = ooc_pass(p, hpsi, 2, cur, nsteps == 1)) != CN_OK) return st;
+    cudaStream_t ss[3] = {p->sIn, p->sCmp, p->sOut};
+    for (int i = 0; i < 3; ++i) {
+        CN_CUDA(p, cudaEventRecord(p->evJoin[i], ss[i]));
+        CN_CUDA(p, cudaStreamWaitEvent(stream, p->evJoin[i], 0));
+    }
+    return CN_OK;
+}
+
 extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *stream_)
 {
     if (!p || !psi_ || nsteps < 0) return CN_EINVAL;
@@ -608,6 +824,7 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
     cudaStream_t stream = (cudaStream_t)stream_;
     cplx *psi = (cplx *)psi_;
     cn_status st;
+    if (p->ooc) return ooc_step(p, psi, nsteps, stream);
     if (p->path == 2 && p->tmPsiFor != psi_) {
         const int box_rows = p->tpb < 256 ? p->tpb : 256;
         if ((st = make_map(p, &p->tmPsi, psi_, 16, box_rows)) != CN_OK) return st;
@@ -744,7 +961,7 @@ extern "C" cn_status cn_batched_sweep(cn_plan *p, void *psi_, int64_t nsys, int6
     const bool xs = (es == 1 && (ss >= N || nsys == 1)), ys = (ss == 1 && es >= nsys && !xs);
     if (!xs && !ys) return CN_EINVAL;
     if (!p->factorized) return CN_ENOTFACTORIZED;
-    if (!p->qB) return CN_EINVAL; // N > CN_BATCHED_NMAX
+    if (!p->qB) return CN_EINVAL; // N > CN_BATCHED_NMAX, or a streamed (out-of-core) plan
     if (nsteps == 0) return CN_OK;
     cudaStream_t stream = (cudaStream_t)stream_;
     cplx *psi = (cplx *)psi_;

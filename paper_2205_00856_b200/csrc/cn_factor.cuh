@@ -78,6 +78,66 @@ __global__ void k_factor_blocks(cn_geom g, double two_dx2, double rho, const dou
     if (bad) atomicExch(err, 1);
 }
 
+// The same for one streamed part of the system (out-of-core mode, cn_ooc.cuh): nb equal blocks of m rows whose
+// V / q / gamma live in part-local arrays; block wl of the part is block w0 + wl of the system.  red* may be
+// NULL (per-step recomputation of the factors: "neither the matrix nor the wavefunction ever need to be placed
+// entirely on a single process").
+// V and gam may be the SAME array (gamma replaces V in place).
+__global__ void k_factor_part(int64_t nb, int64_t m, int64_t w0, double two_dx2, double rho, const double *V,
+                              cplx *__restrict__ q, double *gam, cplx *__restrict__ redSubD,
+                              cplx *__restrict__ redDiagD, cplx *__restrict__ redSupU, cplx *__restrict__ redDiagU,
+                              int *__restrict__ err)
+{
+    int64_t wl = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (wl >= nb) return;
+    const int64_t f = wl * m, J = f + m - 1, w = w0 + wl;
+    cplx qprev = cmake(0.0, 0.0), prod = cmake(1.0, 0.0);
+    bool bad = false;
+    for (int64_t i = f; i < J; ++i) {
+        double gi = fma(two_dx2, V[i], 2.0);
+        gam[i] = gi;
+        cplx p = cmake(-gi - qprev.x, rho - qprev.y);
+        if (!cfinite_nonzero(p)) bad = true;
+        cplx qi = crecip(p);
+        q[i] = qi;
+        if (i < J - 1) prod = cmul(prod, cneg(qi));
+        qprev = qi;
+    }
+    gam[J] = fma(two_dx2, V[J], 2.0);
+    q[J] = cmake(1.0, 0.0);
+    if (redSubD) {
+        if (m >= 2) {
+            cplx Znn = qprev, Zn1 = cmul(qprev, prod), qu = cmake(0.0, 0.0);
+            for (int64_t i = J - 1; i >= f; --i) {
+                cplx p = cmake(-gam[i] - qu.x, rho - qu.y);
+                if (!cfinite_nonzero(p)) bad = true;
+                qu = crecip(p);
+            }
+            redSubD[w] = cneg(Zn1);
+            redDiagD[w] = cneg(Znn);
+            if (w > 0) {
+                redSupU[w - 1] = cneg(Zn1);
+                redDiagU[w - 1] = cneg(qu);
+            }
+        } else {
+            redSubD[w] = cmake(1.0, 0.0);
+            redDiagD[w] = cmake(0.0, 0.0);
+            if (w > 0) {
+                redSupU[w - 1] = cmake(1.0, 0.0);
+                redDiagU[w - 1] = cmake(0.0, 0.0);
+            }
+        }
+    }
+    if (bad) atomicExch(err, 1);
+}
+
+// diagonal of the joint lines for the level-0 reduced matrix when gamma is not resident: gJ[w] = gamma_{J_w}
+__global__ void k_joint_gamma(int64_t nb, int64_t m, int64_t w0, const double *__restrict__ gam, double *__restrict__ gJ)
+{
+    int64_t wl = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (wl < nb) gJ[w0 + wl] = gam[wl * m + m - 1];
+}
+
 // serial LU of the reduced matrix (once per plan): lw_w = sub_w * rq_{w-1}, rq_w = 1/pivot, uw_w = sup_w * rq_w
 __global__ void k_factor_reduced(cn_geom g, double rho, const double *__restrict__ gam,
                                  const cplx *__restrict__ redSubD, const cplx *__restrict__ redDiagD,

@@ -24,10 +24,11 @@
 #include "cn_common.cuh"
 
 struct cn_tiled_params {
-    int64_t nchunks; // N / 8
+    int64_t nchunks; // chunks (8 points) in the array the tensor maps describe: N / 8, or one streamed part of it
+    int64_t chunk0;  // global index of its first chunk (0 unless psi is streamed part by part, cn_ooc.cuh)
     int64_t P;
     double rho;
-    const cplx *psi_raw; // prologue only: old psi for the tile's left halo
+    const cplx *psi_raw; // prologue only: old psi for the tile's left halo (same array as tmPsi)
     const cplx *supOld;  // psi^k   at the joint lines (RS output of the previous step)
     const cplx *supNew;  // psi^k+1 at the joint lines (RS output of this step)
     cplx *slotD, *slotU;
@@ -140,11 +141,12 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
     uint32_t phase = 0;
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int64_t row0 = tile * TPB;
-        const int64_t c = row0 + t; // global chunk index
+        const int64_t c = row0 + t;         // chunk index inside the array
+        const int64_t cg = prm.chunk0 + c;  // global chunk index (chunk0 is a multiple of CPB)
         const bool active = c < prm.nchunks;
         const bool isFirst = (c & (CPB - 1)) == 0;
         const bool isLast = (c & (CPB - 1)) == CPB - 1;
-        const int64_t w = c >> LOGC;
+        const int64_t w = cg >> LOGC;
 
         // the few values that live on the joint lines (issued before waiting for the tile)
         cplx supN = zero;       // new value of the own joint line (last chunk of a block)
@@ -154,7 +156,8 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
             if (w > 0) jointAbove = prm.supNew[w - 1];
         }
         cplx oldAbove = zero; // OLD psi just above the tile (needed by thread 0 only)
-        if (t == 0 && c > 0) oldAbove = P1 ? prm.supOld[w - 1] : prm.psi_raw[8 * c - 1];
+        // (prologue of a streamed part: the row above it is a joint line whose psi^0 the previous part recorded)
+        if (t == 0 && cg > 0) oldAbove = P1 ? prm.supOld[w - 1] : (c > 0 ? prm.psi_raw[8 * c - 1] : prm.supInit[w - 1]);
 
         mbar_wait(bar, phase);
         phase ^= 1;

@@ -206,7 +206,9 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
 // ======================================= factor side (once per plan) =======================================
 
 // level-0 reduced matrix from the block corner entries produced by k_factor_blocks (cn_factor.cuh)
+// (gamJ != NULL: gamma of joint line w is gamJ[w] instead of gam[J_w] -- out-of-core mode, gamma not resident)
 __global__ void k_rs_assemble0(int64_t P, int64_t N, double rho, const double *__restrict__ gam,
+                               const double *__restrict__ gamJ,
                                const cplx *__restrict__ redSubD, const cplx *__restrict__ redDiagD,
                                const cplx *__restrict__ redSupU, const cplx *__restrict__ redDiagU,
                                cplx *__restrict__ sub, cplx *__restrict__ diag, cplx *__restrict__ sup)
@@ -214,7 +216,8 @@ __global__ void k_rs_assemble0(int64_t P, int64_t N, double rho, const double *_
     int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= P) return;
     const int64_t J = ((N % P == 0) ? (w + 1) * (N / P) : (int64_t)(((__int128)(w + 1) * N) / P)) - 1;
-    cplx d = cmake(-gam[J] + redDiagD[w].x, rho + redDiagD[w].y);
+    const double gJ = gamJ ? gamJ[w] : gam[J];
+    cplx d = cmake(-gJ + redDiagD[w].x, rho + redDiagD[w].y);
     cplx s = cmake(0.0, 0.0);
     if (w < P - 1) {
         d = cadd(d, redDiagU[w]);
