@@ -75,6 +75,8 @@ typedef struct {
     size_t device_bytes;     /* device memory owned by the plan */
     int64_t launches;        /* kernels launched by this plan so far (all entry points) */
     double bytes_per_point_step; /* algorithmic HBM bytes per point per fused step of the chosen path */
+    int64_t P_effective;     /* blocks the kernels work with: P, or N / 256 when a block of P exceeds one CTA tile
+                                (4096 rows) and the tiled path partitions it again */
 } cn_plan_info;
 
 /*

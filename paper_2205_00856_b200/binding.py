@@ -34,7 +34,7 @@ class cn_plan_info(ctypes.Structure):
     _fields_ = [("N", ctypes.c_int64), ("P", ctypes.c_int64), ("path", ctypes.c_int32),
                 ("tile_threads", ctypes.c_int32), ("tile_points", ctypes.c_int64), ("rs_levels", ctypes.c_int32),
                 ("out_of_core", ctypes.c_int32), ("device_bytes", ctypes.c_size_t), ("launches", ctypes.c_int64),
-                ("bytes_per_point_step", ctypes.c_double)]
+                ("bytes_per_point_step", ctypes.c_double), ("P_effective", ctypes.c_int64)]
 
 
 _lib = None

@@ -23,7 +23,8 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 struct cn_plan {
-    int64_t N = 0, P = 0;
+    int64_t N = 0, P = 0; // P: blocks the kernels work with (= Pu unless cn_factorize sub-partitions, see there)
+    int64_t Pu = 0;       // the caller's partition count
     double dx = 0, dt = 0, rho = 0, two_dx2 = 0;
     // device state
     double *dV = nullptr;
@@ -160,7 +161,7 @@ extern "C" cn_status cn_plan_create(cn_plan **out, int64_t N, int64_t P, double 
     if (!std::isfinite(dx) || !std::isfinite(dt) || dx <= 0.0 || dt == 0.0) return CN_EINVAL;
     cn_plan *p = new (std::nothrow) cn_plan();
     if (!p) return CN_ENOMEM;
-    p->N = N; p->P = P; p->dx = dx; p->dt = dt;
+    p->N = N; p->P = P; p->Pu = P; p->dx = dx; p->dt = dt;
     p->rho = 4.0 * dx * dx / dt; // 1 / s
     p->two_dx2 = 2.0 * dx * dx;
     cn_status st = dev_alloc(p, &p->dV, (size_t)N);
@@ -201,7 +202,8 @@ extern "C" cn_status cn_destroy(cn_plan *plan)
 // device bytes the in-core path needs: V, q, gamma (psi is the caller's) + the O(P) reduced-system arrays
 static size_t incore_bytes(const cn_plan *p)
 {
-    return (size_t)p->N * (8 + 16 + 8) + (size_t)p->P * 16 * 14;
+    const int64_t P = p->P > p->Pu ? p->P : p->Pu;
+    return (size_t)p->N * (8 + 16 + 8) + (size_t)P * 16 * 14;
 }
 
 extern "C" cn_status cn_plan_set_device_budget(cn_plan *plan, size_t bytes)
@@ -267,7 +269,8 @@ extern "C" cn_status cn_plan_get_info(const cn_plan *plan, cn_plan_info *info)
 {
     if (!plan || !info) return CN_EINVAL;
     memset(info, 0, sizeof *info);
-    info->N = plan->N; info->P = plan->P;
+    info->N = plan->N; info->P = plan->Pu;
+    info->P_effective = plan->P;
     info->path = plan->path;
     info->tile_threads = plan->tpb;
     info->tile_points = plan->ooc ? plan->partPts : (int64_t)plan->tpb * 8;
@@ -430,7 +433,16 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     if (!p) return CN_EINVAL;
     cudaStream_t stream = (cudaStream_t)stream_;
     free_factors(p);
-    const int64_t N = p->N, P = p->P;
+    const int64_t N = p->N;
+    // A caller's block of more than 4096 rows does not fit one CTA tile.  The tiled path then partitions every such
+    // block again into sub-blocks of 256 rows -- the same method one level down; psi does not
+    // depend on the partition.  The generic path (CN_OPT_PATH = 1) always takes the caller's P literally.
+    p->P = p->Pu;
+    if (p->opt_path != 1 && N % p->Pu == 0) {
+        const int64_t mu = N / p->Pu;
+        if (mu > 4096 && (mu & (mu - 1)) == 0) p->P = N / 256;
+    }
+    const int64_t P = p->P;
 
     // choose the path
     const bool uniform = (N % P == 0);
