@@ -977,7 +977,9 @@ extern "C" cn_status cn_batched_sweep(cn_plan *p, void *psi_, int64_t nsys, int6
     if (nsteps == 0) return CN_OK;
     cudaStream_t stream = (cudaStream_t)stream_;
     cplx *psi = (cplx *)psi_;
-    const bool pdl = p->opt_pdl != 0;
+    // no programmatic dependent launch here: CTAs of the next sweep that become resident early fragment the
+    // cluster placement of a persistent grid (measured: x/y alternation 1.93 ms with, 1.44 ms without)
+    const bool pdl = false;
     cn_status st;
 
     // shape of the fast kernels: N = 8 * 2^k (x) / 16 * 2^k (y), at most 8 CTAs of a cluster per system

@@ -44,6 +44,18 @@ CN_DEVINL void dsmem_store(cplx *p, uint32_t rank, cplx v)
     asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(remote), "d"(v.x), "d"(v.y) : "memory");
 }
 
+// The same store, asynchronous, completing 16 bytes of the transaction count of mbarrier `bar` IN THE DESTINATION
+// CTA: the receiver waits on its own mbarrier and needs neither a cluster barrier nor a memory fence.
+CN_DEVINL void dsmem_store_signal(cplx *p, uint64_t *bar, uint32_t rank, cplx v)
+{
+    uint32_t remote, rbar;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(p)), "r"(rank));
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rbar) : "r"(smem_u32(bar)), "r"(rank));
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];" ::"r"(remote),
+                 "d"(v.x), "d"(v.y), "r"(rbar)
+                 : "memory");
+}
+
 CN_DEVINL void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2)
 {
     asm volatile(
@@ -73,7 +85,7 @@ struct cn_bx_params {
 
 constexpr size_t batched_x_smem_bytes()
 {
-    return (size_t)CN_BX_TPB * 256 + (size_t)(CN_BX_TPB / 32) * 4 * sizeof(cplx) + 4 * 8 * sizeof(cplx) + 16;
+    return (size_t)CN_BX_TPB * 256 + (size_t)(CN_BX_TPB / 32) * 4 * sizeof(cplx) + 4 * 8 * sizeof(cplx) + 32;
 }
 
 // 256 threads x 8 points.  LOGC = log2(chunks per system) when a system fits one CTA (CL == 1, several
@@ -97,7 +109,7 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
     cplx *const s_out = (cplx *)(smem + (size_t)TPB * 128);
     cplx *const s_scan = (cplx *)(smem + (size_t)TPB * 256); // [2 dirs][A,B][NW]
     cplx *const s_mail = s_scan + 4 * NW;                    // [2 dirs][A,B][8 ranks]
-    uint64_t *const bar = (uint64_t *)(s_mail + 4 * 8);
+    uint64_t *const bar = (uint64_t *)(s_mail + 4 * 8); // [0] TMA loads, [1] downward mailbox, [2] upward mailbox
 
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const uint32_t rank = (CL > 1) ? cluster_ctarank() : 0u;
@@ -132,6 +144,8 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
     if (t == 0) {
         if ((smem_u32(smem) & 1023u) != 0) __trap();
         mbar_init(bar, 1);
+        mbar_init(bar + 1, 1);
+        mbar_init(bar + 2, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     pdl_wait(); // psi is the output of the preceding sweep
@@ -182,20 +196,25 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
         Bex = first ? cB : cfma(Ae, cB, Be);
     };
 
-    // inflow of this CTA from the other CTAs of its cluster (level 3); every thread returns the same value
+    // inflow of this CTA from the other CTAs of its cluster (level 3); every thread returns the same value.
+    // The aggregates travel by asynchronous DSMEM stores that signal the receiver's mbarrier: a CTA waits only for
+    // the CTAs it depends on, never for the whole cluster.  A sender can never be a whole tile ahead of a receiver,
+    // because it needs that receiver's aggregate of the opposite direction to finish its own tile.
+    uint32_t xphase = 0;
     auto cluster_inflow = [&](auto dirtag, cplx aggA, cplx aggB) -> cplx {
         constexpr int DIR = decltype(dirtag)::value;
         if (CL == 1) return zero;
         cplx *mA = s_mail + (DIR > 0 ? 0 : 16), *mB = mA + 8;
+        uint64_t *mb = bar + (DIR > 0 ? 1 : 2);
         if (warp == 0 && lane < CL) {
             const bool wants = (DIR > 0) ? ((uint32_t)lane > rank) : ((uint32_t)lane < rank);
             if (wants) {
-                dsmem_store(mA + rank, (uint32_t)lane, aggA);
-                dsmem_store(mB + rank, (uint32_t)lane, aggB);
+                dsmem_store_signal(mA + rank, mb, (uint32_t)lane, aggA);
+                dsmem_store_signal(mB + rank, mb, (uint32_t)lane, aggB);
             }
         }
-        cluster_arrive();
-        cluster_wait();
+        const int nsend = (DIR > 0) ? (int)rank : CL - 1 - (int)rank;
+        if (nsend > 0) mbar_wait(mb, xphase);
         cplx in = zero;
         if (DIR > 0) {
             for (int u = 0; u < (int)rank; ++u) in = cfma(mA[u], in, mB[u]);
@@ -208,9 +227,13 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
     uint32_t phase = 0;
     for (int64_t tile = cid; tile < ntiles; tile += ncl) {
         // halo rows at the CTA edges inside a cluster: old psi straight from global memory (the neighbour CTA
-        // stores its new rows only after the second cluster barrier of this tile)
+        // stores its new rows only after it has received this CTA's aggregates of this tile)
         cplx vlo = zero, vhi = zero;
         if (CL > 1) {
+            if (t == 0) { // arm this tile's mailboxes: 32 bytes (A, B) from every CTA this one depends on
+                if (rank > 0) mbar_expect_tx(bar + 1, rank * 32u);
+                if (rank < CL - 1) mbar_expect_tx(bar + 2, (CL - 1 - rank) * 32u);
+            }
             const cplx *row = prm.psi_raw + tile * prm.sys_stride;
             if (t == 0 && rank > 0) vlo = row[8 * pos - 1];
             if (t == TPB - 1 && rank < CL - 1) vhi = row[8 * pos + 8];
@@ -271,6 +294,7 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
             else tma_store_3d(&tmPsi, s_out, 0, 0, (int)(tile * SPT));
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
+        xphase ^= 1;
     }
     if (t == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     if (CL > 1) { // nobody leaves while a neighbour may still address its shared memory
@@ -303,7 +327,7 @@ struct by_layout {
     static constexpr size_t off_agg = off_g + n_g * 8;                        // [2 dirs][A[NW], B[NW][8]]
     static constexpr size_t off_mail = off_agg + (size_t)2 * (NW + NW * 8) * 16; // [2 dirs][8 ranks][A, B[8]]
     static constexpr size_t off_bar = off_mail + (size_t)2 * 8 * 9 * 16;
-    static constexpr size_t bytes = off_bar + 16;
+    static constexpr size_t bytes = off_bar + 32; // [0] TMA loads, [1] downward mailbox, [2] upward mailbox
 };
 template <int LOGG>
 constexpr size_t batched_y_smem_bytes()
@@ -358,6 +382,8 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
     }
     if (t == 0) {
         mbar_init(bar, 1);
+        mbar_init(bar + 1, 1);
+        mbar_init(bar + 2, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     pdl_wait();
@@ -464,10 +490,14 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
         Bex = first ? cB : cfma(Ae, cB, Be);
     };
 
+    // level 3 as in k_batched_x: asynchronous DSMEM stores that signal the receiver's mbarrier (144 bytes per sender:
+    // A and the 8 per-column B)
+    uint32_t xphase = 0;
     auto cluster_inflow = [&](auto dirtag, cplx aggA, cplx aggB) -> cplx {
         constexpr int DIR = decltype(dirtag)::value;
         if (CL == 1) return zero;
         cplx *m = s_mail + (DIR > 0 ? 0 : 8 * 9); // [rank][A, B[8]]
+        uint64_t *mb = bar + (DIR > 0 ? 1 : 2);
         if (warp == 0) {
             // lane (c, gl): destination ranks gl, gl + 4
 #pragma unroll
@@ -475,13 +505,13 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
                 const uint32_t dst = (uint32_t)gl + 4 * k;
                 const bool wants = dst < (uint32_t)CL && ((DIR > 0) ? (dst > rank) : (dst < rank));
                 if (wants) {
-                    if (c == 0) dsmem_store(m + rank * 9, dst, aggA);
-                    dsmem_store(m + rank * 9 + 1 + c, dst, aggB);
+                    if (c == 0) dsmem_store_signal(m + rank * 9, mb, dst, aggA);
+                    dsmem_store_signal(m + rank * 9 + 1 + c, mb, dst, aggB);
                 }
             }
         }
-        cluster_arrive();
-        cluster_wait();
+        const int nsend = (DIR > 0) ? (int)rank : CL - 1 - (int)rank;
+        if (nsend > 0) mbar_wait(mb, xphase);
         cplx in = zero;
         if (DIR > 0) {
             for (int u = 0; u < (int)rank; ++u) in = cfma(m[u * 9], in, m[u * 9 + 1 + c]);
@@ -497,8 +527,12 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
         const bool colOK = col < prm.nsys;
         cplx *const gcol = prm.psi + col;
         // halo rows at the CTA edges inside a cluster: old psi from global memory (the neighbour CTA stores its
-        // new rows only after the second cluster barrier of this strip)
+        // new rows only after it has received this CTA's aggregates of this strip)
         cplx vlo = zero, vhi = zero;
+        if (CL > 1 && t == 0) { // arm this strip's mailboxes
+            if (rank > 0) mbar_expect_tx(bar + 1, rank * 144u);
+            if (rank < CL - 1) mbar_expect_tx(bar + 2, (CL - 1 - rank) * 144u);
+        }
         if (CL > 1 && colOK) {
             if (g == 0 && rank > 0) vlo = gcol[(grow0 - 1) * prm.pitch];
             if (g == G - 1 && rank < CL - 1) vhi = gcol[(grow0 + 16) * prm.pitch];
@@ -553,6 +587,7 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
 #pragma unroll
             for (int j = 0; j < 16; ++j) gcol[(grow0 + j) * prm.pitch] = v[j];
         }
+        xphase ^= 1;
     }
     if (CL > 1) {
         cluster_arrive();
