@@ -32,6 +32,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
+from paper_2205_00856_b200 import replicas as R  # noqa: E402
 from paper_2205_00856_b200 import workloads as W  # noqa: E402
 
 CN_PER_STEP = 100            # CN steps per bench step (one cn_step call)
@@ -117,11 +118,7 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def dist_env():
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    return rank, world, local
+dist_env = R.dist_env
 
 
 def oracle_timed(cfg, V, psi, cn_steps: int):
@@ -220,11 +217,7 @@ def main():
         e1.record(stream)
         barrier()
         w1 = time.time()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = R.max_over_ranks(e0.elapsed_time(e1), world, device="cuda")
         return ms, w0, w1
 
     # ---- value: everything resident in HBM, the call a user makes (kernels chained by programmatic launch) ----
@@ -237,7 +230,7 @@ def main():
     time.sleep(0.1)
     ms, w0, w1 = timed_region(lambda: plan.step(d_psi, cn_per), args.steps)
     launches = plan.info()["launches"] - launches0
-    value = world * cfg.N * cn_per * args.steps / (ms * 1e-3) / 1e9
+    value = R.whole_job_throughput(cfg.N, cn_per * args.steps, ms, world)
 
     # ---- the same K steps again with a CUDA-event pair around every fused-pass launch and every RS chain on the
     # launching stream (CN_OPT_PROFILE).  Events between launches switch the programmatic overlap off, so this
@@ -277,7 +270,7 @@ def main():
         for _ in range(2):
             e2e_step()
         ms_e, _, _ = timed_region(e2e_step, args.steps)
-        e2e = {"value": world * cfg.N * cn_per * args.steps / (ms_e * 1e-3) / 1e9, "unit": UNIT,
+        e2e = {"value": R.whole_job_throughput(cfg.N, cn_per * args.steps, ms_e, world), "unit": UNIT,
                "h2d_bytes_per_step": 16 * cfg.N, "d2h_bytes_per_step": 16 * cfg.N,
                "ms_per_step": ms_e / args.steps}
 

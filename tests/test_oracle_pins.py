@@ -1,6 +1,7 @@
 """Pins of the oracle against things that are NOT the oracle: dense LU (LAPACK), closed forms,
 invariants, textbook physics.  All CPU (`-m "not gpu"`).  Each test names the mistake it would catch."""
 import math
+import os
 
 import numpy as np
 import pytest
@@ -260,3 +261,101 @@ def test_workloads_chunked_generation_is_bitwise_stable():
     full = W.psi0_unnormalised(cfg)
     parts = np.concatenate([W.psi0_unnormalised(cfg, s, min(cfg.N, s + 777_777)) for s in range(0, cfg.N, 777_777)])
     assert np.array_equal(full, parts)
+
+
+# ---- values the paper prints (tests/golden/paper_operation_counts.txt) ---------------------------------------
+def _golden():
+    out = {}
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_operation_counts.txt")
+    for line in open(path):
+        line = line.split("#")[0].strip()
+        if "=" in line:
+            k, v = line.split("=")
+            out[k.strip()] = float(v)
+    return out
+
+
+class _Counted:
+    """complex scalar that counts the arithmetic done with it"""
+    ops = {"div": 0, "mul": 0, "add": 0}
+
+    def __init__(self, v):
+        self.v = complex(v)
+
+    @staticmethod
+    def _v(o):
+        return o.v if isinstance(o, _Counted) else complex(o)
+
+    def __add__(self, o):
+        _Counted.ops["add"] += 1
+        return _Counted(self.v + self._v(o))
+    __radd__ = __add__
+
+    def __sub__(self, o):
+        _Counted.ops["add"] += 1
+        return _Counted(self.v - self._v(o))
+
+    def __mul__(self, o):
+        if isinstance(o, (int, float)) and o == 0:      # building zeros, not arithmetic of the method
+            return _Counted(0)
+        _Counted.ops["mul"] += 1
+        return _Counted(self.v * self._v(o))
+    __rmul__ = __mul__
+
+    def __truediv__(self, o):
+        _Counted.ops["div"] += 1
+        return _Counted(self.v / self._v(o))
+
+    def __rtruediv__(self, o):
+        _Counted.ops["div"] += 1
+        return _Counted(self._v(o) / self.v)
+
+    def __neg__(self):
+        return _Counted(-self.v)
+
+
+def test_table1_operation_counts():
+    """The reconstruction of the lost Table 1 (reading R1) costs what the paper says its method costs, PAPER.md:215:
+    3 divisions, 9 multiplications, 6 additions per interior row.  A missing or extra term anywhere in RD/RU/SS
+    changes one of the three counts."""
+    from oracle import nshape_table1 as T1
+    g = _golden()
+    n, nbl = 241, 8                                   # J = 1, 31, 61, ...: 30 rows per block, 29 interior
+    J = T1.joints_paper(n, nbl)
+    V, rhs = W.random_system(n, seed=2)
+    b, a, c = O.diagonals(0.1, 0.02, V)
+
+    def counted(x):
+        return np.array([_Counted(z) for z in x], dtype=object)
+
+    def run(JJ):
+        _Counted.ops = {"div": 0, "mul": 0, "add": 0}
+        psi, _ = T1.solve(counted(b), counted(a), counted(c), counted(rhs), JJ)
+        return dict(_Counted.ops), np.array([z.v for z in psi])
+
+    ops1, psi1 = run(J)
+    assert np.max(np.abs(psi1 - O.thomas(b, a, c, rhs))) < 1e-12
+    # growing every block by 10 interior rows isolates the per-interior-row cost from the per-block / RS cost
+    n2 = n + 10 * nbl
+    V2, rhs2 = W.random_system(n2, seed=2)
+    b2, a2, c2 = O.diagonals(0.1, 0.02, V2)
+    b, a, c, rhs = b2, a2, c2, rhs2
+    ops2, _ = run(T1.joints_paper(n2, nbl))
+    per_row = {k: (ops2[k] - ops1[k]) / (10 * nbl) for k in ops1}
+    assert per_row["div"] == g["divisions_per_interior_row"]
+    assert per_row["mul"] == g["multiplications_per_interior_row"]
+    assert per_row["add"] == g["additions_per_interior_row"]
+
+
+def test_performance_model_optimum():
+    """Eq. 7: t = alpha n_tot / n_bl + beta n_bl is minimal at n_bl* = sqrt(alpha/beta) sqrt(n_tot),
+    where t* = 2 sqrt(alpha beta n_tot) -- the formula the P sweep of config C2 is compared with."""
+    g = _golden()
+    alpha, beta = 1.41e-6, 0.36e-6
+    for ntot in (3e5, 2.0 ** 24, 2.0 ** 30):
+        P = np.arange(1, 200000, dtype=np.float64)
+        t = alpha * ntot / P + beta * P
+        k = int(np.argmin(t))
+        pstar = math.sqrt(alpha / beta) * ntot ** g["model_optimum_exponent"]
+        assert abs(P[k] - pstar) <= 1.0
+        assert abs(t[k] - 2 * math.sqrt(alpha * beta * ntot)) / t[k] < 1e-8
