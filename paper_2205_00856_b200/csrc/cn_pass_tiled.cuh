@@ -23,6 +23,9 @@
 #include <cuda.h>
 #include "cn_common.cuh"
 
+struct cn_true { static constexpr bool value = true; };
+struct cn_false { static constexpr bool value = false; };
+
 struct cn_tiled_params {
     int64_t nchunks; // chunks (8 points) in the array the tensor maps describe: N / 8, or one streamed part of it
     int64_t chunk0;  // global index of its first chunk (0 unless psi is streamed part by part, cn_ooc.cuh)
@@ -200,7 +203,8 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
         // exclusive inflow of a forward (RD) chain; tin = value on the joint line above the block.
         // Across the warps of one block the per-warp maps are composed by a second shuffle scan that every
         // warp of the block runs redundantly on the WPB aggregates (no serial chain, one barrier).
-        auto scan_fwd = [&](cplx A, cplx B, cplx tin, int buf) -> cplx {
+        auto scan_fwd = [&](cplx A, cplx B, cplx tin, int buf, auto zin) -> cplx {
+            constexpr bool ZEROIN = decltype(zin)::value;
             warp_scan_affine<+1, WSTEPS>(A, B, lane);
             cplx carry = tin;
             if (XWARP) {
@@ -221,8 +225,12 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
                 cplx cA = shfl_c(wA, src < 0 ? 0 : src), cB = shfl_c(wB, src < 0 ? 0 : src);
                 if (src >= 0) carry = cfma(cA, tin, cB);
             }
-            cplx Ae = shfl_up_c(A, 1), Be = shfl_up_c(B, 1);
-            cplx r = cfma(Ae, carry, Be);
+            cplx Be = shfl_up_c(B, 1);
+            cplx r = Be;
+            if (XWARP || !ZEROIN) { // with nothing entering the block the composed A is never needed (dead code)
+                cplx Ae = shfl_up_c(A, 1);
+                r = cfma(Ae, carry, Be);
+            }
             return (lane == 0) ? carry : r;
         };
         // exclusive inflow of a backward (RU) chain; nothing enters a block from below (joint resets)
@@ -247,8 +255,12 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
                 cplx cB = shfl_c(wB, src > 31 ? 31 : src);
                 if (src < WPB) carry = cB;
             }
-            cplx Ae = shfl_down_c(A, 1), Be = shfl_down_c(B, 1);
-            cplx r = cfma(Ae, carry, Be);
+            cplx Be = shfl_down_c(B, 1);
+            cplx r = Be;
+            if (XWARP) {
+                cplx Ae = shfl_down_c(A, 1);
+                r = cfma(Ae, carry, Be);
+            }
             return (lane == 31) ? carry : r;
         };
 
@@ -265,7 +277,7 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
 #pragma unroll
             for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
             if (isLast) D = supN; // the joint line carries its new support value
-            cplx in = scan_fwd(fwdA, D, jointAbove, 0);
+            cplx in = scan_fwd(fwdA, D, jointAbove, 0, cn_false());
             D = in;
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
@@ -326,7 +338,7 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
 #pragma unroll
             for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
             if (isLast) D = zero;
-            cplx in = scan_fwd(fwdA, D, zero, 1);
+            cplx in = scan_fwd(fwdA, D, zero, 1, cn_true());
             D = in;
 #pragma unroll
             for (int j = 0; j < 8; ++j) {

@@ -1,0 +1,238 @@
+"""Per-config throughput report (BASELINE.json: "report throughput on each config at 1 GPU in Gpoint-steps/s and as
+achieved fraction of the HBM roofline, along with the sweep over partition count P").
+
+    python -m paper_2205_00856_b200.report [--configs C1,C2,C3,C4,C5] [--sweep] [--out FILE]
+
+One JSON line per config on stdout (and appended to --out).  Everything runs through the C-ABI binding; nothing here
+touches oracle/ (parity of the same configs is in tests/).  Timing: CUDA events on the launching stream after a
+warm-up call.  `bytes_per_point` is the algorithmic figure of DESIGN.md section 5 (56 B per point-step, 32 B per
+point-sweep for C4, host link 24 B in + 16 B out for C5); `hbm_frac` divides by MEASURED_PEAKS.json's copy rate.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import time
+
+import numpy as np
+
+from . import binding as B
+from . import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"])
+    except Exception:
+        return 6650.0  # B200_PROFILING.md fallback
+
+
+def _events(torch):
+    return torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+
+def _inputs(cfg, chunk=1 << 24):
+    V = np.empty(cfg.N, np.float64)
+    psi = np.empty(cfg.N, np.complex128)
+    norm = W.psi0_norm2(cfg)
+    for s in range(0, cfg.N, chunk):
+        e = min(cfg.N, s + chunk)
+        V[s:e] = W.potential(cfg, s, e)
+        psi[s:e] = W.psi0(cfg, s, e, norm=norm)
+    return V, psi
+
+
+def time_plan(torch, plan, d_psi, nsteps, reps=3):
+    """best and median ms per CN step over `reps` cn_step(nsteps) calls"""
+    plan.step(d_psi, min(nsteps, 5))
+    torch.cuda.synchronize()
+    ms = []
+    for _ in range(reps):
+        e0, e1 = _events(torch)
+        e0.record()
+        plan.step(d_psi, nsteps)
+        e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1) / nsteps)
+    ms.sort()
+    return ms[0], ms[len(ms) // 2]
+
+
+def run_1d(torch, name, peak, nsteps=None, P=None, **opts):
+    cfg = W.CONFIGS[name]
+    V, psi = _inputs(cfg)
+    d = torch.from_numpy(psi).cuda()
+    del psi
+    with B.Plan(cfg.N, P or cfg.P, cfg.dx, cfg.dt, V, **opts) as plan:
+        t0 = time.time()
+        plan.factorize()
+        torch.cuda.synchronize()
+        fms = 1e3 * (time.time() - t0)
+        n = nsteps or cfg.steps
+        best, med = time_plan(torch, plan, d, n)
+        info = plan.info()
+    gbs = 56.0 * cfg.N / (best * 1e-3) / 1e9
+    return {"config": name, "N": cfg.N, "P": P or cfg.P, "P_effective": info["P_effective"], "path": info["path"],
+            "rs_levels": info["rs_levels"], "cn_steps_per_call": n, "us_per_cn_step_best": 1e3 * best,
+            "us_per_cn_step_median": 1e3 * med, "Gpoint_steps_per_s": cfg.N / best / 1e6, "bytes_per_point": 56,
+            "whole_step_GBps": gbs, "hbm_frac_measured_peak": gbs / peak, "hbm_frac_8TBps": gbs / 8000.0,
+            "factorize_ms": fms, "device_bytes": info["device_bytes"]}
+
+
+def run_c4(torch, peak):
+    """x-sweep then y-sweep per 2-D step (reading R18); 32 B per point per sweep."""
+    cfg = W.CONFIGS["C4"]
+    n = cfg.N
+    d = torch.from_numpy(W.psi0_2d(cfg)).cuda()
+    out = {"config": "C4", "N": n, "nsys": cfg.nsys, "bytes_per_point": 32}
+    with B.Plan(n, cfg.P, cfg.dx, cfg.dt, W.potential(cfg)) as px, \
+            B.Plan(n, cfg.P, cfg.dx, cfg.dt, W.potential_y(cfg)) as py:
+        px.factorize()
+        py.factorize()
+        sweeps = {"x": lambda: px.batched_sweep(d, n, 1, n, 1), "y": lambda: py.batched_sweep(d, n, n, 1, 1)}
+        sweeps["xy"] = lambda: (sweeps["x"](), sweeps["y"]())
+        for key, fn in sweeps.items():
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize()
+            e0, e1 = _events(torch)
+            e0.record()
+            for _ in range(cfg.steps):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / cfg.steps
+            nsw = 2 if key == "xy" else 1
+            gbs = 32.0 * n * n * nsw / (ms * 1e-3) / 1e9
+            out[key] = {"ms": ms, "Gpoint_sweeps_per_s": nsw * n * n / ms / 1e6, "GBps": gbs,
+                        "hbm_frac_measured_peak": gbs / peak, "hbm_frac_8TBps": gbs / 8000.0}
+    out["Gpoint_steps_per_s"] = n * n / out["xy"]["ms"] / 1e6  # one 2-D step = both sweeps
+    return out
+
+
+def link_rate(torch, nbytes=1 << 30):
+    """pinned host <-> device copy rates of this box (GB/s): H2D alone, D2H alone, both at once."""
+    h0 = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    h1 = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
+    d0 = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    d1 = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    s0, s1 = torch.cuda.Stream(), torch.cuda.Stream()
+    res = {}
+    for key in ("h2d", "d2h", "both"):
+        best = 1e30
+        for _ in range(3):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            if key in ("h2d", "both"):
+                with torch.cuda.stream(s0):
+                    d0.copy_(h0, non_blocking=True)
+            if key in ("d2h", "both"):
+                with torch.cuda.stream(s1):
+                    h1.copy_(d1, non_blocking=True)
+            torch.cuda.synchronize()
+            best = min(best, time.perf_counter() - t0)
+        res[key] = nbytes / best / 1e9
+    return res
+
+
+def run_c5(torch):
+    """psi in pinned host memory, 2 GB device budget: bound by the host link (24 B in + 16 B out per point-step)."""
+    cfg = W.CONFIGS["C5"]
+    V, psi = _inputs(cfg)
+    h = torch.from_numpy(psi).pin_memory()
+    del psi
+    link = link_rate(torch)
+    with B.Plan(cfg.N, cfg.P, cfg.dx, cfg.dt, V, device_budget=2 << 30) as plan:
+        plan.factorize()
+        info = plan.info()
+        plan.step(h, 1)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        plan.step(h, cfg.steps)
+        torch.cuda.synchronize()
+        sec = time.perf_counter() - t0
+    # a call of n steps makes n + 1 passes in (prologue + n) and n passes out
+    h2d = 24.0 * cfg.N * (cfg.steps + 1) / sec / 1e9
+    d2h = 16.0 * cfg.N * cfg.steps / sec / 1e9
+    return {"config": "C5", "N": cfg.N, "P": cfg.P, "cn_steps_per_call": cfg.steps, "s_per_cn_step": sec / cfg.steps,
+            "Gpoint_steps_per_s": cfg.N * cfg.steps / sec / 1e9, "h2d_GBps": h2d, "d2h_GBps": d2h,
+            "link_GBps": link, "h2d_frac_of_link": h2d / link["both"] if link["both"] else None,
+            "device_bytes": info["device_bytes"], "part_points": info["tile_points"]}
+
+
+def p_sweep(torch, peak, name="C2dense"):
+    """t(P) for P = 2^8..2^16 on both kernel families against the paper's model t = alpha N/P + beta P
+    (PAPER.md:217-237): least-squares fit of alpha, beta (and a floor t0 the model lacks), P* = sqrt(alpha/beta) sqrt(N)."""
+    cfg = W.CONFIGS[name]
+    V, psi = _inputs(cfg)
+    d = torch.from_numpy(psi).cuda()
+    rows = []
+    arms = (("tiled", dict()), ("paper_shape", dict(path=B.PATH_GENERIC, rs_levels=-1)),
+            ("generic_nested_rs", dict(path=B.PATH_GENERIC)))
+    for arm, opts in arms:
+        for Pk in cfg.P_sweep:
+            with B.Plan(cfg.N, Pk, cfg.dx, cfg.dt, V, **opts) as plan:
+                plan.factorize()
+                info = plan.info()
+                best, med = time_plan(torch, plan, d, 20 if arm == "tiled" else 3, reps=3)
+            rows.append({"arm": arm, "P": Pk, "P_effective": info["P_effective"], "rs_levels": info["rs_levels"],
+                         "us_per_cn_step": 1e3 * best})
+    fits = {}
+    for arm, _ in arms:
+        Ps = np.array([r["P"] for r in rows if r["arm"] == arm], float)
+        ts = np.array([r["us_per_cn_step"] for r in rows if r["arm"] == arm], float)
+        A = np.stack([cfg.N / Ps, Ps, np.ones_like(Ps)], 1)
+        (alpha, beta, t0), *_ = np.linalg.lstsq(A, ts, rcond=None)
+        fit = {"alpha_us_per_point": alpha, "beta_us_per_block": beta, "floor_us": t0,
+               "P_measured_argmin": int(Ps[int(np.argmin(ts))])}
+        if alpha > 0 and beta > 0:
+            fit["delta"] = math.sqrt(alpha / beta)
+            fit["P_star_model"] = fit["delta"] * math.sqrt(cfg.N)
+        fits[arm] = fit
+    return {"config": name + " P sweep", "N": cfg.N, "sqrtN": math.isqrt(cfg.N), "rows": rows, "fit": fits}
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--configs", default="C1,C2,C3,C4,C5")
+    ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--out", default="")
+    args = ap.parse_args(argv)
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("report: no CUDA device; this library has no CPU fallback")
+    peak = _peak()
+    lines = []
+
+    def emit(obj):
+        s = json.dumps(obj)
+        print(s, flush=True)
+        lines.append(s)
+        if args.out:
+            with open(args.out, "a") as f:
+                f.write(s + "\n")
+    for name in [c.strip() for c in args.configs.split(",") if c.strip()]:
+        if name == "C1":
+            emit(run_1d(torch, "C1", peak))
+            emit(dict(run_1d(torch, "C1", peak, use_graph=1), variant="cuda_graph"))
+        elif name == "C2":
+            emit(run_1d(torch, "C2dense", peak, nsteps=100))
+        elif name == "C3":
+            emit(run_1d(torch, "C3", peak))
+        elif name == "C4":
+            emit(run_c4(torch, peak))
+        elif name == "C5":
+            emit(run_c5(torch))
+    if args.sweep:
+        emit(p_sweep(torch, peak))
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
