@@ -721,7 +721,7 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
     p->lv[0].X = p->sup[out];
     for (int i = 0; i + 1 < nlv && e == cudaSuccess; ++i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        e = launch_k(k_rs_reduce, (unsigned)U.n, (unsigned)CN_RS_G, 0, stream, pdl, L.n, (const cplx *)L.rD,
+        e = launch_k(k_rs_reduce, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
                      (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
                      (const cplx *)L.sup, U.rD, U.rU);
         p->launches += 1;
@@ -739,7 +739,7 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
     }
     for (int i = nlv - 2; i >= 0 && e == cudaSuccess; --i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        e = launch_k(k_rs_subst, (unsigned)U.n, (unsigned)CN_RS_G, 0, stream, pdl, L.n, (const cplx *)L.rD,
+        e = launch_k(k_rs_subst, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
                      (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X);
         p->launches += 1;
     }

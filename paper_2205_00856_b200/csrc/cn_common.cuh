@@ -62,6 +62,16 @@ CN_DEVINL cplx rhs_E(double gamma, double rho, cplx p, cplx lo, cplx hi)
 CN_DEVINL void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 CN_DEVINL void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
+// Load of a value the PRECEDING kernel of the chain produced, used after pdl_wait().  The pointers of the RS kernels
+// are `const __restrict__`, which allows the compiler to turn a plain load into ld.global.nc and to hoist it above
+// the wait; a volatile asm with a memory clobber stays below it and reads through L2.
+CN_DEVINL cplx ld_dep(const cplx *p)
+{
+    cplx v;
+    asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
+    return v;
+}
+
 CN_DEVINL cplx shfl_up_c(cplx v, int d)
 {
     return make_double2(__shfl_up_sync(0xffffffffu, v.x, d), __shfl_up_sync(0xffffffffu, v.y, d));

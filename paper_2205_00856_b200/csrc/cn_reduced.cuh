@@ -7,9 +7,9 @@
 //   * k_rs_top<K>     -- RS[M_last]: the pre-factored system of the last level is solved by ONE CTA;
 //                        every thread owns K consecutive rows held in registers, the threads are chained
 //                        by the affine-map scan of cn_common.cuh (serial depth K instead of n).
-//   * k_rs_reduce     -- (RD+RU+JD+JU)[M_i], i >= 1, d-side only: one CTA per group of G joint lines of
-//                        level i, one row per thread; emits two slots per joint line of level i+1.
-//   * k_rs_subst      -- SS[M_i], i >= 1: one CTA per group, given the two support values of level i+1.
+//   * k_rs_reduce     -- (RD+RU+JD+JU)[M_i], i >= 1, d-side only: one WARP per group of G joint lines of
+//                        level i, 8 rows per lane in registers; emits two slots per joint line of level i+1.
+//   * k_rs_subst      -- SS[M_i], i >= 1: one warp per group, given the two support values of level i+1.
 //   * k_rs_serial     -- the paper-literal variant (one thread, plain Thomas on the joint lines), kept
 //                        for the P sweep (CN_OPT_RS_LEVELS = -1).
 // All matrix-side quantities (local pivots, fill-in, the next level's matrix) are produced once by the
@@ -23,7 +23,7 @@
 #pragma once
 #include "cn_common.cuh"
 
-#define CN_RS_G 256          // joint lines per group (= threads per CTA of the group kernels)
+#define CN_RS_G 256          // joint lines per group
 #define CN_RS_TOP_THREADS 1024
 
 // Exclusive scan of affine maps over all threads of a CTA (blockDim.x a multiple of 32, <= 1024).
@@ -80,7 +80,7 @@ k_rs_top(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, co
     }
     pdl_wait();
 #pragma unroll
-    for (int k = 0; k < K; ++k) R[k] = (w0 + k < n) ? cadd(rD[w0 + k], rU[w0 + k]) : zero;
+    for (int k = 0; k < K; ++k) R[k] = (w0 + k < n) ? cadd(ld_dep(rD + w0 + k), ld_dep(rU + w0 + k)) : zero;
     pdl_launch_dependents();
 
     cplx A = one, B = zero;
@@ -120,7 +120,7 @@ __global__ void k_rs_serial(int64_t n, const cplx *__restrict__ rD, const cplx *
     pdl_launch_dependents();
     cplx prev = cmake(0.0, 0.0);
     for (int64_t w = 0; w < n; ++w) {
-        prev = cfnma(lw[w], prev, cadd(rD[w], rU[w]));
+        prev = cfnma(lw[w], prev, cadd(ld_dep(rD + w), ld_dep(rU + w)));
         X[w] = prev;
     }
     prev = cmake(0.0, 0.0);
@@ -131,76 +131,151 @@ __global__ void k_rs_serial(int64_t n, const cplx *__restrict__ rD, const cplx *
 }
 
 // ---- (RD+RU+JD+JU)[M_i], d-side: group g of level i -> slots of joint line g of level i+1 ----------------
-__global__ void __launch_bounds__(CN_RS_G, 4)
+// One WARP per group of CN_RS_G = 256 joint lines: lane t owns the CN_RS_K = 8 consecutive rows g0 + 8 t ...
+// in registers and the lanes are chained by the warp scan of cn_common.cuh (no shared memory, no barrier).
+// Nothing enters a group during the reduction (zero support values), so the composed A of the scan is dead.
+#define CN_RS_K (CN_RS_G / 32)
+#define CN_RS_WARPS 4 // groups per CTA of the group kernels
+
+__global__ void __launch_bounds__(32 * CN_RS_WARPS)
 k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
             const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ sub,
             const cplx *__restrict__ sup, cplx *__restrict__ outD, cplx *__restrict__ outU)
 {
-    __shared__ cplx sA[2][32], sB[2][32], sY;
-    const int t = threadIdx.x;
-    const int64_t g = blockIdx.x, g0 = g * CN_RS_G;
-    const int ng = (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G);
-    const int64_t i = g0 + t;
-    const bool interior = t < ng - 1, joint = t == ng - 1;
+    constexpr int K = CN_RS_K;
+    const int lane = threadIdx.x & 31;
+    const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
+    const int64_t g = (int64_t)blockIdx.x * CN_RS_WARPS + (threadIdx.x >> 5);
+    const bool live = g < ngroups; // whole warps only: the shuffles below stay convergent
+    const int64_t g0 = g * CN_RS_G;
+    const int ng = live ? (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G) : 0;
+    const int r0 = lane * K; // first row of this lane inside the group
     const cplx zero = cmake(0.0, 0.0);
-    cplx li = zero, rpi = zero, ui = zero, subJ = zero, supAbove = zero;
-    if (interior) {
-        li = l[i];
-        rpi = rp[i];
-        ui = u[i];
+    cplx lk[K], rpk[K], uk[K], R[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const bool interior = r0 + k < ng - 1;
+        lk[k] = interior ? l[g0 + r0 + k] : zero;
+        rpk[k] = interior ? rp[g0 + r0 + k] : zero;
+        uk[k] = interior ? u[g0 + r0 + k] : zero;
     }
-    if (joint) subJ = sub[i];
-    if (t == 0 && g > 0) supAbove = sup[g0 - 1];
+    cplx subJ = zero, supAbove = zero;
+    if (live && lane == 0) {
+        subJ = sub[g0 + ng - 1];
+        if (g > 0) supAbove = sup[g0 - 1];
+    }
     pdl_wait();
-    cplx R = (t < ng) ? cadd(rD[i], rU[i]) : zero;
+#pragma unroll
+    for (int k = 0; k < K; ++k) R[k] = (r0 + k < ng) ? cadd(ld_dep(rD + g0 + r0 + k), ld_dep(rU + g0 + r0 + k)) : zero;
     pdl_launch_dependents();
-    // RD: D_i = R_i - l_i D_{i-1}, nothing enters the group (zero support values)
-    cplx A = cneg(li), B = interior ? R : zero;
-    cplx in = cta_scan_excl<+1>(A, B, zero, sA[0], sB[0]);
-    cplx D = cfma(A, in, B);
-    // RU + local solution: y_i = rp_i D_i - u_i y_{i+1}, y_joint = 0
-    A = cneg(ui);
-    B = cmul(rpi, D);
-    in = cta_scan_excl<-1>(A, B, zero, sA[1], sB[1]);
-    cplx y = cfma(A, in, B);
-    if (t == ng - 2) sY = y;
-    __syncthreads();
-    if (joint) outD[g] = (ng >= 2) ? cfnma(subJ, sY, R) : R;              // JD
-    if (t == 0 && g > 0) outU[g - 1] = (ng >= 2) ? cneg(cmul(supAbove, y)) : zero; // JU
+    // the joint line's own right-hand side (lane 0 needs it)
+    cplx Rj = zero;
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+        if (r0 + k == ng - 1) Rj = R[k];
+    Rj = shfl_c(Rj, ng > 0 ? (ng - 1) / K : 0);
+    // RD: D_i = R_i - l_i D_{i-1} on the interior rows, D := 0 on the joint line and beyond
+    cplx A = cmake(1.0, 0.0), B = zero;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        B = (r0 + k < ng - 1) ? cfnma(lk[k], B, R[k]) : zero;
+        A = cmul(cneg(lk[k]), A);
+    }
+    warp_scan_affine<+1, 5>(A, B, lane);
+    cplx in = shfl_up_c(B, 1);
+    if (lane == 0) in = zero;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        in = (r0 + k < ng - 1) ? cfnma(lk[k], in, R[k]) : zero;
+        R[k] = cmul(rpk[k], in); // rp_i D_i
+    }
+    // RU + local solution: y_i = rp_i D_i - u_i y_{i+1}, y := 0 on the joint line
+    A = cmake(1.0, 0.0);
+    B = zero;
+#pragma unroll
+    for (int k = K - 1; k >= 0; --k) {
+        B = cfnma(uk[k], B, R[k]);
+        A = cmul(cneg(uk[k]), A);
+    }
+    warp_scan_affine<-1, 5>(A, B, lane);
+    in = shfl_down_c(B, 1);
+    if (lane == 31) in = zero;
+    cplx yN = zero, y0 = zero; // y next to the own joint (row ng-2) and y of the first row
+#pragma unroll
+    for (int k = K - 1; k >= 0; --k) {
+        in = cfnma(uk[k], in, R[k]);
+        if (r0 + k == ng - 2) yN = in;
+        if (k == 0) y0 = in;
+    }
+    yN = shfl_c(yN, ng > 1 ? (ng - 2) / K : 0);
+    if (live && lane == 0) {
+        outD[g] = (ng >= 2) ? cfnma(subJ, yN, Rj) : Rj;                        // JD
+        if (g > 0) outU[g - 1] = (ng >= 2) ? cneg(cmul(supAbove, y0)) : zero; // JU
+    }
 }
 
-// ---- SS[M_i]: group g of level i from the support values of level i+1 ------------------------------------
-__global__ void __launch_bounds__(CN_RS_G, 4)
+// ---- SS[M_i]: group g of level i from the support values of level i+1 (one warp per group, as above) -------
+__global__ void __launch_bounds__(32 * CN_RS_WARPS)
 k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
            const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ Xup,
            cplx *__restrict__ X)
 {
-    __shared__ cplx sA[2][32], sB[2][32];
-    const int t = threadIdx.x;
-    const int64_t g = blockIdx.x, g0 = g * CN_RS_G;
-    const int ng = (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G);
-    const int64_t i = g0 + t;
-    const bool interior = t < ng - 1, joint = t == ng - 1;
+    constexpr int K = CN_RS_K;
+    const int lane = threadIdx.x & 31;
+    const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
+    const int64_t g = (int64_t)blockIdx.x * CN_RS_WARPS + (threadIdx.x >> 5);
+    const bool live = g < ngroups;
+    const int64_t g0 = g * CN_RS_G;
+    const int ng = live ? (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G) : 0;
+    const int r0 = lane * K;
     const cplx zero = cmake(0.0, 0.0);
-    cplx li = zero, rpi = zero, ui = zero;
-    if (interior) {
-        li = l[i];
-        rpi = rp[i];
-        ui = u[i];
+    cplx lk[K], rpk[K], uk[K], R[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const bool interior = r0 + k < ng - 1;
+        lk[k] = interior ? l[g0 + r0 + k] : zero;
+        rpk[k] = interior ? rp[g0 + r0 + k] : zero;
+        uk[k] = interior ? u[g0 + r0 + k] : zero;
+        R[k] = interior ? cadd(rD[g0 + r0 + k], rU[g0 + r0 + k]) : zero; // written two kernels ago: complete
     }
-    cplx R = interior ? cadd(rD[i], rU[i]) : zero; // written two kernels ago: complete
     pdl_wait();
-    const cplx XL = (g > 0) ? Xup[g - 1] : zero, XJ = Xup[g];
+    cplx XL = zero, XJ = zero;
+    if (live) {
+        if (g > 0) XL = ld_dep(Xup + g - 1);
+        XJ = ld_dep(Xup + g);
+    }
     pdl_launch_dependents();
-    cplx A = cneg(li), B = R;
-    if (t == 0 && interior) B = cfnma(li, XL, R); // the joint above carries its support value
-    cplx in = cta_scan_excl<+1>(A, B, zero, sA[0], sB[0]);
-    cplx D = cfma(A, in, B);
-    A = cneg(ui);
-    B = joint ? XJ : cmul(rpi, D);
-    in = cta_scan_excl<-1>(A, B, zero, sA[1], sB[1]);
-    cplx x = cfma(A, in, B);
-    if (t < ng) X[i] = x;
+    // RD with the support value of the joint above entering the first row (rp := 1 there, see the header)
+    cplx A = cmake(1.0, 0.0), B = (lane == 0) ? XL : zero;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        B = cfnma(lk[k], B, R[k]);
+        A = cmul(cneg(lk[k]), A);
+    }
+    warp_scan_affine<+1, 5>(A, B, lane);
+    cplx in = shfl_up_c(B, 1);
+    if (lane == 0) in = XL;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        in = cfnma(lk[k], in, R[k]);
+        R[k] = cmul(rpk[k], in);
+    }
+    // SS: x_i = rp_i D_i - u_i x_{i+1}, x := X_g on the joint line
+    A = cmake(1.0, 0.0);
+    B = zero;
+#pragma unroll
+    for (int k = K - 1; k >= 0; --k) {
+        B = (r0 + k == ng - 1) ? XJ : cfnma(uk[k], B, R[k]);
+        A = cmul(cneg(uk[k]), A);
+    }
+    warp_scan_affine<-1, 5>(A, B, lane);
+    in = shfl_down_c(B, 1);
+    if (lane == 31) in = zero;
+#pragma unroll
+    for (int k = K - 1; k >= 0; --k) {
+        in = (r0 + k == ng - 1) ? XJ : cfnma(uk[k], in, R[k]);
+        if (r0 + k < ng) X[g0 + r0 + k] = in;
+    }
 }
 
 // ======================================= factor side (once per plan) =======================================
