@@ -55,19 +55,22 @@ typedef enum {
     CN_OPT_TILE_THREADS = 2,/* threads per CTA of the tiled kernels: 0 = auto, else 64/128/256/512 (8 points per thread) */
     CN_OPT_RS_TOPMAX = 3,   /* largest reduced system solved by the single-CTA RS kernel (1..8192, default 4096);
                                a larger one is partitioned again into groups of 256 joint lines (next RS level) */
-    CN_OPT_USE_GRAPH = 4,   /* 1 = replay the per-step launches from a CUDA graph inside cn_step (default 0) */
+    CN_OPT_USE_GRAPH = 4,   /* reserved: accepted, no effect (small systems are stepped on chip, CN_OPT_ONCHIP) */
     CN_OPT_RS_LEVELS = 5,   /* 0 = auto (levels added while the system exceeds RS_TOPMAX), k >= 1 = exactly k nested
                                levels where possible (Eq. 6; CN_EINVAL at factorize if the last
                                level exceeds 8192 rows), -1 = paper-literal serial RS by one thread */
     CN_OPT_PROFILE = 6,     /* 1 = bracket every fused-pass and RS launch of cn_step with CUDA events on the
                                launching stream (read back with cn_plan_get_profile); default 0 */
-    CN_OPT_PDL = 7          /* 1 (default) = launch the per-step kernels with programmatic dependent launch so that
+    CN_OPT_PDL = 7,         /* 1 (default) = launch the per-step kernels with programmatic dependent launch so that
                                each kernel's independent prefetch overlaps the tail of its predecessor; 0 = plain */
+    CN_OPT_ONCHIP = 8       /* 1 (default) = a system of N <= 4096 points whose plan forces neither a path nor an RS
+                               structure is stepped by ONE single-CTA launch per cn_step call that keeps psi in
+                               registers and loops over the steps on chip (cn_plan_info.path = 3); 0 = never */
 } cn_option;
 
 typedef struct {
     int64_t N, P;
-    int32_t path;            /* 1 generic, 2 tiled */
+    int32_t path;            /* 1 generic, 2 tiled, 3 whole system on chip (N <= 4096) */
     int32_t tile_threads;    /* threads per CTA of the pass kernel (tiled path) */
     int64_t tile_points;     /* points per CTA (tiled path) */
     int32_t rs_levels;

@@ -17,6 +17,7 @@
 #include "cn_pass_tiled.cuh"
 #include "cn_reduced.cuh"
 #include "cn_batched.cuh"
+#include "cn_onchip.cuh"
 
 typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -60,7 +61,7 @@ struct cn_plan {
     };
     std::vector<rs_level> lv;
     // configuration
-    int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0;
+    int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
     int opt_pdl = 1;
     // profiling (CN_OPT_PROFILE): event pairs around fused-pass (kind 0) and RS (kind 1) launches
     struct ev_pair { cudaEvent_t a, b; int kind; };
@@ -253,6 +254,9 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
     case CN_OPT_USE_GRAPH:
         plan->opt_graph = value ? 1 : 0;
         return CN_OK;
+    case CN_OPT_ONCHIP:
+        plan->opt_onchip = value ? 1 : 0;
+        return CN_OK;
     case CN_OPT_RS_LEVELS:
         if (value < -1 || value > 8) return CN_EINVAL;
         plan->opt_rs_levels = (int)value;
@@ -265,13 +269,20 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
     return CN_EINVAL;
 }
 
+// the whole system is stepped on chip by one CTA (cn_onchip.cuh) when nothing asks for a particular kernel family
+static bool onchip_active(const cn_plan *p)
+{
+    return p->opt_onchip && p->opt_path == 0 && p->opt_rs_levels == 0 && !p->opt_profile && !p->ooc && p->qB &&
+           p->N <= CN_ONCHIP_NMAX;
+}
+
 extern "C" cn_status cn_plan_get_info(const cn_plan *plan, cn_plan_info *info)
 {
     if (!plan || !info) return CN_EINVAL;
     memset(info, 0, sizeof *info);
     info->N = plan->N; info->P = plan->Pu;
     info->P_effective = plan->P;
-    info->path = plan->path;
+    info->path = onchip_active(plan) ? 3 : plan->path;
     info->tile_threads = plan->tpb;
     info->tile_points = plan->ooc ? plan->partPts : (int64_t)plan->tpb * 8;
     info->rs_levels = (plan->opt_rs_levels < 0) ? -1 : (int32_t)plan->lv.size();
@@ -837,6 +848,22 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
     cplx *psi = (cplx *)psi_;
     cn_status st;
     if (p->ooc) return ooc_step(p, psi, nsteps, stream);
+    if (onchip_active(p)) {
+        // one launch for the whole call: psi, q and gamma are read once, the steps loop on chip
+        const int64_t chunks = (p->N + 7) / 8;
+        const bool pdl = p->opt_pdl != 0;
+        cudaError_t e;
+#define CN_ONCHIP(T) launch_k(k_onchip_steps<T>, 1u, (unsigned)T, 0, stream, pdl, p->N, nsteps, p->rho, psi, (const cplx *)p->qB, (const double *)p->gam)
+        if (chunks <= 32) e = CN_ONCHIP(32);
+        else if (chunks <= 64) e = CN_ONCHIP(64);
+        else if (chunks <= 128) e = CN_ONCHIP(128);
+        else if (chunks <= 256) e = CN_ONCHIP(256);
+        else e = CN_ONCHIP(512);
+#undef CN_ONCHIP
+        p->launches += 1;
+        if (e != cudaSuccess) return cuda_fail(p, e);
+        return CN_OK;
+    }
     if (p->path == 2 && p->tmPsiFor != psi_) {
         const int box_rows = p->tpb < 256 ? p->tpb : 256;
         if ((st = make_map(p, &p->tmPsi, psi_, 16, box_rows)) != CN_OK) return st;

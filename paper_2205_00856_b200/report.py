@@ -220,7 +220,7 @@ def main(argv=None):
     for name in [c.strip() for c in args.configs.split(",") if c.strip()]:
         if name == "C1":
             emit(run_1d(torch, "C1", peak))
-            emit(dict(run_1d(torch, "C1", peak, use_graph=1), variant="cuda_graph"))
+            emit(dict(run_1d(torch, "C1", peak, onchip=0), variant="three_kernels_per_step"))
         elif name == "C2":
             emit(run_1d(torch, "C2dense", peak, nsteps=100))
         elif name == "C3":

@@ -90,6 +90,30 @@ def test_tiled_path_random(N, P, tt):
     assert residual(dx, dt, V, psi, out1) <= TOL_RES
 
 
+ONCHIP_SHAPES = [2, 3, 8, 9, 64, 100, 255, 256, 257, 777, 1000, 2048, 4095, 4096]
+
+
+@pytest.mark.parametrize("N", ONCHIP_SHAPES)
+def test_onchip_path_random(N):
+    # whole system in the registers of one CTA, all steps inside one launch (cn_onchip.cuh): every CTA size,
+    # ragged last chunk, a single chunk; P is irrelevant to psi (reading R8)
+    V, psi = W.random_system(N, seed=31)
+    dx, dt = 0.1, 0.02
+    for nsteps in (1, 2, 25):
+        ref = O.step(dx, dt, V, psi, nsteps)
+        out, info = gpu_step(N, 1, dx, dt, V, psi, nsteps)
+        assert info["path"] == B.PATH_ONCHIP
+        err = np.max(np.abs(out - ref))
+        assert err <= TOL_PSI, (N, nsteps, err)
+    out1, _ = gpu_step(N, 1, dx, dt, V, psi, 1)
+    assert residual(dx, dt, V, psi, out1) <= TOL_RES
+    # the same plan with the on-chip stepper switched off takes the per-step kernels and agrees
+    out2, info2 = gpu_step(N, 1, dx, dt, V, psi, 3, onchip=0)
+    out3, _ = gpu_step(N, 1, dx, dt, V, psi, 3)
+    assert info2["path"] != B.PATH_ONCHIP
+    assert np.max(np.abs(out2 - out3)) <= 1e-12
+
+
 RS_CASES = [
     # (N, P, opts): nested RS levels, ragged last group, single-row groups, serial RS
     (1 << 13, 1 << 10, dict(rs_topmax=64)),            # 1024 -> 4 groups of 256
