@@ -63,9 +63,12 @@ typedef enum {
                                launching stream (read back with cn_plan_get_profile); default 0 */
     CN_OPT_PDL = 7,         /* 1 (default) = launch the per-step kernels with programmatic dependent launch so that
                                each kernel's independent prefetch overlaps the tail of its predecessor; 0 = plain */
-    CN_OPT_ONCHIP = 8       /* 1 (default) = a system of N <= 4096 points whose plan forces neither a path nor an RS
+    CN_OPT_ONCHIP = 8,      /* 1 (default) = a system of N <= 4096 points whose plan forces neither a path nor an RS
                                structure is stepped by ONE single-CTA launch per cn_step call that keeps psi in
                                registers and loops over the steps on chip (cn_plan_info.path = 3); 0 = never */
+    CN_OPT_RS_FUSED = 9     /* 1 (default) = the last two RS levels (group reduction, last-level solve, group
+                               substitution; Eq. 6) run as one kernel when the last level has at
+                               most 1024 rows and the grid fits the device; 0 = one kernel per stage */
 } cn_option;
 
 typedef struct {

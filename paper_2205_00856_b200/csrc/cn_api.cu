@@ -62,7 +62,10 @@ struct cn_plan {
     std::vector<rs_level> lv;
     // configuration
     int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
-    int opt_pdl = 1;
+    int opt_pdl = 1, opt_rs_fused = 1;
+    // fused last-two-levels RS kernel (cn_reduced.cuh k_rs_fused): arrival counter + published epoch, launch number
+    unsigned long long *rs_sync = nullptr, rs_epoch = 0;
+    bool rs_fused = false;
     // profiling (CN_OPT_PROFILE): event pairs around fused-pass (kind 0) and RS (kind 1) launches
     struct ev_pair { cudaEvent_t a, b; int kind; };
     std::vector<ev_pair> ev_pool;
@@ -125,6 +128,7 @@ static void free_factors(cn_plan *p)
     p->q = nullptr; p->gam = nullptr; p->lw = p->rq = p->uw = nullptr;
     p->slotD = p->slotU = nullptr; p->sup[0] = p->sup[1] = nullptr; p->work = nullptr; p->derr = nullptr;
     p->qB = nullptr;
+    p->rs_sync = nullptr; p->rs_epoch = 0; p->rs_fused = false;
     p->gamJ = nullptr;
     for (int b = 0; b < cn_plan::NB; ++b) { p->bPsi[b] = nullptr; p->bQ[b] = nullptr; p->bV[b] = nullptr; }
     p->factorized = false;
@@ -256,6 +260,10 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
         return CN_OK;
     case CN_OPT_ONCHIP:
         plan->opt_onchip = value ? 1 : 0;
+        return CN_OK;
+    case CN_OPT_RS_FUSED:
+        plan->opt_rs_fused = value ? 1 : 0;
+        plan->factorized = false;
         return CN_OK;
     case CN_OPT_RS_LEVELS:
         if (value < -1 || value > 8) return CN_EINVAL;
@@ -438,6 +446,8 @@ static cn_status ooc_setup(cn_plan *p, int64_t m)
     return CN_OK;
 }
 
+static cn_status rs_fused_setup(cn_plan *p, cudaStream_t stream);
+
 // ---- factorize ----------------------------------------------------------------------------------------
 extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
 {
@@ -619,6 +629,7 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
         CN_CUDA(p, cudaGetDevice(&dev));
         CN_CUDA(p, cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, dev));
     }
+    if ((st = rs_fused_setup(p, stream)) != CN_OK) return st;
     p->factorized = true;
     return CN_OK;
 }
@@ -722,6 +733,38 @@ static cudaError_t launch_top_k(cn_plan *p, const cn_plan::rs_level &L, cplx *X,
                     (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw, X);
 }
 
+typedef void (*rs_fused_t)(int64_t, const cplx *, const cplx *, const cplx *, const cplx *, const cplx *, const cplx *,
+                           const cplx *, cplx *, cplx *, int64_t, const cplx *, const cplx *, const cplx *, cplx *, cplx *,
+                           unsigned long long *, unsigned long long);
+static rs_fused_t rs_fused_kernel(int64_t ntop)
+{
+    const int64_t T = 32 * CN_RS_WARPS;
+    if (ntop <= T) return k_rs_fused<1>;
+    if (ntop <= 2 * T) return k_rs_fused<2>;
+    if (ntop <= 4 * T) return k_rs_fused<4>;
+    return k_rs_fused<8>;
+}
+
+// the last two RS levels run as ONE kernel when the last level is small and every CTA of the group level can be
+// resident at once (its CTAs wait for the one that solves the last level)
+static cn_status rs_fused_setup(cn_plan *p, cudaStream_t stream)
+{
+    p->rs_fused = false;
+    const int nlv = (int)p->lv.size();
+    if (!p->opt_rs_fused || p->opt_rs_levels < 0 || nlv < 2 || p->lv.back().n > CN_RS_FUSED_TOPMAX) return CN_OK;
+    int per_sm = 0;
+    CN_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)rs_fused_kernel(p->lv.back().n),
+                                                             32 * CN_RS_WARPS, 0));
+    const int64_t grid = (p->lv[nlv - 1].n + CN_RS_WARPS - 1) / CN_RS_WARPS;
+    if (per_sm < 1 || grid > (int64_t)per_sm * p->sms) return CN_OK;
+    cn_status st;
+    if ((st = dev_alloc(p, &p->rs_sync, 2)) != CN_OK) return st;
+    CN_CUDA(p, cudaMemsetAsync(p->rs_sync, 0, 2 * sizeof(unsigned long long), stream));
+    p->rs_epoch = 0;
+    p->rs_fused = true;
+    return CN_OK;
+}
+
 // RS of one step: (RD+RU+JD+JU) level by level, RS of the last level, SS level by level (Eq. 6)
 static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
 {
@@ -730,14 +773,23 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
     const int pi = prof_begin(p, 1, stream);
     cudaError_t e = cudaSuccess;
     p->lv[0].X = p->sup[out];
-    for (int i = 0; i + 1 < nlv && e == cudaSuccess; ++i) {
+    const int nsep = p->rs_fused ? nlv - 2 : nlv - 1; // group levels that run as separate reduce / subst kernels
+    for (int i = 0; i < nsep && e == cudaSuccess; ++i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
         e = launch_k(k_rs_reduce, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
                      (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
                      (const cplx *)L.sup, U.rD, U.rU);
         p->launches += 1;
     }
-    if (e == cudaSuccess) {
+    if (e == cudaSuccess && p->rs_fused) {
+        const cn_plan::rs_level &L = p->lv[nlv - 2], &U = p->lv[nlv - 1];
+        p->rs_epoch += 1;
+        e = launch_k(rs_fused_kernel(U.n), (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl,
+                     L.n, (const cplx *)L.rD, (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u,
+                     (const cplx *)L.sub, (const cplx *)L.sup, U.rD, U.rU, U.n, (const cplx *)p->lw, (const cplx *)p->rq,
+                     (const cplx *)p->uw, U.X, L.X, p->rs_sync, p->rs_epoch);
+        p->launches += 1;
+    } else if (e == cudaSuccess) {
         const cn_plan::rs_level &L = p->lv.back();
         if (p->opt_rs_levels < 0)
             e = launch_k(k_rs_serial, 1u, 32u, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU,
@@ -748,7 +800,7 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
         else e = launch_top_k<8>(p, L, L.X, stream, pdl);
         p->launches += 1;
     }
-    for (int i = nlv - 2; i >= 0 && e == cudaSuccess; --i) {
+    for (int i = nsep - 1; i >= 0 && e == cudaSuccess; --i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
         e = launch_k(k_rs_subst, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
                      (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X);

@@ -247,6 +247,7 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
         for (int j = 0; j < 8; ++j) v[j] = s_psi[t * 8 + (j ^ sw)];
         if (t > 0 && !sysFirst) vlo = s_psi[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
         if (t < TPB - 1 && !sysLast) vhi = s_psi[(t + 1) * 8 + ((t + 1) & 7)];
+        fence_proxy_async(); // generic reads above before the async-proxy refill below (see cn_pass_tiled.cuh)
         __syncthreads();
         if (t == 0 && tile + ncl < ntiles) issue_load(tile + ncl);
 
@@ -544,6 +545,7 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
         for (int j = 0; j < 16; ++j) v[j] = s_psi[(16 * g + j) * 8 + c];
         if (g > 0) vlo = s_psi[(16 * g - 1) * 8 + c];
         if (g < G - 1) vhi = s_psi[(16 * g + 16) * 8 + c];
+        fence_proxy_async(); // generic reads above before the async-proxy refill below (see cn_pass_tiled.cuh)
         __syncthreads();
         if (t == 0 && strip + ncl < nstrips) issue_load(strip + ncl);
 

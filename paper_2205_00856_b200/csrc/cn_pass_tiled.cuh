@@ -189,7 +189,12 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
         if (t < TPB - 1) vhi = s_psi[(t + 1) * 8 + ((t + 1) & 7)];
         if (!P1 && isFirst) jointAbove = vlo; // prologue: psi^0 of the joint above
 
-        // everybody has its copy: refill the input buffers with the next tile while this one is computed
+        // everybody has its copy: refill the input buffers with the next tile while this one is computed.
+        // The refill is a write of the ASYNC proxy (TMA); a CTA barrier alone orders only generic-proxy accesses, and
+        // shared-memory loads still queued in the LSU when the barrier opens were overtaken by a fast (L2-resident)
+        // TMA write: wrong halo values in the first chunks of a tile, about once in 20 calls at N = 2^21, m = 8.
+        // fence.proxy.async orders this thread's earlier generic reads before the later async-proxy writes.
+        fence_proxy_async();
         __syncthreads();
         if (t == 0 && tile + gridDim.x < ntiles) issue_loads(tile + gridDim.x);
 

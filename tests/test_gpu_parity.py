@@ -127,6 +127,15 @@ RS_CASES = [
     (1 << 13, 1 << 10, dict(rs_levels=-1)),             # paper-literal serial RS
     (1 << 13, 1 << 10, dict(pdl=0)),
     (5000, 700, dict(rs_topmax=16)),                    # generic path + nested RS
+    # the same structures with one kernel per RS stage instead of the fused last-two-levels kernel
+    (1 << 13, 1 << 10, dict(rs_topmax=64, rs_fused=0)),
+    (8 * 1000, 1000, dict(rs_topmax=64, rs_fused=0)),
+    (8 * 513, 513, dict(rs_topmax=2, rs_fused=0)),
+    (1 << 17, 1 << 14, dict(rs_fused=0)),
+    # fused kernel with 2, 4 and 8 last-level rows per thread (last level of 160 / 384 / 1024 rows)
+    (8 * 40960, 40960, dict()),
+    (8 * 98304, 98304, dict()),
+    (1 << 21, 1 << 18, dict()),
 ]
 
 
@@ -144,6 +153,23 @@ def test_rs_levels(N, P, opts):
         assert info["rs_levels"] == opts["rs_levels"]
     out1, _ = gpu_step(N, P, dx, dt, V, psi, 1, **opts)
     assert residual(dx, dt, V, psi, out1) <= TOL_RES
+
+
+@pytest.mark.parametrize("N,P,opts", [(1 << 21, 1 << 18, dict()), (1 << 21, 1 << 18, dict(pdl=0)),
+                                       (8 * 98304, 98304, dict()), (8 * 98304, 98304, dict(rs_fused=0))])
+def test_refill_race_stress(N, P, opts):
+    """Repeated fresh plans on L2-resident systems with m = 8: the shapes on which the TMA refill of the input tile
+    overtook shared-memory loads still queued behind the CTA barrier (about 1 call in 10 before the
+    fence.proxy.async in k_pass_tiled, hazards)."""
+    cfg = W.scaled(W.CONFIGS["C2dense"], N=N)
+    V, psi = W.potential(cfg), W.psi0(cfg)
+    dx, dt = 0.01, 0.005
+    ref = O.step(dx, dt, V, psi, 3)
+    worst = 0.0
+    for _ in range(40):
+        out, _ = gpu_step(N, P, dx, dt, V, psi, 3, **opts)
+        worst = max(worst, float(np.max(np.abs(out - ref))))
+    assert worst <= TOL_PSI, worst
 
 
 def test_config_c1_both_paths():
