@@ -62,7 +62,7 @@ struct cn_plan {
     std::vector<rs_level> lv;
     // configuration
     int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
-    int opt_pdl = 1, opt_rs_fused = 1;
+    int opt_pdl = 1, opt_rs_fused = 1, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0;
     // fused last-two-levels RS kernel (cn_reduced.cuh k_rs_fused): arrival counter + published epoch, launch number
     unsigned long long *rs_sync = nullptr, rs_epoch = 0;
     bool rs_fused = false;
@@ -260,6 +260,15 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
         return CN_OK;
     case CN_OPT_ONCHIP:
         plan->opt_onchip = value ? 1 : 0;
+        return CN_OK;
+    case CN_OPT_RS_GROUP:
+        if (value < 2 || value > (1 << 20)) return CN_EINVAL;
+        plan->opt_rs_group = (int)value;
+        plan->factorized = false;
+        return CN_OK;
+    case CN_OPT_RS_SERIAL_TOP:
+        plan->opt_rs_serial_top = value ? 1 : 0;
+        plan->factorized = false;
         return CN_OK;
     case CN_OPT_RS_FUSED:
         plan->opt_rs_fused = value ? 1 : 0;
@@ -514,9 +523,9 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
             const int nl = (int)p->lv.size();
             const bool want_more = (p->opt_rs_levels > 0) ? (nl < p->opt_rs_levels) : (n > topmax);
             if (!want_more || n <= 2) break;
-            n = (n + CN_RS_G - 1) / CN_RS_G;
+            n = (n + p->opt_rs_group - 1) / p->opt_rs_group;
         }
-        if (p->opt_rs_levels >= 0 && p->lv.back().n > 8 * CN_RS_TOP_THREADS) return CN_EINVAL;
+        if (p->opt_rs_levels >= 0 && !p->opt_rs_serial_top && p->lv.back().n > 8 * CN_RS_TOP_THREADS) return CN_EINVAL;
     }
     const int nlv = (int)p->lv.size();
     for (int i = 0; i < nlv; ++i) {
@@ -584,7 +593,7 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     }
     for (int i = 0; i + 1 < nlv; ++i) {
         cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, tmpA,
+        k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, (int64_t)p->opt_rs_group, L.sub, L.diag, L.sup, L.l, L.rp, L.u, tmpA,
                                                                          U.sub, U.diag, tmpB, U.sup, p->derr);
         k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB);
         p->launches += 2;
@@ -751,7 +760,7 @@ static cn_status rs_fused_setup(cn_plan *p, cudaStream_t stream)
 {
     p->rs_fused = false;
     const int nlv = (int)p->lv.size();
-    if (!p->opt_rs_fused || p->opt_rs_levels < 0 || nlv < 2 || p->lv.back().n > CN_RS_FUSED_TOPMAX) return CN_OK;
+    if (!p->opt_rs_fused || p->opt_rs_levels < 0 || p->opt_rs_serial_top || p->opt_rs_group != CN_RS_G || nlv < 2 || p->lv.back().n > CN_RS_FUSED_TOPMAX) return CN_OK;
     int per_sm = 0;
     CN_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)rs_fused_kernel(p->lv.back().n),
                                                              32 * CN_RS_WARPS, 0));
@@ -774,8 +783,15 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
     cudaError_t e = cudaSuccess;
     p->lv[0].X = p->sup[out];
     const int nsep = p->rs_fused ? nlv - 2 : nlv - 1; // group levels that run as separate reduce / subst kernels
+    const bool tg = p->opt_rs_group != CN_RS_G; // one thread per group of any size (paper-shaped, cn_reduced.cuh)
+    const int64_t G = p->opt_rs_group;
     for (int i = 0; i < nsep && e == cudaSuccess; ++i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
+        if (tg)
+            e = launch_k(k_rs_reduce_thread, (unsigned)((U.n + 63) / 64), 64u, 0, stream, pdl, L.n, G, (const cplx *)L.rD,
+                         (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
+                         (const cplx *)L.sup, L.X, U.rD, U.rU);
+        else
         e = launch_k(k_rs_reduce, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
                      (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
                      (const cplx *)L.sup, U.rD, U.rU);
@@ -791,7 +807,7 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
         p->launches += 1;
     } else if (e == cudaSuccess) {
         const cn_plan::rs_level &L = p->lv.back();
-        if (p->opt_rs_levels < 0)
+        if (p->opt_rs_levels < 0 || p->opt_rs_serial_top)
             e = launch_k(k_rs_serial, 1u, 32u, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU,
                          (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw, L.X);
         else if (L.n <= CN_RS_TOP_THREADS) e = launch_top_k<1>(p, L, L.X, stream, pdl);
@@ -802,6 +818,10 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
     }
     for (int i = nsep - 1; i >= 0 && e == cudaSuccess; --i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
+        if (tg)
+            e = launch_k(k_rs_subst_thread, (unsigned)((U.n + 63) / 64), 64u, 0, stream, pdl, L.n, G, (const cplx *)L.rD,
+                         (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X);
+        else
         e = launch_k(k_rs_subst, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
                      (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X);
         p->launches += 1;

@@ -471,6 +471,60 @@ k_rs_fused(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
     }
 }
 
+// ---- paper-shaped group kernels: ONE THREAD serves one group of G joint lines (any G) ------------------------
+// The multi-iteration GPU program of PAPER.md:276 ("interleaving" the block kernels for the nested method): the same
+// stages as k_rs_reduce / k_rs_subst by serial sweeps straight in global memory.  X of the level is the scratch for
+// rp_i D_i between the two sweeps.  Used when CN_OPT_RS_GROUP is not 256 (the nested-level study).
+__global__ void k_rs_reduce_thread(int64_t n, int64_t G, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
+                                   const cplx *__restrict__ l, const cplx *__restrict__ rp, const cplx *__restrict__ u,
+                                   const cplx *__restrict__ sub, const cplx *__restrict__ sup, cplx *scratch,
+                                   cplx *__restrict__ outD, cplx *__restrict__ outU)
+{
+    pdl_wait();
+    pdl_launch_dependents();
+    const int64_t ngroups = (n + G - 1) / G;
+    const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= ngroups) return;
+    const int64_t g0 = g * G, J = ((g0 + G < n) ? (g0 + G) : n) - 1;
+    const cplx zero = cmake(0.0, 0.0);
+    cplx D = zero;
+    for (int64_t i = g0; i < J; ++i) {
+        D = cfnma(l[i], D, cadd(ld_dep(rD + i), ld_dep(rU + i)));
+        scratch[i] = cmul(rp[i], D);
+    }
+    cplx y = zero, yN = zero;
+    for (int64_t i = J - 1; i >= g0; --i) {
+        y = cfnma(u[i], y, scratch[i]);
+        if (i == J - 1) yN = y;
+    }
+    const cplx RJ = cadd(ld_dep(rD + J), ld_dep(rU + J));
+    outD[g] = (J > g0) ? cfnma(sub[J], yN, RJ) : RJ;
+    if (g > 0) outU[g - 1] = (J > g0) ? cneg(cmul(sup[g0 - 1], y)) : zero;
+}
+
+__global__ void k_rs_subst_thread(int64_t n, int64_t G, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
+                                  const cplx *__restrict__ l, const cplx *__restrict__ rp, const cplx *__restrict__ u,
+                                  const cplx *__restrict__ Xup, cplx *X)
+{
+    pdl_wait();
+    pdl_launch_dependents();
+    const int64_t ngroups = (n + G - 1) / G;
+    const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= ngroups) return;
+    const int64_t g0 = g * G, J = ((g0 + G < n) ? (g0 + G) : n) - 1;
+    cplx D = (g > 0) ? ld_dep(Xup + g - 1) : cmake(0.0, 0.0);
+    for (int64_t i = g0; i < J; ++i) {
+        D = cfnma(l[i], D, cadd(ld_dep(rD + i), ld_dep(rU + i)));
+        X[i] = cmul(rp[i], D);
+    }
+    cplx x = ld_dep(Xup + g);
+    X[J] = x;
+    for (int64_t i = J - 1; i >= g0; --i) {
+        x = cfnma(u[i], x, X[i]);
+        X[i] = x;
+    }
+}
+
 // ======================================= factor side (once per plan) =======================================
 
 // level-0 reduced matrix from the block corner entries produced by k_factor_blocks (cn_factor.cuh)
@@ -498,17 +552,17 @@ __global__ void k_rs_assemble0(int64_t P, int64_t N, double rho, const double *_
 
 // one thread per group of a non-last level: local LU of the interior rows, responses to unit support
 // values, and from them the rows of the next level's matrix (the JD / JU matrix side)
-__global__ void k_rs_factor_level(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
+__global__ void k_rs_factor_level(int64_t n, int64_t G, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
                                   const cplx *__restrict__ sup, cplx *__restrict__ l, cplx *__restrict__ rp,
                                   cplx *__restrict__ u, cplx *__restrict__ tmp, cplx *__restrict__ sub2,
                                   cplx *__restrict__ diag2, cplx *__restrict__ diag2U, cplx *__restrict__ sup2,
                                   int *__restrict__ err)
 {
-    const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
+    const int64_t ngroups = (n + G - 1) / G;
     const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= ngroups) return;
-    const int64_t g0 = g * CN_RS_G;
-    const int64_t J = ((g0 + CN_RS_G < n) ? (g0 + CN_RS_G) : n) - 1;
+    const int64_t g0 = g * G;
+    const int64_t J = ((g0 + G < n) ? (g0 + G) : n) - 1;
     const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
     bool bad = false;
     cplx prp = one, psup = zero, Dal = one; // Dal: forward sweep of the response to X_{g-1} = 1

@@ -198,10 +198,45 @@ def p_sweep(torch, peak, name="C2dense"):
     return {"config": name + " P sweep", "N": cfg.N, "sqrtN": math.isqrt(cfg.N), "rows": rows, "fit": fits}
 
 
+def levels_study(torch, N=300000):
+    """Nested multi-iteration study (Eq. 8-9, Fig. 2) with the paper-shaped kernels:
+    one thread per block, one thread per group at every nested level, serial last level.  n_it = number of
+    partition levels; for a given thread count P0 of the first iteration the later fan-outs are equal
+    (r = P0^(1/n_it), the optimal split of Eq. 8).  Predicted optimum "up to a fixed constant": P0* = N^(n_it/(n_it+1))."""
+    cfg = W.scaled(W.CONFIGS["C2dense"], N=N)
+    V, psi = _inputs(cfg)
+    d = torch.from_numpy(psi).cuda()
+    rows = []
+    for n_it in (1, 2, 3):
+        for k in range(4, 18):
+            P0 = 1 << k
+            if P0 > N // 2:
+                break
+            if n_it == 1:
+                opts = dict(path=B.PATH_GENERIC, rs_levels=-1)
+                r = None
+            else:
+                r = max(2, int(round(P0 ** (1.0 / n_it))))
+                r += (r == 256)  # 256 would select the warp-per-group kernels, not the paper-shaped ones
+                opts = dict(path=B.PATH_GENERIC, rs_levels=n_it, rs_group=r, rs_serial_top=1)
+            with B.Plan(cfg.N, P0, cfg.dx, cfg.dt, V, **opts) as plan:
+                plan.factorize()
+                best, _ = time_plan(torch, plan, d, 10, reps=3)
+            rows.append({"n_it": n_it, "P0": P0, "fanout": r, "us_per_cn_step": 1e3 * best})
+    summary = {}
+    for n_it in (1, 2, 3):
+        sel = [x for x in rows if x["n_it"] == n_it]
+        bestrow = min(sel, key=lambda x: x["us_per_cn_step"])
+        summary[n_it] = {"P0_measured_argmin": bestrow["P0"], "us_at_argmin": bestrow["us_per_cn_step"],
+                         "P0_predicted_eq8": N ** (n_it / (n_it + 1.0))}
+    return {"config": "nested levels study", "N": N, "rows": rows, "summary": summary}
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", default="C1,C2,C3,C4,C5")
     ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--levels", action="store_true", help="nested multi-iteration study at n_tot = 3e5")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
     import torch
@@ -231,6 +266,8 @@ def main(argv=None):
             emit(run_c5(torch))
     if args.sweep:
         emit(p_sweep(torch, peak))
+    if args.levels:
+        emit(levels_study(torch))
     return 0
 
 

@@ -132,6 +132,12 @@ RS_CASES = [
     (8 * 1000, 1000, dict(rs_topmax=64, rs_fused=0)),
     (8 * 513, 513, dict(rs_topmax=2, rs_fused=0)),
     (1 << 17, 1 << 14, dict(rs_fused=0)),
+    # paper-shaped nested levels: one thread per group of any size, serial last level
+    (8 * 1000, 1000, dict(rs_group=10, rs_levels=3, rs_serial_top=1)),
+    (1 << 13, 1 << 10, dict(rs_group=32, rs_levels=2)),
+    (5000, 700, dict(rs_group=7, rs_levels=3, rs_serial_top=1)),
+    (300000, 4489, dict(rs_group=67, rs_levels=2, rs_serial_top=1)),
+    (300000, 12167, dict(rs_group=23, rs_levels=3, rs_serial_top=1)),
     # fused kernel with 2, 4 and 8 last-level rows per thread (last level of 160 / 384 / 1024 rows)
     (8 * 40960, 40960, dict()),
     (8 * 98304, 98304, dict()),
