@@ -128,6 +128,21 @@ cn_status cn_factorize(cn_plan *plan, void *stream);
 cn_status cn_step(cn_plan *plan, void *psi, int64_t nsteps, void *stream);
 
 /*
+ * Time-dependent Hamiltonian (the propagator of a step uses H(t + dt/2); the laser-driven use
+ * case of PAPER.md:70).  H(t) = H0 + f(t) g(x): the potential of step k is V_j + field[k] g_j.
+ *   cn_plan_set_td_shape : g, N real values, HOST or DEVICE pointer, copied (e.g. g_j = x_j for a dipole term).
+ *   cn_step_td           : nsteps steps in place on the DEVICE vector psi; field = nsteps HOST values
+ *                          f(t_k + dt/2), read during the call.  Every step redoes the factorization on the device
+ *                          (launches only, no allocation, no synchronisation) and runs
+ *                          RHS + RD/RU/JD/JU -> RS -> SS with that step's factors; on return the plan again holds
+ *                          the factors of the static H.  Not available for out-of-core plans (CN_EINVAL);
+ *                          CN_EINVAL without a shape; a breakdown cannot occur for real V and g (T stays strictly
+ *                          diagonally dominant) and is not checked inside the loop.
+ */
+cn_status cn_plan_set_td_shape(cn_plan *plan, const double *g);
+cn_status cn_step_td(cn_plan *plan, void *psi, int64_t nsteps, const double *field, void *stream);
+
+/*
  * cn_batched_sweep -- the same step for nsys independent systems that share the plan's matrix
  * (operator splitting; config C4).  System k, row j lives at
  * psi[k * sys_stride + j * elem_stride] (strides in complex elements).  Supported layouts:

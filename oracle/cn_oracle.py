@@ -125,6 +125,19 @@ def step_inplace(dx: float, dt: float, V, psi, nsteps: int = 1, lean: bool = Fal
     return sec.value
 
 
+def step_td(dx: float, dt: float, V0, g, field, psi):
+    """Time-dependent H(t) = H0 + f(t) g(x) (the propagator of step k uses H at t_k + dt/2):
+    len(field) plain CN steps, step k with the potential V0 + field[k] * g -- the definition written out, one
+    full Thomas solve (with its own diagonals) per step.  Pinned in tests/test_oracle_pins.py by the closed-form
+    Cayley phases for a uniform shift g = 1, per-step dense LU, norm conservation and field = 0."""
+    V0 = np.ascontiguousarray(V0, dtype=np.float64)
+    g = np.ascontiguousarray(g, dtype=np.float64)
+    out = np.array(psi, dtype=np.complex128, copy=True)
+    for f in np.asarray(field, dtype=np.float64):
+        out = step(dx, dt, V0 + float(f) * g, out, 1)
+    return out
+
+
 def step_2d(dx: float, dt: float, Vx, Vy, psi, nsteps: int = 1, return_seconds: bool = False):
     """C4: psi[y][x] <- (CN_y(dt) CN_x(dt))^nsteps psi (reading R18)."""
     Vx = np.ascontiguousarray(Vx, dtype=np.float64)

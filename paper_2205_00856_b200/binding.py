@@ -20,7 +20,7 @@ PATH_AUTO, PATH_GENERIC, PATH_TILED, PATH_ONCHIP = 0, 1, 2, 3
 
 EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", "cn_factorize", "cn_step",
            "cn_batched_sweep", "cn_destroy", "cn_plan_get_info", "cn_plan_get_profile", "cn_status_string",
-           "cn_last_cuda_error", "cn_version"]
+           "cn_last_cuda_error", "cn_version", "cn_plan_set_td_shape", "cn_step_td"]
 
 
 class CnError(RuntimeError):
@@ -60,6 +60,10 @@ def lib():
         L.cn_factorize.argtypes = [vp, vp]
         L.cn_step.restype = i32
         L.cn_step.argtypes = [vp, vp, i64, vp]
+        L.cn_plan_set_td_shape.restype = i32
+        L.cn_plan_set_td_shape.argtypes = [vp, vp]
+        L.cn_step_td.restype = i32
+        L.cn_step_td.argtypes = [vp, vp, i64, vp, vp]
         L.cn_batched_sweep.restype = i32
         L.cn_batched_sweep.argtypes = [vp, vp, i64, i64, i64, i64, vp]
         L.cn_destroy.restype = i32
@@ -136,6 +140,17 @@ def cn_step(plan, psi, nsteps: int = 1, stream=None):
     _check(plan, lib().cn_step(plan, _ptr(psi), nsteps, _stream(stream)), "cn_step")
 
 
+def cn_plan_set_td_shape(plan, g):
+    _check(plan, lib().cn_plan_set_td_shape(plan, _ptr(g)), "cn_plan_set_td_shape")
+
+
+def cn_step_td(plan, psi, field, stream=None):
+    # field: host float64 array, one value f(t_k + dt/2) per step
+    import numpy as np
+    f = np.ascontiguousarray(field, dtype=np.float64)
+    _check(plan, lib().cn_step_td(plan, _ptr(psi), f.size, f.ctypes.data, _stream(stream)), "cn_step_td")
+
+
 def cn_batched_sweep(plan, psi, nsys: int, elem_stride: int, sys_stride: int, nsteps: int = 1, stream=None):
     _check(plan, lib().cn_batched_sweep(plan, _ptr(psi), nsys, elem_stride, sys_stride, nsteps, _stream(stream)),
            "cn_batched_sweep")
@@ -185,6 +200,12 @@ class Plan:
 
     def step(self, psi, nsteps=1, stream=None):
         cn_step(self.h, psi, nsteps, stream)
+
+    def set_td_shape(self, g):
+        cn_plan_set_td_shape(self.h, g)
+
+    def step_td(self, psi, field, stream=None):
+        cn_step_td(self.h, psi, field, stream)
 
     def batched_sweep(self, psi, nsys, elem_stride, sys_stride, nsteps=1, stream=None):
         cn_batched_sweep(self.h, psi, nsys, elem_stride, sys_stride, nsteps, stream)

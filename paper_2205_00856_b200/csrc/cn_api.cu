@@ -66,6 +66,11 @@ struct cn_plan {
     // fused last-two-levels RS kernel (cn_reduced.cuh k_rs_fused): arrival counter + published epoch, launch number
     unsigned long long *rs_sync = nullptr, rs_epoch = 0;
     bool rs_fused = false;
+    // time-dependent H (cn_step_td): spatial shape g of the driving term, the potential of the current step and the
+    // temporaries of the factorization kept alive so that cn_step_td never allocates
+    double *tdG = nullptr, *tdV = nullptr;
+    cplx *tdRed = nullptr;
+    int64_t tdRedP = 0;
     // profiling (CN_OPT_PROFILE): event pairs around fused-pass (kind 0) and RS (kind 1) launches
     struct ev_pair { cudaEvent_t a, b; int kind; };
     std::vector<ev_pair> ev_pool;
@@ -184,6 +189,9 @@ extern "C" cn_status cn_destroy(cn_plan *plan)
     if (!plan) return CN_EINVAL;
     free_factors(plan);
     if (plan->dV) cudaFree(plan->dV);
+    if (plan->tdG) cudaFree(plan->tdG);
+    if (plan->tdV) cudaFree(plan->tdV);
+    if (plan->tdRed) cudaFree(plan->tdRed);
     if (plan->hV) cudaFreeHost(plan->hV);
     if (plan->sIn) cudaStreamDestroy(plan->sIn);
     if (plan->sCmp) cudaStreamDestroy(plan->sCmp);
@@ -457,6 +465,63 @@ static cn_status ooc_setup(cn_plan *p, int64_t m)
 
 static cn_status rs_fused_setup(cn_plan *p, cudaStream_t stream);
 
+// The arithmetic of the factorization: every matrix-side quantity of RD/RU/JD/JU from the potential
+// `Vsrc`, the reduced matrices of all RS levels and their factors.  Launches only (no allocation, no synchronisation):
+// cn_factorize calls it once, cn_step_td once per step with the potential of that step.  `red`: 6 P complex scratch.
+static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64_t m, cudaStream_t stream, bool whole = true)
+{
+    const int64_t N = p->N, P = p->P;
+    const int nlv = (int)p->lv.size();
+    cn_status st;
+    cplx *redSubD = red, *redDiagD = red + P, *redSupU = red + 2 * P, *redDiagU = red + 3 * P;
+    cplx *tmpA = red + 4 * P, *tmpB = red + 5 * P;
+    CN_CUDA(p, cudaMemsetAsync(red, 0, sizeof(cplx) * 6 * (size_t)P, stream));
+    CN_CUDA(p, cudaMemsetAsync(p->derr, 0, sizeof(int), stream));
+    CN_CUDA(p, cudaMemsetAsync(p->slotU, 0, sizeof(cplx) * (size_t)P, stream));
+
+    cn_geom g{N, P};
+    const int T = 128;
+    if (!p->ooc) {
+        k_factor_blocks<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(g, p->two_dx2, p->rho, Vsrc, p->q, p->gam, redSubD,
+                                                                      redDiagD, redSupU, redDiagU, p->derr);
+    } else {
+        // stream V through the device once, part by part: only the corner entries of every block's inverse and
+        // gamma on the joint lines stay (O(P)); q and gamma are recomputed per part in every pass of cn_step
+        if ((st = ooc_setup(p, m)) != CN_OK) return st;
+        for (int64_t i = 0; i < p->nparts; ++i) {
+            const int b = (int)(i % cn_plan::NB);
+            const int64_t r0 = i * p->partPts, n = (N - r0 < p->partPts) ? (N - r0) : p->partPts;
+            CN_CUDA(p, cudaMemcpyAsync(p->bV[b], p->hV + r0, sizeof(double) * (size_t)n, cudaMemcpyHostToDevice, stream));
+            const int64_t nb = n / m;
+            k_factor_part<<<(unsigned)((nb + T - 1) / T), T, 0, stream>>>(nb, m, r0 / m, p->two_dx2, p->rho, p->bV[b], p->bQ[b],
+                                                                         p->bV[b], redSubD, redDiagD, redSupU, redDiagU,
+                                                                         p->derr);
+            k_joint_gamma<<<(unsigned)((nb + T - 1) / T), T, 0, stream>>>(nb, m, r0 / m, p->bV[b], p->gamJ);
+            p->launches += 2;
+        }
+    }
+    k_rs_assemble0<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(P, N, p->rho, p->gam, p->gamJ, redSubD, redDiagD, redSupU,
+                                                                 redDiagU, p->lv[0].sub, p->lv[0].diag, p->lv[0].sup);
+    p->launches += 2;
+    if (p->qB && whole) { // one block per system: the factors of cn_batched_sweep and of the on-chip stepper
+        k_factor_whole<<<1, 32, 0, stream>>>(N, p->rho, p->gam, p->qB, p->derr);
+        p->launches += 1;
+    }
+    for (int i = 0; i + 1 < nlv; ++i) {
+        cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
+        k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, (int64_t)p->opt_rs_group, L.sub, L.diag, L.sup, L.l, L.rp, L.u, tmpA,
+                                                                         U.sub, U.diag, tmpB, U.sup, p->derr);
+        k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB);
+        p->launches += 2;
+    }
+    {
+        cn_plan::rs_level &L = p->lv.back();
+        k_rs_factor_top<<<1, 32, 0, stream>>>(L.n, L.sub, L.diag, L.sup, p->lw, p->rq, p->uw, p->derr);
+        p->launches += 1;
+    }
+    return CN_OK;
+}
+
 // ---- factorize ----------------------------------------------------------------------------------------
 extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
 {
@@ -557,52 +622,7 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     // temporaries of the factorization (freed below)
     cplx *red = nullptr;
     CN_CUDA(p, cudaMalloc((void **)&red, sizeof(cplx) * 6 * (size_t)P));
-    cplx *redSubD = red, *redDiagD = red + P, *redSupU = red + 2 * P, *redDiagU = red + 3 * P;
-    cplx *tmpA = red + 4 * P, *tmpB = red + 5 * P;
-    CN_CUDA(p, cudaMemsetAsync(red, 0, sizeof(cplx) * 6 * (size_t)P, stream));
-    CN_CUDA(p, cudaMemsetAsync(p->derr, 0, sizeof(int), stream));
-    CN_CUDA(p, cudaMemsetAsync(p->slotU, 0, sizeof(cplx) * (size_t)P, stream));
-
-    cn_geom g{N, P};
-    const int T = 128;
-    if (!p->ooc) {
-        k_factor_blocks<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(g, p->two_dx2, p->rho, p->dV, p->q, p->gam, redSubD,
-                                                                      redDiagD, redSupU, redDiagU, p->derr);
-    } else {
-        // stream V through the device once, part by part: only the corner entries of every block's inverse and
-        // gamma on the joint lines stay (O(P)); q and gamma are recomputed per part in every pass of cn_step
-        if ((st = ooc_setup(p, m)) != CN_OK) { cudaFree(red); return st; }
-        for (int64_t i = 0; i < p->nparts; ++i) {
-            const int b = (int)(i % cn_plan::NB);
-            const int64_t r0 = i * p->partPts, n = (N - r0 < p->partPts) ? (N - r0) : p->partPts;
-            CN_CUDA(p, cudaMemcpyAsync(p->bV[b], p->hV + r0, sizeof(double) * (size_t)n, cudaMemcpyHostToDevice, stream));
-            const int64_t nb = n / m;
-            k_factor_part<<<(unsigned)((nb + T - 1) / T), T, 0, stream>>>(nb, m, r0 / m, p->two_dx2, p->rho, p->bV[b], p->bQ[b],
-                                                                         p->bV[b], redSubD, redDiagD, redSupU, redDiagU,
-                                                                         p->derr);
-            k_joint_gamma<<<(unsigned)((nb + T - 1) / T), T, 0, stream>>>(nb, m, r0 / m, p->bV[b], p->gamJ);
-            p->launches += 2;
-        }
-    }
-    k_rs_assemble0<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(P, N, p->rho, p->gam, p->gamJ, redSubD, redDiagD, redSupU,
-                                                                 redDiagU, p->lv[0].sub, p->lv[0].diag, p->lv[0].sup);
-    p->launches += 2;
-    if (p->qB) { // one block per system: the factors of cn_batched_sweep
-        k_factor_whole<<<1, 32, 0, stream>>>(N, p->rho, p->gam, p->qB, p->derr);
-        p->launches += 1;
-    }
-    for (int i = 0; i + 1 < nlv; ++i) {
-        cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, (int64_t)p->opt_rs_group, L.sub, L.diag, L.sup, L.l, L.rp, L.u, tmpA,
-                                                                         U.sub, U.diag, tmpB, U.sup, p->derr);
-        k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB);
-        p->launches += 2;
-    }
-    {
-        cn_plan::rs_level &L = p->lv.back();
-        k_rs_factor_top<<<1, 32, 0, stream>>>(L.n, L.sub, L.diag, L.sup, p->lw, p->rq, p->uw, p->derr);
-        p->launches += 1;
-    }
+    if ((st = factor_compute(p, p->dV, red, m, stream)) != CN_OK) { cudaFree(red); return st; }
     int herr = 0;
     cudaError_t e = cudaMemcpyAsync(&herr, p->derr, sizeof(int), cudaMemcpyDeviceToHost, stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
@@ -951,6 +971,69 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
         cur ^= 1;
     }
     return launch_pass(p, psi, 2, cur, stream);
+}
+
+// ---- time-dependent Hamiltonian (the propagator uses H(t + dt/2)) ---------------------
+// H(t) = H0 + f(t) g(x): V_j(t_k + dt/2) = V_j + f_k g_j, e.g. g = x and f = the laser field.  Every step
+// has its own T, so the factorization is redone on the device inside the step loop -- launches only,
+// no allocation, no synchronisation -- and a step is prologue (RHS + RD/RU/JD/JU) -> RS -> epilogue (SS) with the
+// factors of that step.  SS(k) cannot be fused with RD/RU(k+1) here: the two use different matrices.
+__global__ void k_td_potential(int64_t N, const double *__restrict__ V0, const double *__restrict__ g, double f,
+                               double *__restrict__ V)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) V[i] = fma(f, g[i], V0[i]);
+}
+
+extern "C" cn_status cn_plan_set_td_shape(cn_plan *p, const double *g)
+{
+    if (!p || !g) return CN_EINVAL;
+    if (!p->dV) return CN_EINVAL; // not for streamed (out-of-core) plans
+    const size_t vb = sizeof(double) * (size_t)p->N;
+    if (!p->tdG) {
+        CN_CUDA(p, cudaMalloc((void **)&p->tdG, vb));
+        CN_CUDA(p, cudaMalloc((void **)&p->tdV, vb));
+    }
+    CN_CUDA(p, cudaMemcpy(p->tdG, g, vb, cudaMemcpyDefault));
+    return CN_OK;
+}
+
+extern "C" cn_status cn_step_td(cn_plan *p, void *psi_, int64_t nsteps, const double *field, void *stream_)
+{
+    if (!p || !psi_ || nsteps < 0 || (nsteps > 0 && !field)) return CN_EINVAL;
+    if (((uintptr_t)psi_ & 15) != 0) return CN_EINVAL;
+    if (!p->factorized) return CN_ENOTFACTORIZED;
+    if (p->ooc || !p->tdG) return CN_EINVAL;
+    if (nsteps == 0) return CN_OK;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    cplx *psi = (cplx *)psi_;
+    cn_status st;
+    if (p->tdRedP != p->P) { // scratch of the factorization, sized for this partition (first call only)
+        if (p->tdRed) cudaFree(p->tdRed);
+        p->tdRed = nullptr;
+        CN_CUDA(p, cudaMalloc((void **)&p->tdRed, sizeof(cplx) * 6 * (size_t)p->P));
+        p->tdRedP = p->P;
+    }
+    if (p->path == 2 && p->tmPsiFor != psi_) {
+        const int box_rows = p->tpb < 256 ? p->tpb : 256;
+        if ((st = make_map(p, &p->tmPsi, psi_, 16, box_rows)) != CN_OK) return st;
+        p->tmPsiFor = psi_;
+    }
+    const int64_t m = (p->N % p->P == 0) ? p->N / p->P : 0;
+    const int T = 256;
+    for (int64_t k = 0; k < nsteps; ++k) {
+        k_td_potential<<<(unsigned)((p->N + T - 1) / T), T, 0, stream>>>(p->N, p->dV, p->tdG, field[k], p->tdV);
+        p->launches += 1;
+        if ((st = factor_compute(p, p->tdV, p->tdRed, m, stream, false)) != CN_OK) return st;
+        if ((st = launch_pass(p, psi, 0, /*cur=*/1, stream)) != CN_OK) return st;
+        if ((st = launch_rs(p, 1, stream)) != CN_OK) return st;
+        if ((st = launch_pass(p, psi, 2, /*cur=*/1, stream)) != CN_OK) return st;
+    }
+    // leave the plan with the factors of the static H again, so that cn_step keeps its meaning
+    if ((st = factor_compute(p, p->dV, p->tdRed, m, stream, false)) != CN_OK) return st;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    return CN_OK;
 }
 
 // ---- batched sweep (config C4) --------------------------------------------------------------------------

@@ -198,6 +198,32 @@ def p_sweep(torch, peak, name="C2dense"):
     return {"config": name + " P sweep", "N": cfg.N, "sqrtN": math.isqrt(cfg.N), "rows": rows, "fit": fits}
 
 
+def run_td(torch, peak, name="C2dense", nsteps=20):
+    """Driven steps (H(t) = H0 + f(t) x, cn_step_td): factorization inside the step loop, two passes per step."""
+    cfg = W.CONFIGS[name]
+    V, psi = _inputs(cfg)
+    d = torch.from_numpy(psi).cuda()
+    x = W.grid(cfg)
+    t = (np.arange(nsteps) + 0.5) * cfg.dt
+    field = 0.05 * np.sin(0.3 * t)
+    with B.Plan(cfg.N, cfg.P, cfg.dx, cfg.dt, V) as plan:
+        plan.factorize()
+        plan.set_td_shape(x)
+        plan.step_td(d, field[:2])
+        torch.cuda.synchronize()
+        ms = []
+        for _ in range(3):
+            e0, e1 = _events(torch)
+            e0.record()
+            plan.step_td(d, field)
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1) / (nsteps + 1))  # + the restoring factorization at the end of a call
+    best = min(ms)
+    return {"config": name + " time-dependent H", "N": cfg.N, "P": cfg.P, "us_per_driven_step": 1e3 * best,
+            "Gpoint_steps_per_s": cfg.N / best / 1e6}
+
+
 def levels_study(torch, N=300000):
     """Nested multi-iteration study (Eq. 8-9, Fig. 2) with the paper-shaped kernels:
     one thread per block, one thread per group at every nested level, serial last level.  n_it = number of
@@ -264,6 +290,8 @@ def main(argv=None):
             emit(run_c4(torch, peak))
         elif name == "C5":
             emit(run_c5(torch))
+        elif name == "TD":
+            emit(run_td(torch, peak))
     if args.sweep:
         emit(p_sweep(torch, peak))
     if args.levels:

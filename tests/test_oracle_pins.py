@@ -359,3 +359,38 @@ def test_performance_model_optimum():
         pstar = math.sqrt(alpha / beta) * ntot ** g["model_optimum_exponent"]
         assert abs(P[k] - pstar) <= 1.0
         assert abs(t[k] - 2 * math.sqrt(alpha * beta * ntot)) / t[k] < 1e-8
+
+
+# ---- time-dependent H: oracle/cn_oracle.step_td ---------------------------------------------------
+def test_td_uniform_shift_closed_form():
+    """g = 1 (spatially uniform f(t)): T_k = T0 + i dt/2 f_k commutes with the Laplacian, so a Dirichlet sine mode is
+    multiplied at step k by the exact Cayley phase of lambda + f_k -- a closed form that pins the midpoint rule, the
+    sign of i and the order of the steps independently of the code."""
+    N, dx, dt = 97, 0.13, 0.021
+    rng = np.random.default_rng(5)
+    field = rng.uniform(-3.0, 3.0, 40)
+    j = np.arange(1, N + 1)
+    for k in (1, 5, N):
+        v = np.sin(np.pi * k * j / (N + 1)).astype(np.complex128)
+        lam = (1.0 - np.cos(np.pi * k / (N + 1))) / dx ** 2
+        phase = np.prod((1 - 0.5j * dt * (lam + field)) / (1 + 0.5j * dt * (lam + field)))
+        out = O.step_td(dx, dt, np.zeros(N), np.ones(N), field, v)
+        assert np.max(np.abs(out - phase * v)) <= 1e-12
+
+
+def test_td_dense_lu_per_step_and_norm():
+    N, dx, dt = 48, 0.2, 0.05
+    rng = np.random.default_rng(6)
+    V0, g = rng.uniform(-1, 1, N), rng.uniform(-2, 2, N)
+    field = rng.uniform(-1, 1, 7)
+    psi = rng.normal(size=N) + 1j * rng.normal(size=N)
+    ref = psi.copy()
+    lap = (np.diag(np.full(N, 2.0)) - np.diag(np.ones(N - 1), 1) - np.diag(np.ones(N - 1), -1)) / (2 * dx * dx)
+    for f in field:  # H typed out here, dense solve per step
+        H = lap + np.diag(V0 + f * g)
+        ref = np.linalg.solve(np.eye(N) + 0.5j * dt * H, (np.eye(N) - 0.5j * dt * H) @ ref)
+    out = O.step_td(dx, dt, V0, g, field, psi)
+    assert np.max(np.abs(out - ref)) <= 1e-12
+    assert abs(np.vdot(out, out).real / np.vdot(psi, psi).real - 1.0) <= 1e-12
+    # field = 0 is the static stepper
+    assert np.array_equal(O.step_td(dx, dt, V0, g, np.zeros(5), psi), O.step(dx, dt, V0, psi, 5))
