@@ -66,9 +66,10 @@ typedef enum {
     CN_OPT_ONCHIP = 8,      /* 1 (default) = a system of N <= 4096 points whose plan forces neither a path nor an RS
                                structure is stepped by ONE single-CTA launch per cn_step call that keeps psi in
                                registers and loops over the steps on chip (cn_plan_info.path = 3); 0 = never */
-    CN_OPT_RS_FUSED = 9,    /* 1 (default) = the last two RS levels (group reduction, last-level solve, group
+    CN_OPT_RS_FUSED = 9,    /* 1 = the last two RS levels (group reduction, last-level solve, group
                                substitution; Eq. 6) run as one kernel when the last level has at
-                               most 1024 rows and the grid fits the device; 0 = one kernel per stage */
+                               most 1024 rows and the grid fits the device; 0 (default) = one kernel per stage, which is
+                               1-2 % faster at C2 under programmatic dependent launch */
     CN_OPT_RS_GROUP = 10,   /* joint lines per group of a nested RS level (2..2^20, default 256): the fan-out
                                n_bl(i) / n_bl(i+1) of PAPER.md:239-247 Eq. 8; any value but 256 selects the
                                paper-shaped kernels in which one thread serves one group */

@@ -62,7 +62,7 @@ struct cn_plan {
     std::vector<rs_level> lv;
     // configuration
     int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
-    int opt_pdl = 1, opt_rs_fused = 1, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0;
+    int opt_pdl = 1, opt_rs_fused = 0, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0;
     // fused last-two-levels RS kernel (cn_reduced.cuh k_rs_fused): arrival counter + published epoch, launch number
     unsigned long long *rs_sync = nullptr, rs_epoch = 0;
     bool rs_fused = false;
@@ -482,8 +482,27 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
     cn_geom g{N, P};
     const int T = 128;
     if (!p->ooc) {
-        k_factor_blocks<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(g, p->two_dx2, p->rho, Vsrc, p->q, p->gam, redSubD,
-                                                                      redDiagD, redSupU, redDiagU, p->derr);
+        // blocks of 8 * 2^k <= 256 rows (the shapes of the tiled path): chunk-parallel pivots by the Moebius-map scan
+        int logc = -1;
+        if (m >= 8 && m <= 256 && (m & (m - 1)) == 0 && (N / 8) % 32 == 0) {
+            logc = 0;
+            while ((8LL << logc) < m) ++logc;
+        }
+        const int64_t nch = N / 8;
+        const unsigned gridc = (unsigned)((nch + 127) / 128);
+#define CN_FB(L) k_factor_blocks_chunked<L><<<gridc, 128, 0, stream>>>(nch, p->two_dx2, p->rho, Vsrc, p->q, p->gam, redSubD, redDiagD, redSupU, redDiagU, p->derr)
+        switch (logc) {
+        case 0: CN_FB(0); break;
+        case 1: CN_FB(1); break;
+        case 2: CN_FB(2); break;
+        case 3: CN_FB(3); break;
+        case 4: CN_FB(4); break;
+        case 5: CN_FB(5); break;
+        default:
+            k_factor_blocks<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(g, p->two_dx2, p->rho, Vsrc, p->q, p->gam, redSubD,
+                                                                          redDiagD, redSupU, redDiagU, p->derr);
+        }
+#undef CN_FB
     } else {
         // stream V through the device once, part by part: only the corner entries of every block's inverse and
         // gamma on the joint lines stay (O(P)); q and gamma are recomputed per part in every pass of cn_step
@@ -509,6 +528,10 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
     }
     for (int i = 0; i + 1 < nlv; ++i) {
         cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
+        if (p->opt_rs_group == CN_RS_G)
+            k_rs_factor_level_smem<<<(unsigned)((U.n + CN_RS_FL_WARPS - 1) / CN_RS_FL_WARPS), 32 * CN_RS_FL_WARPS, 0, stream>>>(
+                L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr);
+        else
         k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, (int64_t)p->opt_rs_group, L.sub, L.diag, L.sup, L.l, L.rp, L.u, tmpA,
                                                                          U.sub, U.diag, tmpB, U.sup, p->derr);
         k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB);
@@ -516,7 +539,7 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
     }
     {
         cn_plan::rs_level &L = p->lv.back();
-        k_rs_factor_top<<<1, 32, 0, stream>>>(L.n, L.sub, L.diag, L.sup, p->lw, p->rq, p->uw, p->derr);
+        k_rs_factor_top_smem<<<1, 32, 0, stream>>>(L.n, L.sub, L.diag, L.sup, p->lw, p->rq, p->uw, p->derr);
         p->launches += 1;
     }
     return CN_OK;

@@ -78,6 +78,149 @@ __global__ void k_factor_blocks(cn_geom g, double two_dx2, double rho, const dou
     if (bad) atomicExch(err, 1);
 }
 
+// ---- the same, chunk-parallel: one THREAD per chunk of 8 rows, a block = 2^LOGC consecutive lanes of a warp --------
+// The pivot recurrence q_i = 1 / (mu_i - q_{i-1}) is a Moebius map of q_{i-1}; maps compose as 2x2 matrices
+// [[a, b], [c, d]] : q -> (a q + b) / (c q + d), row i contributing [[0, 1], [-1, mu_i]].  Every thread multiplies the
+// matrices of its 8 rows, a segmented Kogge-Stone scan over the lanes of the block composes them (a block's first
+// chunk is entered by q = 0, so its map is the CONSTANT b / d and everything downstream of it is constant too), and
+// each thread then recomputes its own 8 pivots serially from its true inflow.  The upward pivots (only Z_{1,1} is
+// needed) are the same scan in the other direction.  Matrices are rescaled by their largest component after every
+// product (a Moebius map does not change when its matrix is scaled), so |mu|^m never overflows.
+// Memory: a thread reads 64 contiguous bytes of V and writes 128 of q and 64 of gamma -- whole sectors, against one
+// 8-byte access per row and per thread in k_factor_blocks (619 us at C2, P = 2^17; this kernel: see DESIGN.md 8c).
+struct cn_mob {
+    cplx a, b, c, d;
+};
+CN_DEVINL cn_mob mob_row(cn_mob M, cplx mu) // [[0, 1], [-1, mu]] * M
+{
+    cn_mob R;
+    R.a = M.c;
+    R.b = M.d;
+    R.c = csub(cmul(mu, M.c), M.a);
+    R.d = csub(cmul(mu, M.d), M.b);
+    return R;
+}
+CN_DEVINL cn_mob mob_mul(cn_mob H, cn_mob L) // H * L : first L, then H
+{
+    cn_mob R;
+    R.a = cfma(H.a, L.a, cmul(H.b, L.c));
+    R.b = cfma(H.a, L.b, cmul(H.b, L.d));
+    R.c = cfma(H.c, L.a, cmul(H.d, L.c));
+    R.d = cfma(H.c, L.b, cmul(H.d, L.d));
+    return R;
+}
+CN_DEVINL cn_mob mob_scale(cn_mob M)
+{
+    double s = fmax(fmax(fmax(fabs(M.a.x), fabs(M.a.y)), fmax(fabs(M.b.x), fabs(M.b.y))),
+                    fmax(fmax(fabs(M.c.x), fabs(M.c.y)), fmax(fabs(M.d.x), fabs(M.d.y))));
+    const double r = (s > 0.0 && isfinite(s)) ? 1.0 / s : 1.0;
+    M.a = cmake(M.a.x * r, M.a.y * r);
+    M.b = cmake(M.b.x * r, M.b.y * r);
+    M.c = cmake(M.c.x * r, M.c.y * r);
+    M.d = cmake(M.d.x * r, M.d.y * r);
+    return M;
+}
+CN_DEVINL cn_mob mob_shfl(cn_mob M, int src)
+{
+    cn_mob R;
+    R.a = shfl_c(M.a, src);
+    R.b = shfl_c(M.b, src);
+    R.c = shfl_c(M.c, src);
+    R.d = shfl_c(M.d, src);
+    return R;
+}
+
+template <int LOGC>
+__global__ void __launch_bounds__(128)
+k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const double *__restrict__ V,
+                        cplx *__restrict__ q, double *__restrict__ gam, cplx *__restrict__ redSubD,
+                        cplx *__restrict__ redDiagD, cplx *__restrict__ redSupU, cplx *__restrict__ redDiagU,
+                        int *__restrict__ err)
+{
+    constexpr int CPB = 1 << LOGC;
+    const int lane = threadIdx.x & 31;
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; // nchunks is a multiple of 32: whole warps
+    if (c >= nchunks) return;
+    const int pos = lane & (CPB - 1); // chunk position inside its block
+    const bool isFirst = pos == 0, isLast = pos == CPB - 1;
+    const int64_t w = c >> LOGC;
+    const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
+    double g[8];
+    {
+        const double2 *v2 = reinterpret_cast<const double2 *>(V + 8 * c);
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+            const double2 vv = v2[jj];
+            g[2 * jj] = fma(two_dx2, vv.x, 2.0);
+            g[2 * jj + 1] = fma(two_dx2, vv.y, 2.0);
+        }
+        double2 *g2 = reinterpret_cast<double2 *>(gam + 8 * c);
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) g2[jj] = make_double2(g[2 * jj], g[2 * jj + 1]);
+    }
+    const int nrow = isLast ? 7 : 8; // the joint line (row 7 of a block's last chunk) is not part of the recurrence
+    // ---- downward: inflow of every chunk -----------------------------------------------------------------
+    cn_mob M{one, zero, zero, one};
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+        if (j < nrow) M = mob_row(M, cmake(-g[j], rho));
+    if (isFirst) { M.a = zero; M.c = zero; } // entered by q = 0: the constant map b / d
+    M = mob_scale(M);
+#pragma unroll
+    for (int k = 0; k < LOGC; ++k) {
+        const int dd = 1 << k;
+        cn_mob S = mob_shfl(M, lane - dd < 0 ? 0 : lane - dd);
+        if (pos >= dd) M = mob_scale(mob_mul(M, S));
+    }
+    cn_mob Pm = mob_shfl(M, lane == 0 ? 0 : lane - 1); // inclusive map of the chunk above: a constant inside a block
+    cplx qin = isFirst ? zero : cmul(Pm.b, crecip(Pm.d));
+    bool bad = false;
+    cplx pp = one, qlast = zero; // product of (-q) over this chunk's rows except the block's last interior row
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        if (j < nrow) {
+            cplx p = cmake(-g[j] - qin.x, rho - qin.y);
+            if (!cfinite_nonzero(p)) bad = true;
+            qin = crecip(p);
+            q[8 * c + j] = qin;
+            if (!(isLast && j == 6)) pp = cmul(pp, cneg(qin));
+            qlast = qin;
+        }
+    }
+    if (isLast) q[8 * c + 7] = one;
+#pragma unroll
+    for (int k = 0; k < LOGC; ++k) { // product over the block, wanted at its last chunk
+        const int dd = 1 << k;
+        cplx sp = shfl_c(pp, lane - dd < 0 ? 0 : lane - dd);
+        if (pos >= dd) pp = cmul(pp, sp);
+    }
+    // ---- upward: only Z_{1,1} = qu of the block's first row ---------------------------------------------------
+    cn_mob U{one, zero, zero, one};
+#pragma unroll
+    for (int j = 7; j >= 0; --j)
+        if (j < nrow) U = mob_row(U, cmake(-g[j], rho));
+    if (isLast) { U.a = zero; U.c = zero; } // nothing enters from the joint line below
+    U = mob_scale(U);
+#pragma unroll
+    for (int k = 0; k < LOGC; ++k) {
+        const int dd = 1 << k;
+        cn_mob S = mob_shfl(U, lane + dd > 31 ? 31 : lane + dd);
+        if (pos + dd < CPB) U = mob_scale(mob_mul(U, S));
+    }
+    if (isLast) {
+        const cplx Zn1 = cmul(qlast, pp);
+        redSubD[w] = cneg(Zn1);
+        redDiagD[w] = cneg(qlast);
+        if (w > 0) redSupU[w - 1] = cneg(Zn1);
+    }
+    if (isFirst && w > 0) {
+        const cplx quf = cmul(U.b, crecip(U.d)); // with LOGC == 0 isFirst == isLast and U is already the constant map
+        if (!cfinite_nonzero(U.d)) bad = true;
+        redDiagU[w - 1] = cneg(quf);
+    }
+    if (bad) atomicExch(err, 1);
+}
+
 // The same for one streamed part of the system (out-of-core mode, cn_ooc.cuh): nb equal blocks of m rows whose
 // V / q / gamma live in part-local arrays; block wl of the part is block w0 + wl of the system.  red* may be
 // NULL (per-step recomputation of the factors: "neither the matrix nor the wavefunction ever need to be placed

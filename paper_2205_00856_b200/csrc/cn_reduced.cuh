@@ -608,6 +608,127 @@ __global__ void k_rs_factor_level(int64_t n, int64_t G, const cplx *__restrict__
     if (bad) atomicExch(err, 1);
 }
 
+// The same for groups of CN_RS_G = 256 rows with the group's rows staged in shared memory: one WARP per group loads
+// and stores its rows coalesced, lane 0 runs the (inherently serial) recurrences on shared memory.  The thread-per-
+// group kernel above pays a full global-memory latency per row (268 us for 512 groups at C2); this one 35 us.
+#define CN_RS_FL_WARPS 2
+__global__ void __launch_bounds__(32 * CN_RS_FL_WARPS)
+k_rs_factor_level_smem(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
+                       const cplx *__restrict__ sup, cplx *__restrict__ l, cplx *__restrict__ rp, cplx *__restrict__ u,
+                       cplx *__restrict__ sub2, cplx *__restrict__ diag2, cplx *__restrict__ diag2U,
+                       cplx *__restrict__ sup2, int *__restrict__ err)
+{
+    __shared__ cplx sm[CN_RS_FL_WARPS][4][CN_RS_G]; // sub -> l, diag -> rp, sup -> u, tmp
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
+    const int64_t g = (int64_t)blockIdx.x * CN_RS_FL_WARPS + wp;
+    if (g >= ngroups) return; // whole warps
+    const int64_t g0 = g * CN_RS_G;
+    const int ng = (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G);
+    const int nj = ng - 1; // interior rows; row nj is the joint line
+    cplx *sS = sm[wp][0], *sD = sm[wp][1], *sU = sm[wp][2], *sT = sm[wp][3];
+    for (int i = lane; i < ng; i += 32) {
+        sS[i] = sub[g0 + i];
+        sD[i] = diag[g0 + i];
+        sU[i] = sup[g0 + i];
+    }
+    __syncwarp();
+    const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
+    if (lane == 0) {
+        const cplx subJ = sS[nj], diagJ = sD[nj];
+        bool bad = false;
+        cplx prp = one, psup = zero, Dal = one;
+        for (int i = 0; i < nj; ++i) {
+            const cplx supi = sU[i];
+            cplx li = cmul(sS[i], prp);
+            cplx piv = cfnma(li, psup, sD[i]);
+            if (!cfinite_nonzero(piv)) bad = true;
+            cplx r = crecip(piv);
+            sS[i] = li;
+            sD[i] = r;
+            sU[i] = cmul(supi, r);
+            Dal = cneg(cmul(li, Dal));
+            sT[i] = Dal;
+            prp = r;
+            psup = supi;
+        }
+        sS[nj] = zero;
+        sD[nj] = zero;
+        sU[nj] = zero;
+        const bool has = nj > 0;
+        cplx al = zero, be = one, alLast = zero, beLast = zero;
+        for (int i = nj - 1; i >= 0; --i) {
+            al = cfnma(sU[i], al, cmul(sD[i], sT[i]));
+            be = cneg(cmul(sU[i], be));
+            if (i == nj - 1) {
+                alLast = al;
+                beLast = be;
+            }
+        }
+        sub2[g] = (g == 0) ? zero : (has ? cmul(subJ, alLast) : subJ);
+        diag2[g] = has ? cfma(subJ, beLast, diagJ) : diagJ;
+        if (g > 0) {
+            const cplx sa = sup[g0 - 1];
+            diag2U[g - 1] = has ? cmul(sa, al) : zero;
+            sup2[g - 1] = has ? cmul(sa, be) : sa;
+        }
+        if (g == ngroups - 1) {
+            diag2U[g] = zero;
+            sup2[g] = zero;
+        }
+        if (bad) atomicExch(err, 1);
+    }
+    __syncwarp();
+    for (int i = lane; i < ng; i += 32) {
+        l[g0 + i] = sS[i];
+        rp[g0 + i] = sD[i];
+        u[g0 + i] = sU[i];
+    }
+}
+
+// serial LU of the last level's matrix with the rows staged in shared memory, 256 at a time (one warp)
+__global__ void __launch_bounds__(32)
+k_rs_factor_top_smem(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
+                     const cplx *__restrict__ sup, cplx *__restrict__ lw, cplx *__restrict__ rq, cplx *__restrict__ uw,
+                     int *__restrict__ err)
+{
+    __shared__ cplx sS[CN_RS_G], sD[CN_RS_G], sU[CN_RS_G];
+    const int lane = threadIdx.x;
+    cplx rqprev = cmake(0.0, 0.0), supprev = cmake(0.0, 0.0);
+    bool bad = false;
+    for (int64_t c0 = 0; c0 < n; c0 += CN_RS_G) {
+        const int nc = (int)((n - c0 < CN_RS_G) ? (n - c0) : CN_RS_G);
+        for (int i = lane; i < nc; i += 32) {
+            sS[i] = sub[c0 + i];
+            sD[i] = diag[c0 + i];
+            sU[i] = sup[c0 + i];
+        }
+        __syncwarp();
+        if (lane == 0) {
+            for (int i = 0; i < nc; ++i) {
+                const cplx supi = sU[i];
+                cplx lq = (c0 + i > 0) ? cmul(sS[i], rqprev) : cmake(0.0, 0.0);
+                cplx piv = cfnma(lq, supprev, sD[i]);
+                if (!cfinite_nonzero(piv)) bad = true;
+                cplx r = crecip(piv);
+                sS[i] = lq;
+                sD[i] = r;
+                sU[i] = cmul(supi, r);
+                rqprev = r;
+                supprev = supi;
+            }
+        }
+        __syncwarp();
+        for (int i = lane; i < nc; i += 32) {
+            lw[c0 + i] = sS[i];
+            rq[c0 + i] = sD[i];
+            uw[c0 + i] = sU[i];
+        }
+        __syncwarp();
+    }
+    if (lane == 0 && bad) atomicExch(err, 1);
+}
+
 // diag += diagU (the two-writer accumulation of the next level's diagonal)
 __global__ void k_rs_add(int64_t n, cplx *__restrict__ diag, const cplx *__restrict__ diagU)
 {
@@ -615,24 +736,3 @@ __global__ void k_rs_add(int64_t n, cplx *__restrict__ diag, const cplx *__restr
     if (i < n) diag[i] = cadd(diag[i], diagU[i]);
 }
 
-// serial LU of the last level's matrix: lw_w = sub_w * rq_{w-1}, rq_w = 1 / pivot_w, uw_w = sup_w * rq_w
-__global__ void k_rs_factor_top(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
-                                const cplx *__restrict__ sup, cplx *__restrict__ lw, cplx *__restrict__ rq,
-                                cplx *__restrict__ uw, int *__restrict__ err)
-{
-    if (blockIdx.x != 0 || threadIdx.x != 0) return;
-    cplx rqprev = cmake(0.0, 0.0), supprev = cmake(0.0, 0.0);
-    bool bad = false;
-    for (int64_t w = 0; w < n; ++w) {
-        cplx lq = (w > 0) ? cmul(sub[w], rqprev) : cmake(0.0, 0.0);
-        cplx piv = cfnma(lq, supprev, diag[w]);
-        if (!cfinite_nonzero(piv)) bad = true;
-        cplx r = crecip(piv);
-        lw[w] = lq;
-        rq[w] = r;
-        uw[w] = cmul(sup[w], r);
-        rqprev = r;
-        supprev = sup[w];
-    }
-    if (bad) atomicExch(err, 1);
-}

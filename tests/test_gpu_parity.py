@@ -139,9 +139,12 @@ RS_CASES = [
     (300000, 4489, dict(rs_group=67, rs_levels=2, rs_serial_top=1)),
     (300000, 12167, dict(rs_group=23, rs_levels=3, rs_serial_top=1)),
     # fused kernel with 2, 4 and 8 last-level rows per thread (last level of 160 / 384 / 1024 rows)
-    (8 * 40960, 40960, dict()),
-    (8 * 98304, 98304, dict()),
-    (1 << 21, 1 << 18, dict()),
+    (8 * 40960, 40960, dict(rs_fused=1)),
+    (8 * 98304, 98304, dict(rs_fused=1)),
+    (1 << 21, 1 << 18, dict(rs_fused=1)),
+    (1 << 13, 1 << 10, dict(rs_topmax=64, rs_fused=1)),
+    (8 * 1000, 1000, dict(rs_topmax=64, rs_fused=1)),
+    (8 * 513, 513, dict(rs_topmax=2, rs_fused=1)),
 ]
 
 
@@ -162,7 +165,7 @@ def test_rs_levels(N, P, opts):
 
 
 @pytest.mark.parametrize("N,P,opts", [(1 << 21, 1 << 18, dict()), (1 << 21, 1 << 18, dict(pdl=0)),
-                                       (8 * 98304, 98304, dict()), (8 * 98304, 98304, dict(rs_fused=0))])
+                                       (8 * 98304, 98304, dict()), (8 * 98304, 98304, dict(rs_fused=1))])
 def test_refill_race_stress(N, P, opts):
     """Repeated fresh plans on L2-resident systems with m = 8: the shapes on which the TMA refill of the input tile
     overtook shared-memory loads still queued behind the CTA barrier (about 1 call in 10 before the
