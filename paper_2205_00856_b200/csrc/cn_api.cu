@@ -468,7 +468,8 @@ static cn_status rs_fused_setup(cn_plan *p, cudaStream_t stream);
 // The arithmetic of the factorization: every matrix-side quantity of RD/RU/JD/JU from the potential
 // `Vsrc`, the reduced matrices of all RS levels and their factors.  Launches only (no allocation, no synchronisation):
 // cn_factorize calls it once, cn_step_td once per step with the potential of that step.  `red`: 6 P complex scratch.
-static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64_t m, cudaStream_t stream, bool whole = true)
+static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64_t m, cudaStream_t stream, bool whole = true,
+                                const double *tdG = nullptr, double tdF = 0.0)
 {
     const int64_t N = p->N, P = p->P;
     const int nlv = (int)p->lv.size();
@@ -490,7 +491,7 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
         }
         const int64_t nch = N / 8;
         const unsigned gridc = (unsigned)((nch + 127) / 128);
-#define CN_FB(L) k_factor_blocks_chunked<L><<<gridc, 128, 0, stream>>>(nch, p->two_dx2, p->rho, Vsrc, p->q, p->gam, redSubD, redDiagD, redSupU, redDiagU, p->derr)
+#define CN_FB(L) k_factor_blocks_chunked<L><<<gridc, 128, 0, stream>>>(nch, p->two_dx2, p->rho, Vsrc, tdG, tdF, p->q, p->gam, redSubD, redDiagD, redSupU, redDiagU, p->derr)
         switch (logc) {
         case 0: CN_FB(0); break;
         case 1: CN_FB(1); break;
@@ -499,6 +500,11 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
         case 4: CN_FB(4); break;
         case 5: CN_FB(5); break;
         default:
+            if (tdG) { // the thread-per-block kernel takes the potential of the step ready-made
+                k_td_potential<<<(unsigned)((N + 255) / 256), 256, 0, stream>>>(N, Vsrc, tdG, tdF, p->tdV);
+                Vsrc = p->tdV;
+                p->launches += 1;
+            }
             k_factor_blocks<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(g, p->two_dx2, p->rho, Vsrc, p->q, p->gam, redSubD,
                                                                           redDiagD, redSupU, redDiagU, p->derr);
         }
@@ -539,7 +545,7 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
     }
     {
         cn_plan::rs_level &L = p->lv.back();
-        k_rs_factor_top_smem<<<1, 32, 0, stream>>>(L.n, L.sub, L.diag, L.sup, p->lw, p->rq, p->uw, p->derr);
+        k_rs_factor_top_scan<<<1, 32, 0, stream>>>(L.n, L.sub, L.diag, L.sup, p->lw, p->rq, p->uw, p->derr);
         p->launches += 1;
     }
     return CN_OK;
@@ -1001,12 +1007,6 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
 // has its own T, so the factorization is redone on the device inside the step loop -- launches only,
 // no allocation, no synchronisation -- and a step is prologue (RHS + RD/RU/JD/JU) -> RS -> epilogue (SS) with the
 // factors of that step.  SS(k) cannot be fused with RD/RU(k+1) here: the two use different matrices.
-__global__ void k_td_potential(int64_t N, const double *__restrict__ V0, const double *__restrict__ g, double f,
-                               double *__restrict__ V)
-{
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < N) V[i] = fma(f, g[i], V0[i]);
-}
 
 extern "C" cn_status cn_plan_set_td_shape(cn_plan *p, const double *g)
 {
@@ -1045,9 +1045,7 @@ extern "C" cn_status cn_step_td(cn_plan *p, void *psi_, int64_t nsteps, const do
     const int64_t m = (p->N % p->P == 0) ? p->N / p->P : 0;
     const int T = 256;
     for (int64_t k = 0; k < nsteps; ++k) {
-        k_td_potential<<<(unsigned)((p->N + T - 1) / T), T, 0, stream>>>(p->N, p->dV, p->tdG, field[k], p->tdV);
-        p->launches += 1;
-        if ((st = factor_compute(p, p->tdV, p->tdRed, m, stream, false)) != CN_OK) return st;
+        if ((st = factor_compute(p, p->dV, p->tdRed, m, stream, false, p->tdG, field[k])) != CN_OK) return st;
         if ((st = launch_pass(p, psi, 0, /*cur=*/1, stream)) != CN_OK) return st;
         if ((st = launch_rs(p, 1, stream)) != CN_OK) return st;
         if ((st = launch_pass(p, psi, 2, /*cur=*/1, stream)) != CN_OK) return st;

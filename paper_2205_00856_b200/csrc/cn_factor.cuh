@@ -133,6 +133,7 @@ CN_DEVINL cn_mob mob_shfl(cn_mob M, int src)
 template <int LOGC>
 __global__ void __launch_bounds__(128)
 k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const double *__restrict__ V,
+                        const double *__restrict__ tdG, double tdF, // potential = V + tdF * tdG when tdG != NULL (cn_step_td)
                         cplx *__restrict__ q, double *__restrict__ gam, cplx *__restrict__ redSubD,
                         cplx *__restrict__ redDiagD, cplx *__restrict__ redSupU, cplx *__restrict__ redDiagU,
                         int *__restrict__ err)
@@ -150,7 +151,12 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
         const double2 *v2 = reinterpret_cast<const double2 *>(V + 8 * c);
 #pragma unroll
         for (int jj = 0; jj < 4; ++jj) {
-            const double2 vv = v2[jj];
+            double2 vv = v2[jj];
+            if (tdG) {
+                const double2 gg = reinterpret_cast<const double2 *>(tdG + 8 * c)[jj];
+                vv.x = fma(tdF, gg.x, vv.x);
+                vv.y = fma(tdF, gg.y, vv.y);
+            }
             g[2 * jj] = fma(two_dx2, vv.x, 2.0);
             g[2 * jj + 1] = fma(two_dx2, vv.y, 2.0);
         }
@@ -219,6 +225,14 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
         redDiagU[w - 1] = cneg(quf);
     }
     if (bad) atomicExch(err, 1);
+}
+
+// potential of one driven step, V + f g (cn_step_td with the thread-per-block factor kernel)
+__global__ void k_td_potential(int64_t N, const double *__restrict__ V0, const double *__restrict__ g, double f,
+                               double *__restrict__ V)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) V[i] = fma(f, g[i], V0[i]);
 }
 
 // The same for one streamed part of the system (out-of-core mode, cn_ooc.cuh): nb equal blocks of m rows whose

@@ -22,6 +22,7 @@
 // rp_i = 1 / pivot_i,  u_i = sup_i * rp_i.
 #pragma once
 #include "cn_common.cuh"
+#include "cn_factor.cuh" // cn_mob
 
 #define CN_RS_G 256          // joint lines per group
 #define CN_RS_TOP_THREADS 1024
@@ -686,47 +687,54 @@ k_rs_factor_level_smem(int64_t n, const cplx *__restrict__ sub, const cplx *__re
     }
 }
 
-// serial LU of the last level's matrix with the rows staged in shared memory, 256 at a time (one warp)
+// LU of the last level's matrix by ONE WARP: rq_i = 1 / (diag_i - sub_i sup_{i-1} rq_{i-1}) is a Moebius map of
+// rq_{i-1} (row matrix [[0, 1], [-sub_i sup_{i-1}, diag_i]], cn_factor.cuh); every lane composes the maps of its
+// ceil(n/32) consecutive rows, a Kogge-Stone scan over the lanes gives each lane its inflow (row 0 has sub = 0, so
+// everything is a constant map), and the lane recomputes its rows serially.  lw_w = sub_w rq_{w-1}, uw_w = sup_w rq_w.
 __global__ void __launch_bounds__(32)
-k_rs_factor_top_smem(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
+k_rs_factor_top_scan(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
                      const cplx *__restrict__ sup, cplx *__restrict__ lw, cplx *__restrict__ rq, cplx *__restrict__ uw,
                      int *__restrict__ err)
 {
-    __shared__ cplx sS[CN_RS_G], sD[CN_RS_G], sU[CN_RS_G];
     const int lane = threadIdx.x;
-    cplx rqprev = cmake(0.0, 0.0), supprev = cmake(0.0, 0.0);
-    bool bad = false;
-    for (int64_t c0 = 0; c0 < n; c0 += CN_RS_G) {
-        const int nc = (int)((n - c0 < CN_RS_G) ? (n - c0) : CN_RS_G);
-        for (int i = lane; i < nc; i += 32) {
-            sS[i] = sub[c0 + i];
-            sD[i] = diag[c0 + i];
-            sU[i] = sup[c0 + i];
-        }
-        __syncwarp();
-        if (lane == 0) {
-            for (int i = 0; i < nc; ++i) {
-                const cplx supi = sU[i];
-                cplx lq = (c0 + i > 0) ? cmul(sS[i], rqprev) : cmake(0.0, 0.0);
-                cplx piv = cfnma(lq, supprev, sD[i]);
-                if (!cfinite_nonzero(piv)) bad = true;
-                cplx r = crecip(piv);
-                sS[i] = lq;
-                sD[i] = r;
-                sU[i] = cmul(supi, r);
-                rqprev = r;
-                supprev = supi;
-            }
-        }
-        __syncwarp();
-        for (int i = lane; i < nc; i += 32) {
-            lw[c0 + i] = sS[i];
-            rq[c0 + i] = sD[i];
-            uw[c0 + i] = sU[i];
-        }
-        __syncwarp();
+    const int64_t R = (n + 31) / 32, i0 = lane * R, i1 = (i0 + R < n) ? (i0 + R) : n;
+    const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
+    cn_mob M{one, zero, zero, one};
+    cplx supprev = (i0 > 0 && i0 < n) ? sup[i0 - 1] : zero;
+    const cplx sup0 = supprev;
+    for (int64_t i = i0; i < i1; ++i) {
+        const cplx ci = (i > 0) ? cmul(sub[i], supprev) : zero, di = diag[i];
+        cn_mob Rm; // [[0, 1], [-c_i, d_i]] * M
+        Rm.a = M.c;
+        Rm.b = M.d;
+        Rm.c = csub(cmul(di, M.c), cmul(ci, M.a));
+        Rm.d = csub(cmul(di, M.d), cmul(ci, M.b));
+        M = mob_scale(Rm);
+        supprev = sup[i];
     }
-    if (lane == 0 && bad) atomicExch(err, 1);
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const int dd = 1 << k;
+        cn_mob S = mob_shfl(M, lane - dd < 0 ? 0 : lane - dd);
+        if (lane >= dd) M = mob_scale(mob_mul(M, S));
+    }
+    cn_mob Pm = mob_shfl(M, lane == 0 ? 0 : lane - 1);
+    cplx rqprev = (lane == 0) ? zero : cmul(Pm.b, crecip(Pm.d));
+    bool bad = false;
+    supprev = sup0;
+    for (int64_t i = i0; i < i1; ++i) {
+        const cplx si = sup[i];
+        cplx lq = (i > 0) ? cmul(sub[i], rqprev) : zero;
+        cplx piv = cfnma(lq, supprev, diag[i]);
+        if (!cfinite_nonzero(piv)) bad = true;
+        cplx r = crecip(piv);
+        lw[i] = lq;
+        rq[i] = r;
+        uw[i] = cmul(si, r);
+        rqprev = r;
+        supprev = si;
+    }
+    if (bad) atomicExch(err, 1);
 }
 
 // diag += diagU (the two-writer accumulation of the next level's diagonal)
