@@ -71,15 +71,16 @@ class ClockSampler:
          "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index: int):
+    def __init__(self, index: int, interval_ms: int = 20):
         self.proc = None
         self.lines = []
         self.index = index
+        self.interval_ms = interval_ms
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "20"],
+                                          "--format=csv,noheader,nounits", "-lms", str(self.interval_ms)],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._pump, daemon=True)
             self.t.start()
@@ -169,6 +170,7 @@ def main():
     ap.add_argument("--cn-per-step", type=int, default=CN_PER_STEP)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--clock-interval-ms", type=int, default=20, help="nvidia-smi sampling period during the timed region")
     ap.add_argument("--sweep", action="store_true", help="also time the P sweep 2^8..2^16 (extra JSON key)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -225,7 +227,7 @@ def main():
         plan.step(d_psi, cn_per)
     torch.cuda.synchronize()
     launches0 = plan.info()["launches"]
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(local, args.clock_interval_ms)
     sampler.start()
     time.sleep(0.1)
     ms, w0, w1 = timed_region(lambda: plan.step(d_psi, cn_per), args.steps)

@@ -166,6 +166,21 @@ const char *cn_status_string(cn_status s);
 cn_status cn_last_cuda_error(const cn_plan *plan, int *cuda_err);
 const char *cn_version(void);
 
+/*
+ * General complex tridiagonal front end (Eq. 5):  b_i x_{i-1} + a_i x_i + c_i x_{i+1} = d_i,
+ * i = 1..N, x_0 = x_{N+1} = 0, ARBITRARY complex b, a, c (b_1 and c_N are ignored).  Solved by the same N-shaped
+ * partition scheme, nested: blocks of 256 rows, the last row of a block is its joint line.
+ *   cn_tridiag_create : b, a, c = N complex128 each, HOST or DEVICE pointers, copied; does all matrix-side work
+ *                        on `stream` and synchronises it once.  No pivoting (as in the paper):
+ *                       CN_EBREAKDOWN if a zero or non-finite pivot is met; diagonally dominant matrices are safe.
+ *   cn_tridiag_solve  : d, x = N complex128 DEVICE vectors (x may alias d); asynchronous on `stream`, no allocation.
+ *   cn_tridiag_destroy: frees everything.
+ */
+typedef struct cn_tridiag cn_tridiag;
+cn_status cn_tridiag_create(cn_tridiag **out, int64_t N, const void *b, const void *a, const void *c, void *stream);
+cn_status cn_tridiag_solve(cn_tridiag *t, const void *d, void *x, void *stream);
+cn_status cn_tridiag_destroy(cn_tridiag *t);
+
 #ifdef __cplusplus
 }
 #endif

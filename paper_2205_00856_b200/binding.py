@@ -20,7 +20,8 @@ PATH_AUTO, PATH_GENERIC, PATH_TILED, PATH_ONCHIP = 0, 1, 2, 3
 
 EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", "cn_factorize", "cn_step",
            "cn_batched_sweep", "cn_destroy", "cn_plan_get_info", "cn_plan_get_profile", "cn_status_string",
-           "cn_last_cuda_error", "cn_version", "cn_plan_set_td_shape", "cn_step_td"]
+           "cn_last_cuda_error", "cn_version", "cn_plan_set_td_shape", "cn_step_td",
+           "cn_tridiag_create", "cn_tridiag_solve", "cn_tridiag_destroy"]
 
 
 class CnError(RuntimeError):
@@ -64,6 +65,12 @@ def lib():
         L.cn_plan_set_td_shape.argtypes = [vp, vp]
         L.cn_step_td.restype = i32
         L.cn_step_td.argtypes = [vp, vp, i64, vp, vp]
+        L.cn_tridiag_create.restype = i32
+        L.cn_tridiag_create.argtypes = [ctypes.POINTER(vp), i64, vp, vp, vp, vp]
+        L.cn_tridiag_solve.restype = i32
+        L.cn_tridiag_solve.argtypes = [vp, vp, vp, vp]
+        L.cn_tridiag_destroy.restype = i32
+        L.cn_tridiag_destroy.argtypes = [vp]
         L.cn_batched_sweep.restype = i32
         L.cn_batched_sweep.argtypes = [vp, vp, i64, i64, i64, i64, vp]
         L.cn_destroy.restype = i32
@@ -174,6 +181,42 @@ def cn_plan_get_profile(plan) -> dict:
 
 def cn_version() -> str:
     return lib().cn_version().decode()
+
+
+class Tridiag:
+    """General complex tridiagonal system (cn_tridiag_*): marshalling only."""
+
+    def __init__(self, b, a, c, stream=None):
+        n = int(a.shape[0])
+        h = ctypes.c_void_p()
+        st = lib().cn_tridiag_create(ctypes.byref(h), n, _ptr(b), _ptr(a), _ptr(c), _stream(stream))
+        if st != CN_OK:
+            raise CnError(st, "cn_tridiag_create")
+        self.h, self.N = h, n
+
+    def solve(self, d, x=None, stream=None):
+        x = d if x is None else x
+        st = lib().cn_tridiag_solve(self.h, _ptr(d), _ptr(x), _stream(stream))
+        if st != CN_OK:
+            raise CnError(st, "cn_tridiag_solve")
+        return x
+
+    def close(self):
+        if self.h:
+            lib().cn_tridiag_destroy(self.h)
+            self.h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 class Plan:

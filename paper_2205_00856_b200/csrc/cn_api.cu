@@ -1057,6 +1057,120 @@ extern "C" cn_status cn_step_td(cn_plan *p, void *psi_, int64_t nsteps, const do
     return CN_OK;
 }
 
+// ---- general complex tridiagonal front end (Eq. 5) ---------------------------------------
+// b_i x_{i-1} + a_i x_i + c_i x_{i+1} = d_i for ARBITRARY complex b, a, c (non-constant off-diagonals, any N), solved
+// by the same N-shaped partition scheme: the system is handed to the nested-level machinery of cn_reduced.cuh as its
+// level 0 (groups of 256 rows = the blocks of PAPER.md:90-94, the last row of a group = its joint line; reduce =
+// RD+RU+JD+JU on the d-side, Eq. 6), so every kernel on this path is one the CN stepper already uses.
+struct cn_tridiag {
+    cn_plan *p = nullptr;
+    cplx *zero = nullptr; // the second right-hand-side slot of level 0, always 0 here
+};
+
+extern "C" cn_status cn_tridiag_destroy(cn_tridiag *t)
+{
+    if (!t) return CN_EINVAL;
+    if (t->p) {
+        free_factors(t->p);
+        delete t->p;
+    }
+    delete t;
+    return CN_OK;
+}
+
+extern "C" cn_status cn_tridiag_create(cn_tridiag **out, int64_t N, const void *b, const void *a, const void *c,
+                                       void *stream_)
+{
+    if (!out) return CN_EINVAL;
+    *out = nullptr;
+    if (N < 1 || !b || !a || !c) return CN_EINVAL;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    cn_tridiag *t = new (std::nothrow) cn_tridiag;
+    cn_plan *p = new (std::nothrow) cn_plan;
+    if (!t || !p) { delete t; delete p; return CN_ENOMEM; }
+    t->p = p;
+    p->N = N; p->P = N; p->Pu = N;
+    p->path = 1;
+    cn_status st = CN_OK;
+    auto fail = [&](cn_status e) { cn_tridiag_destroy(t); return e; };
+    {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+            return fail(CN_ECUDA);
+    }
+    // levels: n_0 = N, n_{i+1} = ceil(n_i / 256) while n_i > 4096
+    for (int64_t n = N;;) {
+        cn_plan::rs_level L;
+        L.n = n;
+        p->lv.push_back(L);
+        if (n <= p->opt_rs_topmax || n <= 2) break;
+        n = (n + CN_RS_G - 1) / CN_RS_G;
+    }
+    const int nlv = (int)p->lv.size();
+    for (int i = 0; i < nlv; ++i) {
+        cn_plan::rs_level &L = p->lv[i];
+        const size_t n = (size_t)L.n;
+        if ((st = dev_alloc(p, &L.sub, n)) != CN_OK || (st = dev_alloc(p, &L.diag, n)) != CN_OK ||
+            (st = dev_alloc(p, &L.sup, n)) != CN_OK)
+            return fail(st);
+        if (i < nlv - 1)
+            if ((st = dev_alloc(p, &L.l, n)) != CN_OK || (st = dev_alloc(p, &L.rp, n)) != CN_OK ||
+                (st = dev_alloc(p, &L.u, n)) != CN_OK)
+                return fail(st);
+        if (i > 0) {
+            if ((st = dev_alloc(p, &L.rD, n)) != CN_OK || (st = dev_alloc(p, &L.rU, n)) != CN_OK ||
+                (st = dev_alloc(p, &L.X, n)) != CN_OK)
+                return fail(st);
+            if (cudaMemsetAsync(L.rU, 0, sizeof(cplx) * n, stream) != cudaSuccess) return fail(CN_ECUDA);
+        }
+    }
+    const size_t ntop = (size_t)p->lv.back().n;
+    cplx *tmpB = nullptr;
+    if ((st = dev_alloc(p, &p->lw, ntop)) != CN_OK || (st = dev_alloc(p, &p->rq, ntop)) != CN_OK ||
+        (st = dev_alloc(p, &p->uw, ntop)) != CN_OK || (st = dev_alloc(p, &p->derr, 1)) != CN_OK ||
+        (st = dev_alloc(p, &t->zero, (size_t)N)) != CN_OK ||
+        (st = dev_alloc(p, &tmpB, (size_t)((N + CN_RS_G - 1) / CN_RS_G))) != CN_OK)
+        return fail(st);
+    cn_plan::rs_level &L0 = p->lv[0];
+    const size_t nb = sizeof(cplx) * (size_t)N;
+    if (cudaMemsetAsync(t->zero, 0, nb, stream) != cudaSuccess || cudaMemsetAsync(p->derr, 0, sizeof(int), stream) != cudaSuccess ||
+        cudaMemcpyAsync(L0.sub, b, nb, cudaMemcpyDefault, stream) != cudaSuccess ||
+        cudaMemcpyAsync(L0.diag, a, nb, cudaMemcpyDefault, stream) != cudaSuccess ||
+        cudaMemcpyAsync(L0.sup, c, nb, cudaMemcpyDefault, stream) != cudaSuccess ||
+        cudaMemsetAsync(L0.sub, 0, sizeof(cplx), stream) != cudaSuccess ||               // b_1 = 0
+        cudaMemsetAsync(L0.sup + (N - 1), 0, sizeof(cplx), stream) != cudaSuccess)       // c_N = 0
+        return fail(CN_ECUDA);
+    const int T = 128;
+    for (int i = 0; i + 1 < nlv; ++i) {
+        cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
+        k_rs_factor_level_smem<<<(unsigned)((U.n + CN_RS_FL_WARPS - 1) / CN_RS_FL_WARPS), 32 * CN_RS_FL_WARPS, 0, stream>>>(
+            L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr);
+        k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB);
+    }
+    k_rs_factor_top_scan<<<1, 32, 0, stream>>>(p->lv.back().n, p->lv.back().sub, p->lv.back().diag, p->lv.back().sup, p->lw,
+                                               p->rq, p->uw, p->derr);
+    int herr = 0;
+    if (cudaMemcpyAsync(&herr, p->derr, sizeof(int), cudaMemcpyDeviceToHost, stream) != cudaSuccess ||
+        cudaStreamSynchronize(stream) != cudaSuccess)
+        return fail(CN_ECUDA);
+    if (herr) return fail(CN_EBREAKDOWN);
+    p->factorized = true;
+    *out = t;
+    return CN_OK;
+}
+
+extern "C" cn_status cn_tridiag_solve(cn_tridiag *t, const void *d, void *x, void *stream_)
+{
+    if (!t || !t->p || !d || !x) return CN_EINVAL;
+    if ((((uintptr_t)d) & 15) != 0 || (((uintptr_t)x) & 15) != 0) return CN_EINVAL;
+    cn_plan *p = t->p;
+    cn_plan::rs_level &L0 = p->lv[0];
+    L0.rD = (cplx *)d; // read only
+    L0.rU = t->zero;
+    p->sup[0] = (cplx *)x;
+    return launch_rs(p, 0, (cudaStream_t)stream_);
+}
+
 // ---- batched sweep (config C4) --------------------------------------------------------------------------
 typedef void (*bx_kernel_t)(const CUtensorMap, const cn_bx_params);
 typedef void (*by_kernel_t)(const CUtensorMap, const cn_by_params);

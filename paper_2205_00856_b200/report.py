@@ -224,6 +224,36 @@ def run_td(torch, peak, name="C2dense", nsteps=20):
             "Gpoint_steps_per_s": cfg.N / best / 1e6}
 
 
+def run_tridiag(torch, peak, N=1 << 24):
+    """General complex tridiagonal front end (cn_tridiag_*): seeded random diagonally dominant system, solves per
+    second; algorithmic bytes per row and solve: the reduction reads l, rp, u, d and the zero slot (80 B), the
+    substitution reads them again and writes x (96 B) = 176 B."""
+    W.random_system  # the generators of the workloads module hold no arithmetic of the method
+    rng = np.random.default_rng(2205)
+    z = lambda: rng.normal(size=N) + 1j * rng.normal(size=N)
+    b, c, d = z(), z(), z()
+    a = (np.abs(b) + np.abs(c)) * 2.5 * np.exp(1j * rng.uniform(0, 2 * np.pi, N))
+    dd = torch.from_numpy(d).cuda()
+    xx = torch.empty_like(dd)
+    t0 = time.time()
+    with B.Tridiag(b, a, c) as t:
+        torch.cuda.synchronize()
+        fms = 1e3 * (time.time() - t0)
+        for _ in range(3):
+            t.solve(dd, xx)
+        torch.cuda.synchronize()
+        e0, e1 = _events(torch)
+        e0.record()
+        for _ in range(20):
+            t.solve(dd, xx)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 20
+    gbs = 176.0 * N / (ms * 1e-3) / 1e9
+    return {"config": "general tridiagonal", "N": N, "us_per_solve": 1e3 * ms, "Grows_per_s": N / ms / 1e6,
+            "bytes_per_row": 176, "GBps": gbs, "hbm_frac_measured_peak": gbs / peak, "create_ms": fms}
+
+
 def levels_study(torch, N=300000):
     """Nested multi-iteration study (Eq. 8-9, Fig. 2) with the paper-shaped kernels:
     one thread per block, one thread per group at every nested level, serial last level.  n_it = number of
@@ -292,6 +322,8 @@ def main(argv=None):
             emit(run_c5(torch))
         elif name == "TD":
             emit(run_td(torch, peak))
+        elif name == "TRI":
+            emit(run_tridiag(torch, peak))
     if args.sweep:
         emit(p_sweep(torch, peak))
     if args.levels:
