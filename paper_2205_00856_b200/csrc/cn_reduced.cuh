@@ -138,6 +138,37 @@ __global__ void k_rs_serial(int64_t n, const cplx *__restrict__ rD, const cplx *
 #define CN_RS_K (CN_RS_G / 32)
 #define CN_RS_WARPS 4 // groups per CTA of the group kernels
 
+// Coalesced transfer of one group's rows between global memory and the lanes' registers (lane t owns rows 8 t .. 8 t + 7)
+// through a swizzled 4 KB shared-memory buffer of the warp: a warp-level load touches 4 lines instead of 32.
+CN_DEVINL int rs_swz(int r) { return (r & ~7) | ((r ^ (r >> 3)) & 7); }
+template <bool DEP>
+CN_DEVINL void rs_load_rows(const cplx *__restrict__ src, int ng, cplx *sbuf, int lane, cplx (&out)[CN_RS_G / 32])
+{
+#pragma unroll
+    for (int k = 0; k < CN_RS_G / 32; ++k) {
+        const int r = k * 32 + lane;
+        cplx v = cmake(0.0, 0.0);
+        if (r < ng) v = DEP ? ld_dep(src + r) : src[r];
+        sbuf[rs_swz(r)] = v;
+    }
+    __syncwarp();
+#pragma unroll
+    for (int j = 0; j < CN_RS_G / 32; ++j) out[j] = sbuf[rs_swz(lane * 8 + j)];
+    __syncwarp();
+}
+CN_DEVINL void rs_store_rows(cplx *__restrict__ dst, int ng, cplx *sbuf, int lane, const cplx (&in)[CN_RS_G / 32])
+{
+#pragma unroll
+    for (int j = 0; j < CN_RS_G / 32; ++j) sbuf[rs_swz(lane * 8 + j)] = in[j];
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < CN_RS_G / 32; ++k) {
+        const int r = k * 32 + lane;
+        if (r < ng) dst[r] = sbuf[rs_swz(r)];
+    }
+    __syncwarp();
+}
+
 __global__ void __launch_bounds__(32 * CN_RS_WARPS)
 k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
             const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ sub,
@@ -152,22 +183,25 @@ k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
     const int ng = live ? (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G) : 0;
     const int r0 = lane * K; // first row of this lane inside the group
     const cplx zero = cmake(0.0, 0.0);
+    __shared__ cplx sbuf_all[CN_RS_WARPS][CN_RS_G];
+    cplx *const sbuf = sbuf_all[threadIdx.x >> 5];
     cplx lk[K], rpk[K], uk[K], R[K];
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-        const bool interior = r0 + k < ng - 1;
-        lk[k] = interior ? l[g0 + r0 + k] : zero;
-        rpk[k] = interior ? rp[g0 + r0 + k] : zero;
-        uk[k] = interior ? u[g0 + r0 + k] : zero;
-    }
+    rs_load_rows<false>(l + g0, ng - 1, sbuf, lane, lk); // rows >= ng - 1 (the joint line and beyond) read as 0
+    rs_load_rows<false>(rp + g0, ng - 1, sbuf, lane, rpk);
+    rs_load_rows<false>(u + g0, ng - 1, sbuf, lane, uk);
     cplx subJ = zero, supAbove = zero;
     if (live && lane == 0) {
         subJ = sub[g0 + ng - 1];
         if (g > 0) supAbove = sup[g0 - 1];
     }
     pdl_wait();
+    {
+        cplx Ru[K];
+        rs_load_rows<true>(rD + g0, ng, sbuf, lane, R);
+        rs_load_rows<true>(rU + g0, ng, sbuf, lane, Ru);
 #pragma unroll
-    for (int k = 0; k < K; ++k) R[k] = (r0 + k < ng) ? cadd(ld_dep(rD + g0 + r0 + k), ld_dep(rU + g0 + r0 + k)) : zero;
+        for (int k = 0; k < K; ++k) R[k] = cadd(R[k], Ru[k]);
+    }
     pdl_launch_dependents();
     // the joint line's own right-hand side (lane 0 needs it)
     cplx Rj = zero;
@@ -230,14 +264,18 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
     const int ng = live ? (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G) : 0;
     const int r0 = lane * K;
     const cplx zero = cmake(0.0, 0.0);
+    __shared__ cplx sbuf_all[CN_RS_WARPS][CN_RS_G];
+    cplx *const sbuf = sbuf_all[threadIdx.x >> 5];
     cplx lk[K], rpk[K], uk[K], R[K];
+    rs_load_rows<false>(l + g0, ng - 1, sbuf, lane, lk);
+    rs_load_rows<false>(rp + g0, ng - 1, sbuf, lane, rpk);
+    rs_load_rows<false>(u + g0, ng - 1, sbuf, lane, uk);
+    {
+        cplx Ru[K]; // the right-hand sides were written two kernels ago: complete (interior rows only)
+        rs_load_rows<false>(rD + g0, ng - 1, sbuf, lane, R);
+        rs_load_rows<false>(rU + g0, ng - 1, sbuf, lane, Ru);
 #pragma unroll
-    for (int k = 0; k < K; ++k) {
-        const bool interior = r0 + k < ng - 1;
-        lk[k] = interior ? l[g0 + r0 + k] : zero;
-        rpk[k] = interior ? rp[g0 + r0 + k] : zero;
-        uk[k] = interior ? u[g0 + r0 + k] : zero;
-        R[k] = interior ? cadd(rD[g0 + r0 + k], rU[g0 + r0 + k]) : zero; // written two kernels ago: complete
+        for (int k = 0; k < K; ++k) R[k] = cadd(R[k], Ru[k]);
     }
     pdl_wait();
     cplx XL = zero, XJ = zero;
@@ -275,8 +313,9 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
 #pragma unroll
     for (int k = K - 1; k >= 0; --k) {
         in = (r0 + k == ng - 1) ? XJ : cfnma(uk[k], in, R[k]);
-        if (r0 + k < ng) X[g0 + r0 + k] = in;
+        R[k] = in;
     }
+    rs_store_rows(X + g0, ng, sbuf, lane, R);
 }
 
 // ---- (RD+RU+JD+JU)[M_i] + RS[M_last] + SS[M_i] of the last two levels in ONE launch -----------------------------
