@@ -169,6 +169,33 @@ CN_DEVINL void rs_store_rows(cplx *__restrict__ dst, int ng, cplx *sbuf, int lan
     __syncwarp();
 }
 
+// The same for up to three arrays at once: all global loads are issued before the first shared-memory round trip, so a
+// warp pays one memory latency for the lot (sbuf: 3 buffers of CN_RS_G elements).
+template <bool DEP, int NA>
+CN_DEVINL void rs_load_rows_n(const cplx *const (&src)[NA], const int (&lim)[NA], cplx *sbuf, int lane,
+                              cplx (&out)[NA][CN_RS_G / 32])
+{
+    cplx tmp[NA][CN_RS_G / 32];
+#pragma unroll
+    for (int a = 0; a < NA; ++a)
+#pragma unroll
+        for (int k = 0; k < CN_RS_G / 32; ++k) {
+            const int r = k * 32 + lane;
+            tmp[a][k] = cmake(0.0, 0.0);
+            if (r < lim[a]) tmp[a][k] = DEP ? ld_dep(src[a] + r) : src[a][r];
+        }
+#pragma unroll
+    for (int a = 0; a < NA; ++a)
+#pragma unroll
+        for (int k = 0; k < CN_RS_G / 32; ++k) sbuf[a * CN_RS_G + rs_swz(k * 32 + lane)] = tmp[a][k];
+    __syncwarp();
+#pragma unroll
+    for (int a = 0; a < NA; ++a)
+#pragma unroll
+        for (int j = 0; j < CN_RS_G / 32; ++j) out[a][j] = sbuf[a * CN_RS_G + rs_swz(lane * 8 + j)];
+    __syncwarp();
+}
+
 __global__ void __launch_bounds__(32 * CN_RS_WARPS)
 k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
             const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ sub,
@@ -183,12 +210,15 @@ k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
     const int ng = live ? (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G) : 0;
     const int r0 = lane * K; // first row of this lane inside the group
     const cplx zero = cmake(0.0, 0.0);
-    __shared__ cplx sbuf_all[CN_RS_WARPS][CN_RS_G];
+    __shared__ cplx sbuf_all[CN_RS_WARPS][3 * CN_RS_G];
     cplx *const sbuf = sbuf_all[threadIdx.x >> 5];
-    cplx lk[K], rpk[K], uk[K], R[K];
-    rs_load_rows<false>(l + g0, ng - 1, sbuf, lane, lk); // rows >= ng - 1 (the joint line and beyond) read as 0
-    rs_load_rows<false>(rp + g0, ng - 1, sbuf, lane, rpk);
-    rs_load_rows<false>(u + g0, ng - 1, sbuf, lane, uk);
+    cplx F[3][K], R[K];
+    {   // rows >= ng - 1 (the joint line and beyond) read as 0
+        const cplx *const src[3] = {l + g0, rp + g0, u + g0};
+        const int lim[3] = {ng - 1, ng - 1, ng - 1};
+        rs_load_rows_n<false, 3>(src, lim, sbuf, lane, F);
+    }
+    cplx (&lk)[K] = F[0], (&rpk)[K] = F[1], (&uk)[K] = F[2];
     cplx subJ = zero, supAbove = zero;
     if (live && lane == 0) {
         subJ = sub[g0 + ng - 1];
@@ -196,11 +226,12 @@ k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
     }
     pdl_wait();
     {
-        cplx Ru[K];
-        rs_load_rows<true>(rD + g0, ng, sbuf, lane, R);
-        rs_load_rows<true>(rU + g0, ng, sbuf, lane, Ru);
+        cplx RR[2][K];
+        const cplx *const src[2] = {rD + g0, rU + g0};
+        const int lim[2] = {ng, ng};
+        rs_load_rows_n<true, 2>(src, lim, sbuf, lane, RR);
 #pragma unroll
-        for (int k = 0; k < K; ++k) R[k] = cadd(R[k], Ru[k]);
+        for (int k = 0; k < K; ++k) R[k] = cadd(RR[0][k], RR[1][k]);
     }
     pdl_launch_dependents();
     // the joint line's own right-hand side (lane 0 needs it)
@@ -264,18 +295,22 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
     const int ng = live ? (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G) : 0;
     const int r0 = lane * K;
     const cplx zero = cmake(0.0, 0.0);
-    __shared__ cplx sbuf_all[CN_RS_WARPS][CN_RS_G];
+    __shared__ cplx sbuf_all[CN_RS_WARPS][3 * CN_RS_G];
     cplx *const sbuf = sbuf_all[threadIdx.x >> 5];
-    cplx lk[K], rpk[K], uk[K], R[K];
-    rs_load_rows<false>(l + g0, ng - 1, sbuf, lane, lk);
-    rs_load_rows<false>(rp + g0, ng - 1, sbuf, lane, rpk);
-    rs_load_rows<false>(u + g0, ng - 1, sbuf, lane, uk);
+    cplx F[3][K], R[K];
     {
-        cplx Ru[K]; // the right-hand sides were written two kernels ago: complete (interior rows only)
-        rs_load_rows<false>(rD + g0, ng - 1, sbuf, lane, R);
-        rs_load_rows<false>(rU + g0, ng - 1, sbuf, lane, Ru);
+        const cplx *const src[3] = {l + g0, rp + g0, u + g0};
+        const int lim[3] = {ng - 1, ng - 1, ng - 1};
+        rs_load_rows_n<false, 3>(src, lim, sbuf, lane, F);
+    }
+    cplx (&lk)[K] = F[0], (&rpk)[K] = F[1], (&uk)[K] = F[2];
+    {   // the right-hand sides were written two kernels ago: complete (interior rows only)
+        cplx RR[2][K];
+        const cplx *const src[2] = {rD + g0, rU + g0};
+        const int lim[2] = {ng - 1, ng - 1};
+        rs_load_rows_n<false, 2>(src, lim, sbuf, lane, RR);
 #pragma unroll
-        for (int k = 0; k < K; ++k) R[k] = cadd(R[k], Ru[k]);
+        for (int k = 0; k < K; ++k) R[k] = cadd(RR[0][k], RR[1][k]);
     }
     pdl_wait();
     cplx XL = zero, XJ = zero;
