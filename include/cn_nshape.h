@@ -73,6 +73,9 @@ typedef enum {
     CN_OPT_RS_GROUP = 10,   /* joint lines per group of a nested RS level (2..2^20, default 256): the fan-out
                                n_bl(i) / n_bl(i+1) of PAPER.md:239-247 Eq. 8; any value but 256 selects the
                                paper-shaped kernels in which one thread serves one group */
+    CN_OPT_RS_TOP_IN_SUBST = 12, /* 1 (default) = a last level of at most 256 rows is solved inside the substitution
+                               kernel of the level below it, redundantly by every CTA (one launch less per step);
+                               a value v > 1 sets the row limit to min(v, 1024); 0 = always by its own kernel */
     CN_OPT_RS_SERIAL_TOP = 11 /* 1 = the LAST level is solved serially by one thread (the beta n_bl term of Eq. 8)
                                whatever the number of nested levels; default 0 = one CTA in parallel */
 } cn_option;

@@ -62,7 +62,8 @@ struct cn_plan {
     std::vector<rs_level> lv;
     // configuration
     int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
-    int opt_pdl = 1, opt_rs_fused = 0, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0;
+    int opt_pdl = 1, opt_rs_fused = 0, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0, opt_rs_top_in_subst = 1;
+    int64_t opt_rs_top_in_subst_max = 256; // measured at C2: faster up to 256 rows (160.8 vs 163.0 us), slower from 512 on
     // fused last-two-levels RS kernel (cn_reduced.cuh k_rs_fused): arrival counter + published epoch, launch number
     unsigned long long *rs_sync = nullptr, rs_epoch = 0;
     bool rs_fused = false;
@@ -277,6 +278,10 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
     case CN_OPT_RS_SERIAL_TOP:
         plan->opt_rs_serial_top = value ? 1 : 0;
         plan->factorized = false;
+        return CN_OK;
+    case CN_OPT_RS_TOP_IN_SUBST:
+        plan->opt_rs_top_in_subst = value ? 1 : 0;
+        plan->opt_rs_top_in_subst_max = value > 1 ? (value > 1024 ? 1024 : value) : 256; // value > 1: the row limit
         return CN_OK;
     case CN_OPT_RS_FUSED:
         plan->opt_rs_fused = value ? 1 : 0;
@@ -833,6 +838,9 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
     p->lv[0].X = p->sup[out];
     const int nsep = p->rs_fused ? nlv - 2 : nlv - 1; // group levels that run as separate reduce / subst kernels
     const bool tg = p->opt_rs_group != CN_RS_G; // one thread per group of any size (paper-shaped, cn_reduced.cuh)
+    // the last level is solved inside the substitution kernel of the level below it (one launch less per step)
+    const bool tis = !tg && !p->rs_fused && p->opt_rs_top_in_subst && p->opt_rs_levels >= 0 && !p->opt_rs_serial_top &&
+                     nlv >= 2 && p->lv.back().n <= p->opt_rs_top_in_subst_max;
     const int64_t G = p->opt_rs_group;
     for (int i = 0; i < nsep && e == cudaSuccess; ++i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
@@ -854,7 +862,7 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
                      (const cplx *)L.sub, (const cplx *)L.sup, U.rD, U.rU, U.n, (const cplx *)p->lw, (const cplx *)p->rq,
                      (const cplx *)p->uw, U.X, L.X, p->rs_sync, p->rs_epoch);
         p->launches += 1;
-    } else if (e == cudaSuccess) {
+    } else if (e == cudaSuccess && !tis) {
         const cn_plan::rs_level &L = p->lv.back();
         if (p->opt_rs_levels < 0 || p->opt_rs_serial_top)
             e = launch_k(k_rs_serial, 1u, 32u, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU,
@@ -870,9 +878,16 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
         if (tg)
             e = launch_k(k_rs_subst_thread, (unsigned)((U.n + 63) / 64), 64u, 0, stream, pdl, L.n, G, (const cplx *)L.rD,
                          (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X);
-        else
-        e = launch_k(k_rs_subst, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
-                     (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X);
+        else {
+            const unsigned gr = (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS);
+            const int64_t T = 32 * CN_RS_WARPS;
+            const int kt = (tis && i == nlv - 2) ? (U.n <= T ? 1 : (U.n <= 2 * T ? 2 : (U.n <= 4 * T ? 4 : 8))) : 0;
+#define CN_SUBST(KT) launch_k(k_rs_subst<KT>, gr, 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU, \
+                              (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X, U.n,                 \
+                              (const cplx *)U.rD, (const cplx *)U.rU, (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw)
+            e = kt == 0 ? CN_SUBST(0) : (kt == 1 ? CN_SUBST(1) : (kt == 2 ? CN_SUBST(2) : (kt == 4 ? CN_SUBST(4) : CN_SUBST(8))));
+#undef CN_SUBST
+        }
         p->launches += 1;
     }
     prof_end(p, pi, stream);

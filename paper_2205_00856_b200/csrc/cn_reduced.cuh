@@ -281,10 +281,15 @@ k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
 }
 
 // ---- SS[M_i]: group g of level i from the support values of level i+1 (one warp per group, as above) -------
+// KT > 0: the LAST level (ntop <= 128 KT rows) is solved inside this kernel, redundantly by every CTA, from the slots
+// topD / topU the reduction kernel just wrote -- one launch less on the per-step chain (reduce -> substitute instead
+// of reduce -> last level -> substitute); Xup is then not read.  KT == 0: Xup comes from k_rs_top.
+template <int KT>
 __global__ void __launch_bounds__(32 * CN_RS_WARPS)
 k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
            const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ Xup,
-           cplx *__restrict__ X)
+           cplx *__restrict__ X, int64_t ntop, const cplx *topD, const cplx *topU, const cplx *__restrict__ lw,
+           const cplx *__restrict__ rq, const cplx *__restrict__ uw)
 {
     constexpr int K = CN_RS_K;
     const int lane = threadIdx.x & 31;
@@ -312,13 +317,67 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
 #pragma unroll
         for (int k = 0; k < K; ++k) R[k] = cadd(RR[0][k], RR[1][k]);
     }
-    pdl_wait();
     cplx XL = zero, XJ = zero;
-    if (live) {
-        if (g > 0) XL = ld_dep(Xup + g - 1);
-        XJ = ld_dep(Xup + g);
+    if (KT > 0) {
+        // ---- RS[M_last] by the whole CTA (as k_rs_top), result in shared memory ------------------------------
+        constexpr int KK = KT > 0 ? KT : 1;
+        const int t = threadIdx.x;
+        const int64_t w0 = (int64_t)t * KK;
+        const cplx one = cmake(1.0, 0.0);
+        cplx tl[KK], tr[KK], tu[KK], tR[KK];
+#pragma unroll
+        for (int k = 0; k < KK; ++k) {
+            const bool in = w0 + k < ntop;
+            tl[k] = in ? lw[w0 + k] : zero;
+            tr[k] = in ? rq[w0 + k] : zero;
+            tu[k] = in ? uw[w0 + k] : zero;
+        }
+        pdl_wait();
+#pragma unroll
+        for (int k = 0; k < KK; ++k) tR[k] = (w0 + k < ntop) ? cadd(ld_dep(topD + w0 + k), ld_dep(topU + w0 + k)) : zero;
+        pdl_launch_dependents();
+        __syncthreads(); // every warp is done with its transfer buffer: the buffers become the scratch of the solve
+        cplx *const sX = &sbuf_all[0][0];                    // [32 * CN_RS_WARPS * 8] <= 1024 values
+        cplx *const sA = sX + 32 * CN_RS_WARPS * 8, *const sB = sA + 64; // [2][32] each
+        cplx A = one, B = zero;
+#pragma unroll
+        for (int k = 0; k < KK; ++k) {
+            B = cfnma(tl[k], B, tR[k]);
+            A = cmul(cneg(tl[k]), A);
+        }
+        cplx in = cta_scan_excl<+1>(A, B, zero, sA, sB);
+#pragma unroll
+        for (int k = 0; k < KK; ++k) {
+            in = cfnma(tl[k], in, tR[k]);
+            tR[k] = cmul(tr[k], in);
+        }
+        A = one;
+        B = zero;
+#pragma unroll
+        for (int k = KK - 1; k >= 0; --k) {
+            B = cfnma(tu[k], B, tR[k]);
+            A = cmul(cneg(tu[k]), A);
+        }
+        in = cta_scan_excl<-1>(A, B, zero, sA + 32, sB + 32);
+#pragma unroll
+        for (int k = KK - 1; k >= 0; --k) {
+            in = cfnma(tu[k], in, tR[k]);
+            if (w0 + k < ntop) sX[w0 + k] = in;
+        }
+        __syncthreads();
+        if (live) {
+            if (g > 0) XL = sX[g - 1];
+            XJ = sX[g];
+        }
+        __syncthreads(); // sX is read: the warps may use their transfer buffers again (rs_store_rows below)
+    } else {
+        pdl_wait();
+        if (live) {
+            if (g > 0) XL = ld_dep(Xup + g - 1);
+            XJ = ld_dep(Xup + g);
+        }
+        pdl_launch_dependents();
     }
-    pdl_launch_dependents();
     // RD with the support value of the joint above entering the first row (rp := 1 there, see the header)
     cplx A = cmake(1.0, 0.0), B = (lane == 0) ? XL : zero;
 #pragma unroll

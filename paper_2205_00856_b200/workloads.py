@@ -49,10 +49,10 @@ class Config:
 CONFIGS = {
     # PAPER-free constants come from BASELINE.json configs[0..4]
     "C1": Config("C1", 4096, 0.1, 0.01, "harmonic", "packet_noise", 64, 100, seed=20220501),
-    "C2": Config("C2", 1 << 24, 0.05, 0.005, "soft_coulomb", "gaussian_random_phase", 1 << 17, 1000,
+    "C2": Config("C2", 1 << 24, 0.05, 0.005, "soft_coulomb", "gaussian_random_phase", 1 << 16, 1000,
                  seed=20220502, x0=0.0, P_sweep=tuple(1 << k for k in range(8, 17))),
     # dense-support twin of C2: same envelope + C1-style noise so that far blocks are exercised
-    "C2dense": Config("C2dense", 1 << 24, 0.05, 0.005, "soft_coulomb", "gaussian_phase_noise", 1 << 17, 1000,
+    "C2dense": Config("C2dense", 1 << 24, 0.05, 0.005, "soft_coulomb", "gaussian_phase_noise", 1 << 16, 1000,
                       seed=20220502, x0=0.0, P_sweep=tuple(1 << k for k in range(8, 17))),
     "C3": Config("C3", 1 << 30, 0.01, 0.001, "random_gaussians", "packet_noise", 1 << 16, 50, seed=20220503),
     "C4": Config("C4", 8192, 0.05, 0.002, "harmonic", "packet_noise", 8, 20, seed=20220504, nsys=8192,

@@ -132,6 +132,14 @@ RS_CASES = [
     (8 * 1000, 1000, dict(rs_topmax=64, rs_fused=0)),
     (8 * 513, 513, dict(rs_topmax=2, rs_fused=0)),
     (1 << 17, 1 << 14, dict(rs_fused=0)),
+    # last level by its own kernel instead of inside the substitution kernel
+    (1 << 13, 1 << 10, dict(rs_topmax=64, rs_top_in_subst=0)),
+    (8 * 1000, 1000, dict(rs_topmax=64, rs_top_in_subst=0)),
+    (8 * 513, 513, dict(rs_topmax=2, rs_top_in_subst=0)),
+    (1 << 17, 1 << 14, dict(rs_top_in_subst=0)),
+    (8 * 98304, 98304, dict(rs_top_in_subst=0)),
+    (8 * 98304, 98304, dict(rs_top_in_subst=1024)),      # last level of 384 rows inside the substitution (KT = 4)
+    (1 << 21, 1 << 18, dict(rs_top_in_subst=1024)),      # 1024 rows (KT = 8)
     # paper-shaped nested levels: one thread per group of any size, serial last level
     (8 * 1000, 1000, dict(rs_group=10, rs_levels=3, rs_serial_top=1)),
     (1 << 13, 1 << 10, dict(rs_group=32, rs_levels=2)),
