@@ -121,3 +121,29 @@ def test_batched_argument_errors():
                 plan.batched_sweep(psi, *args, 1)
             assert ei.value.status == B.CN_EINVAL, args
         plan.batched_sweep(psi, 4, 1, 64, 0)
+
+
+@pytest.mark.parametrize("kind,N,nsys", [("x", 512, 6000), ("x", 8192, 600), ("y", 1024, 2048), ("y", 8192, 512)])
+def test_batched_refill_stress(kind, N, nsys):
+    """Many tiles per persistent CTA on L2-resident grids, repeated: the shapes on which a TMA refill can overtake
+    shared-memory loads that are still queued when the CTA barrier opens (hazard 1).  The first
+    64 systems against the oracle, all systems by norm conservation (the matrix is shared, CN is unitary)."""
+    torch = torch_()
+    V, sysm = rand_batch(N, nsys, 11)
+    dx, dt = 0.1, 0.02
+    ref = oracle_batch(dx, dt, V, sysm[:64], 2)
+    host = sysm if kind == "x" else np.ascontiguousarray(sysm.T)
+    n0 = np.sum(np.abs(sysm) ** 2, 1)
+    with B.Plan(N, 2, dx, dt, V) as plan:
+        plan.factorize()
+        for _ in range(15):
+            d = torch.from_numpy(host).cuda()
+            if kind == "x":
+                plan.batched_sweep(d, nsys, 1, N, 2)
+            else:
+                plan.batched_sweep(d, nsys, nsys, 1, 2)
+            torch.cuda.synchronize()
+            out = d.cpu().numpy()
+            out = out if kind == "x" else out.T
+            assert np.max(np.abs(out[:64] - ref)) <= TOL_PSI
+            assert np.max(np.abs(np.sum(np.abs(out) ** 2, 1) / n0 - 1.0)) <= 1e-11
