@@ -109,3 +109,19 @@ CN_DEVINL void warp_scan_affine(cplx &A, cplx &B, int lane)
         }
     }
 }
+
+// The same scan without the lane predicate.  Valid when A = 0 at the FIRST element of every chain in direction DIR
+// (a lane whose prefix already starts at its chain's first element then has A = 0, so combining it with whatever the
+// out-of-range or foreign lane holds leaves B unchanged): saves the compare and the selects of every step.
+template <int DIR, int STEPS>
+CN_DEVINL void warp_scan_affine_uncond(cplx &A, cplx &B)
+{
+#pragma unroll
+    for (int k = 0; k < STEPS; ++k) {
+        const int d = 1 << k;
+        cplx As = (DIR > 0) ? shfl_up_c(A, d) : shfl_down_c(A, d);
+        cplx Bs = (DIR > 0) ? shfl_up_c(B, d) : shfl_down_c(B, d);
+        B = cfma(A, Bs, B);
+        A = cmul(A, As);
+    }
+}

@@ -278,11 +278,21 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
                 cplx hi = (j == 7) ? vhi : v[j + 1];
                 E[j] = rhs_E(g[j], rho, v[j], lo, hi);
             }
-            cplx D = zero;
+            // a block inside one warp: the support value of the joint above enters the block's first chunk directly,
+            // so that A = 0 at every chain start and the scan needs no lane predicate (warp_scan_affine_uncond)
+            cplx D = (!XWARP && isFirst) ? jointAbove : zero;
 #pragma unroll
             for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
             if (isLast) D = supN; // the joint line carries its new support value
-            cplx in = scan_fwd(fwdA, D, jointAbove, 0, cn_false());
+            cplx in;
+            if (XWARP) {
+                in = scan_fwd(fwdA, D, jointAbove, 0, cn_false());
+            } else {
+                cplx A = isFirst ? zero : fwdA;
+                warp_scan_affine_uncond<+1, WSTEPS>(A, D);
+                in = shfl_up_c(D, 1);
+                if (isFirst) in = jointAbove;
+            }
             D = in;
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
@@ -294,7 +304,14 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
             if (isLast) X = supN;
 #pragma unroll
             for (int j = 6; j >= 0; --j) X = cmul(qv[j], csub(E[j], X));
-            cplx xin = scan_bwd(bwdA, X, 1);
+            cplx xin;
+            if (XWARP) {
+                xin = scan_bwd(bwdA, X, 1);
+            } else { // bwdA = 0 on a block's last chunk: every chain of this direction starts with A = 0
+                cplx A = bwdA, Bx = X;
+                warp_scan_affine_uncond<-1, WSTEPS>(A, Bx);
+                xin = shfl_down_c(Bx, 1); // ignored by a block's last chunk
+            }
             X = cmul(qv[7], csub(E[7], xin));
             if (isLast) X = supN;
             v[7] = X;
@@ -343,7 +360,15 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
 #pragma unroll
             for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
             if (isLast) D = zero;
-            cplx in = scan_fwd(fwdA, D, zero, 1, cn_true());
+            cplx in;
+            if (XWARP) {
+                in = scan_fwd(fwdA, D, zero, 1, cn_true());
+            } else {
+                cplx A = isFirst ? zero : fwdA;
+                warp_scan_affine_uncond<+1, WSTEPS>(A, D);
+                in = shfl_up_c(D, 1);
+                if (isFirst) in = zero;
+            }
             D = in;
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
@@ -356,7 +381,15 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
             const cplx yn = Y; // local solution next to the own joint (meaningful for a last chunk)
 #pragma unroll
             for (int j = 5; j >= 0; --j) Y = cmul(qv[j], csub(E[j], Y));
-            cplx yin = scan_bwd(bwdA, Y, 0);
+            cplx yin;
+            if (XWARP) {
+                yin = scan_bwd(bwdA, Y, 0);
+            } else {
+                cplx A = bwdA, By = Y;
+                warp_scan_affine_uncond<-1, WSTEPS>(A, By);
+                yin = shfl_down_c(By, 1);
+                if (isLast) yin = zero;
+            }
             if (active) {
                 if (isLast) {
                     prm.slotD[w] = csub(EJ, yn);
