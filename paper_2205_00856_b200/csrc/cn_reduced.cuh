@@ -247,7 +247,8 @@ k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
         B = (r0 + k < ng - 1) ? cfnma(lk[k], B, R[k]) : zero;
         A = cmul(cneg(lk[k]), A);
     }
-    warp_scan_affine<+1, 5>(A, B, lane);
+    if (lane == 0) A = zero; // nothing enters the group through the scan: no lane predicate needed
+    warp_scan_affine_uncond<+1, 5>(A, B);
     cplx in = shfl_up_c(B, 1);
     if (lane == 0) in = zero;
 #pragma unroll
@@ -263,7 +264,7 @@ k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
         B = cfnma(uk[k], B, R[k]);
         A = cmul(cneg(uk[k]), A);
     }
-    warp_scan_affine<-1, 5>(A, B, lane);
+    warp_scan_affine_uncond<-1, 5>(A, B); // u = 0 on the joint line and beyond: A = 0 at the chain start
     in = shfl_down_c(B, 1);
     if (lane == 31) in = zero;
     cplx yN = zero, y0 = zero; // y next to the own joint (row ng-2) and y of the first row
@@ -385,7 +386,8 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
         B = cfnma(lk[k], B, R[k]);
         A = cmul(cneg(lk[k]), A);
     }
-    warp_scan_affine<+1, 5>(A, B, lane);
+    if (lane == 0) A = zero; // nothing enters the group through the scan: no lane predicate needed
+    warp_scan_affine_uncond<+1, 5>(A, B);
     cplx in = shfl_up_c(B, 1);
     if (lane == 0) in = XL;
 #pragma unroll
@@ -401,7 +403,7 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
         B = (r0 + k == ng - 1) ? XJ : cfnma(uk[k], B, R[k]);
         A = cmul(cneg(uk[k]), A);
     }
-    warp_scan_affine<-1, 5>(A, B, lane);
+    warp_scan_affine_uncond<-1, 5>(A, B); // u = 0 on the joint line and beyond: A = 0 at the chain start
     in = shfl_down_c(B, 1);
     if (lane == 31) in = zero;
 #pragma unroll
