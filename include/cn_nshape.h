@@ -76,6 +76,9 @@ typedef enum {
     CN_OPT_RS_TOP_IN_SUBST = 12, /* 1 (default) = a last level of at most 256 rows is solved inside the substitution
                                kernel of the level below it, redundantly by every CTA (one launch less per step);
                                a value v > 1 sets the row limit to min(v, 1024); 0 = always by its own kernel */
+    CN_OPT_KEEP_P = 13,     /* 0 (default) = the tiled path partitions caller blocks of more than 256 rows again into
+                               blocks of 256 rows (cn_plan_info.P_effective; psi does not depend on the partition);
+                               1 = blocks of up to 4096 rows are kept as given (slower: a block then spans warps) */
     CN_OPT_RS_SERIAL_TOP = 11 /* 1 = the LAST level is solved serially by one thread (the beta n_bl term of Eq. 8)
                                whatever the number of nested levels; default 0 = one CTA in parallel */
 } cn_option;

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(PKG, "libcn_nshape.so")
 
 CN_OK, CN_EINVAL, CN_ENOMEM, CN_ECUDA, CN_ENOTFACTORIZED, CN_EBREAKDOWN = range(6)
 CN_OPT_PATH, CN_OPT_TILE_THREADS, CN_OPT_RS_TOPMAX, CN_OPT_USE_GRAPH, CN_OPT_RS_LEVELS, CN_OPT_PROFILE, CN_OPT_PDL, CN_OPT_ONCHIP, CN_OPT_RS_FUSED = 1, 2, 3, 4, 5, 6, 7, 8, 9
-CN_OPT_RS_GROUP, CN_OPT_RS_SERIAL_TOP, CN_OPT_RS_TOP_IN_SUBST = 10, 11, 12
+CN_OPT_RS_GROUP, CN_OPT_RS_SERIAL_TOP, CN_OPT_RS_TOP_IN_SUBST, CN_OPT_KEEP_P = 10, 11, 12, 13
 PATH_AUTO, PATH_GENERIC, PATH_TILED, PATH_ONCHIP = 0, 1, 2, 3
 
 EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", "cn_factorize", "cn_step",
@@ -235,7 +235,7 @@ class Plan:
             cn_plan_set_option(self.h, {"rs_topmax": CN_OPT_RS_TOPMAX, "use_graph": CN_OPT_USE_GRAPH,
                                         "rs_levels": CN_OPT_RS_LEVELS, "profile": CN_OPT_PROFILE,
                                         "pdl": CN_OPT_PDL, "onchip": CN_OPT_ONCHIP, "rs_fused": CN_OPT_RS_FUSED, "rs_group": CN_OPT_RS_GROUP,
-                                        "rs_serial_top": CN_OPT_RS_SERIAL_TOP, "rs_top_in_subst": CN_OPT_RS_TOP_IN_SUBST}[k], v)
+                                        "rs_serial_top": CN_OPT_RS_SERIAL_TOP, "rs_top_in_subst": CN_OPT_RS_TOP_IN_SUBST, "keep_p": CN_OPT_KEEP_P}[k], v)
 
     def factorize(self, stream=None):
         cn_factorize(self.h, stream)

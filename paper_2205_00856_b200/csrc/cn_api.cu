@@ -62,7 +62,7 @@ struct cn_plan {
     std::vector<rs_level> lv;
     // configuration
     int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
-    int opt_pdl = 1, opt_rs_fused = 0, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0, opt_rs_top_in_subst = 1;
+    int opt_pdl = 1, opt_rs_fused = 0, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0, opt_rs_top_in_subst = 1, opt_keep_p = 0;
     int64_t opt_rs_top_in_subst_max = 256; // measured at C2: faster up to 256 rows (160.8 vs 163.0 us), slower from 512 on
     // fused last-two-levels RS kernel (cn_reduced.cuh k_rs_fused): arrival counter + published epoch, launch number
     unsigned long long *rs_sync = nullptr, rs_epoch = 0;
@@ -282,6 +282,10 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
     case CN_OPT_RS_TOP_IN_SUBST:
         plan->opt_rs_top_in_subst = value ? 1 : 0;
         plan->opt_rs_top_in_subst_max = value > 1 ? (value > 1024 ? 1024 : value) : 256; // value > 1: the row limit
+        return CN_OK;
+    case CN_OPT_KEEP_P:
+        plan->opt_keep_p = value ? 1 : 0;
+        plan->factorized = false;
         return CN_OK;
     case CN_OPT_RS_FUSED:
         plan->opt_rs_fused = value ? 1 : 0;
@@ -563,13 +567,15 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     cudaStream_t stream = (cudaStream_t)stream_;
     free_factors(p);
     const int64_t N = p->N;
-    // A caller's block of more than 4096 rows does not fit one CTA tile.  The tiled path then partitions every such
-    // block again into sub-blocks of 256 rows -- the same method one level down; psi does not
-    // depend on the partition.  The generic path (CN_OPT_PATH = 1) always takes the caller's P literally.
+    // A caller's block of more than 4096 rows does not fit one CTA tile, and a block of 512..4096 rows spans several
+    // warps (shared-memory scans and CTA barriers: 189-235 us per C2 step against 158).  The tiled path therefore
+    // partitions every block of more than 256 rows again into sub-blocks of 256 rows -- the same method one level down
+    // (PAPER.md:128-149); psi does not depend on the partition.  CN_OPT_KEEP_P = 1 keeps blocks of up to 4096 rows as
+    // the caller gave them; the generic path (CN_OPT_PATH = 1) always takes the caller's P literally.
     p->P = p->Pu;
     if (p->opt_path != 1 && N % p->Pu == 0) {
         const int64_t mu = N / p->Pu;
-        if (mu > 4096 && (mu & (mu - 1)) == 0) p->P = N / 256;
+        if (mu > (p->opt_keep_p ? 4096 : 256) && (mu & (mu - 1)) == 0) p->P = N / 256;
     }
     const int64_t P = p->P;
 

@@ -173,7 +173,7 @@ def p_sweep(torch, peak, name="C2dense"):
     V, psi = _inputs(cfg)
     d = torch.from_numpy(psi).cuda()
     rows = []
-    arms = (("tiled", dict()), ("paper_shape", dict(path=B.PATH_GENERIC, rs_levels=-1)),
+    arms = (("tiled", dict(keep_p=1)), ("paper_shape", dict(path=B.PATH_GENERIC, rs_levels=-1)),
             ("generic_nested_rs", dict(path=B.PATH_GENERIC)))
     for arm, opts in arms:
         for Pk in cfg.P_sweep:

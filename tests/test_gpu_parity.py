@@ -75,18 +75,24 @@ TILED_SHAPES = [
 ]
 
 
+@pytest.mark.parametrize("keep_p", [1, 0])
 @pytest.mark.parametrize("N,P,tt", TILED_SHAPES)
-def test_tiled_path_random(N, P, tt):
-    # several tiles and a ragged last tile; every scan depth (block inside a warp, across warps)
+def test_tiled_path_random(N, P, tt, keep_p):
+    # several tiles and a ragged last tile; every scan depth (block inside a warp, across warps: keep_p = 1 keeps the
+    # caller's blocks of 512..4096 rows, keep_p = 0 partitions them again into blocks of 256 rows)
     V, psi = W.random_system(N, seed=23)
     dx, dt = 0.1, 0.02
     for nsteps in (1, 3):
         ref = O.step(dx, dt, V, psi, nsteps)
-        out, info = gpu_step(N, P, dx, dt, V, psi, nsteps, path=B.PATH_TILED, tile_threads=tt)
+        out, info = gpu_step(N, P, dx, dt, V, psi, nsteps, path=B.PATH_TILED, tile_threads=tt, keep_p=keep_p)
         assert info["path"] == B.PATH_TILED
+        if keep_p or N // P <= 256:
+            assert info["P_effective"] == P
+        else:
+            assert info["P_effective"] == N // 256
         err = np.max(np.abs(out - ref))
         assert err <= TOL_PSI, (N, P, tt, nsteps, err)
-    out1, _ = gpu_step(N, P, dx, dt, V, psi, 1, path=B.PATH_TILED, tile_threads=tt)
+    out1, _ = gpu_step(N, P, dx, dt, V, psi, 1, path=B.PATH_TILED, tile_threads=tt, keep_p=keep_p)
     assert residual(dx, dt, V, psi, out1) <= TOL_RES
 
 
