@@ -9,8 +9,9 @@ Metric (BASELINE.json): CN grid-point-steps per second in complex128 on config C
 One bench "step" = one `cn_step(plan, psi, nsteps = CN_PER_STEP)` call through the C-ABI, i.e. one pass of
 the whole hot path (RHS, RD, RU, JD/JU, RS, SS and psi write -- every row of SURVEY 8a) CN_PER_STEP times
 over the resident wave function; K = 10 such steps are the 1000 CN steps of the config.
-`value` has psi, V and the factors resident in HBM; `e2e` is the same call with psi in PINNED HOST memory,
-copied host->device before and device->host after every bench step inside the timed region.
+`value` has psi, V and the factors resident in HBM; `e2e` is the same call with every bench step's wave function
+taken from PINNED HOST memory (H2D) and its result returned there (D2H) inside the timed region; the steps are
+independent batches, so their copies overlap the neighbouring steps' compute (three streams, two device buffers).
 
 N > 1 (torchrun, one rank per GPU): the path does not shard in this build ("replicas only", DESIGN.md);
 every rank advances its own replica of the system, no data-path collective; value = sum over ranks.
@@ -208,14 +209,19 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
-    def timed_region(fn, steps):
-        """EXACTLY `steps` calls of fn between barrier+sync, CUDA events on the launching stream, max over ranks."""
+    def timed_region(fn, steps, begin=None, finish=None):
+        """EXACTLY `steps` calls of fn between barrier+sync, CUDA events on the launching stream, max over ranks.
+        begin / finish: fork side streams from / join them into the launching stream inside the timed region."""
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         w0 = time.time()
         e0.record(stream)
+        if begin:
+            begin()
         for _ in range(steps):
             fn()
+        if finish:
+            finish()
         e1.record(stream)
         barrier()
         w1 = time.time()
@@ -262,19 +268,51 @@ def main():
                 "algorithmic_bytes_per_launch": BYTES_PER_POINT_STEP * cfg.N, "peak_source": peak_src,
                 "whole_step_GBps": BYTES_PER_POINT_STEP * cfg.N * cn_per * args.steps / (ms * 1e-3) / 1e9}
 
-    # ---- e2e: psi lives in pinned host memory, H2D + cn_step + D2H inside the timed region ---------------
+    # ---- e2e: every bench step takes its wave function from PINNED HOST memory (H2D), advances it by cn_per CN steps
+    # through the public API and returns the result to pinned host memory (D2H), all inside the timed region.  The
+    # steps are independent batches, so the copies of neighbouring steps overlap the compute: two device buffers,
+    # copy-in / compute / copy-out on three streams chained by events (the API is asynchronous on the caller's stream).
     e2e = None
     if not args.no_e2e:
+        s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+        d_buf = [d_psi, torch.empty_like(d_psi)]
+        h_out = [torch.empty_like(psi_pin).pin_memory(), torch.empty_like(psi_pin).pin_memory()]
+        ev_in = [torch.cuda.Event() for _ in range(2)]
+        ev_cmp = [torch.cuda.Event() for _ in range(2)]
+        ev_out = [torch.cuda.Event() for _ in range(2)]
+        state = {"i": 0}
+
+        def e2e_begin():
+            s_in.wait_stream(stream)
+            s_out.wait_stream(stream)
+            for b in range(2):
+                ev_out[b].record(s_out)
+
         def e2e_step():
-            d_psi.copy_(psi_pin, non_blocking=True)
-            plan.step(d_psi, cn_per)
-            psi_pin.copy_(d_psi, non_blocking=True)
-        for _ in range(2):
-            e2e_step()
-        ms_e, _, _ = timed_region(e2e_step, args.steps)
+            b = state["i"] & 1
+            state["i"] += 1
+            s_in.wait_event(ev_out[b])            # the buffer's previous result has left the device
+            with torch.cuda.stream(s_in):
+                d_buf[b].copy_(psi_pin, non_blocking=True)
+                ev_in[b].record(s_in)
+            stream.wait_event(ev_in[b])
+            plan.step(d_buf[b], cn_per)
+            ev_cmp[b].record(stream)
+            s_out.wait_event(ev_cmp[b])
+            with torch.cuda.stream(s_out):
+                h_out[b].copy_(d_buf[b], non_blocking=True)
+                ev_out[b].record(s_out)
+
+        def e2e_finish():
+            stream.wait_stream(s_out)
+            stream.wait_stream(s_in)
+
+        timed_region(e2e_step, 2, e2e_begin, e2e_finish)  # warm-up
+        ms_e, _, _ = timed_region(e2e_step, args.steps, e2e_begin, e2e_finish)
         e2e = {"value": R.whole_job_throughput(cfg.N, cn_per * args.steps, ms_e, world), "unit": UNIT,
                "h2d_bytes_per_step": 16 * cfg.N, "d2h_bytes_per_step": 16 * cfg.N,
-               "ms_per_step": ms_e / args.steps}
+               "ms_per_step": ms_e / args.steps,
+               "pipeline": "independent batches; H2D | cn_step | D2H on three streams over two device buffers"}
 
     # ---- optional P sweep (config C2: P = 2^8..2^16 against the paper's optimal-P model) -----------------
     sweep = None
