@@ -235,7 +235,7 @@ __global__ void k_td_potential(int64_t N, const double *__restrict__ V0, const d
     if (i < N) V[i] = fma(f, g[i], V0[i]);
 }
 
-// The same for one streamed part of the system (out-of-core mode, cn_ooc.cuh): nb equal blocks of m rows whose
+// The same for one streamed part of the system (out-of-core mode, ooc_* in cn_api.cu): nb equal blocks of m rows whose
 // V / q / gamma live in part-local arrays; block wl of the part is block w0 + wl of the system.  red* may be
 // NULL (per-step recomputation of the factors: "neither the matrix nor the wavefunction ever need to be placed
 // entirely on a single process").

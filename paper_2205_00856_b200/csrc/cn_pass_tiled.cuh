@@ -28,7 +28,7 @@ struct cn_false { static constexpr bool value = false; };
 
 struct cn_tiled_params {
     int64_t nchunks; // chunks (8 points) in the array the tensor maps describe: N / 8, or one streamed part of it
-    int64_t chunk0;  // global index of its first chunk (0 unless psi is streamed part by part, cn_ooc.cuh)
+    int64_t chunk0;  // global index of its first chunk (0 unless psi is streamed part by part, ooc_* in cn_api.cu)
     int64_t P;
     double rho;
     const cplx *psi_raw; // prologue only: old psi for the tile's left halo (same array as tmPsi)
@@ -76,11 +76,6 @@ CN_DEVINL void tma_store_2d(const CUtensorMap *map, const void *src, int c0, int
     asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(map),
                  "r"(smem_u32(src)), "r"(c0), "r"(c1)
                  : "memory");
-}
-CN_DEVINL void tma_store_commit_wait()
-{
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 CN_DEVINL void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
