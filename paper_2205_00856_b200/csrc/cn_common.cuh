@@ -41,6 +41,16 @@ CN_DEVINL cplx crecip(cplx a)
     double d = 1.0 / (fma(xr, xr, xi * xi));
     return make_double2(xr * d * inv_m, -xi * d * inv_m);
 }
+// the same with ONE division when |a|^2 can neither overflow nor underflow (the factor kernels: ~10 reciprocals per thread)
+CN_DEVINL cplx crecip_fast(cplx a)
+{
+    const double m = fmax(fabs(a.x), fabs(a.y));
+    if (m > 1e-140 && m < 1e140) {
+        const double d = 1.0 / fma(a.x, a.x, a.y * a.y);
+        return make_double2(a.x * d, -a.y * d);
+    }
+    return crecip(a);
+}
 CN_DEVINL bool cfinite_nonzero(cplx a)
 {
     return isfinite(a.x) && isfinite(a.y) && (a.x != 0.0 || a.y != 0.0);

@@ -111,9 +111,12 @@ CN_DEVINL cn_mob mob_mul(cn_mob H, cn_mob L) // H * L : first L, then H
 }
 CN_DEVINL cn_mob mob_scale(cn_mob M)
 {
-    double s = fmax(fmax(fmax(fabs(M.a.x), fabs(M.a.y)), fmax(fabs(M.b.x), fabs(M.b.y))),
-                    fmax(fmax(fabs(M.c.x), fabs(M.c.y)), fmax(fabs(M.d.x), fabs(M.d.y))));
-    const double r = (s > 0.0 && isfinite(s)) ? 1.0 / s : 1.0;
+    // scale by the power of two that brings the largest component into [1, 2): exact, and no division
+    const double s = fmax(fmax(fmax(fabs(M.a.x), fabs(M.a.y)), fmax(fabs(M.b.x), fabs(M.b.y))),
+                          fmax(fmax(fabs(M.c.x), fabs(M.c.y)), fmax(fabs(M.d.x), fabs(M.d.y))));
+    const int e = (int)((__double_as_longlong(s) >> 52) & 0x7ff); // biased exponent
+    double r = 1.0;
+    if (e > 0 && e < 0x7ff && e < 2046 - 1) r = __longlong_as_double((long long)(2046 - e) << 52); // 2^(1023 - e)
     M.a = cmake(M.a.x * r, M.a.y * r);
     M.b = cmake(M.b.x * r, M.b.y * r);
     M.c = cmake(M.c.x * r, M.c.y * r);
@@ -179,7 +182,7 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
         if (pos >= dd) M = mob_scale(mob_mul(M, S));
     }
     cn_mob Pm = mob_shfl(M, lane == 0 ? 0 : lane - 1); // inclusive map of the chunk above: a constant inside a block
-    cplx qin = isFirst ? zero : cmul(Pm.b, crecip(Pm.d));
+    cplx qin = isFirst ? zero : cmul(Pm.b, crecip_fast(Pm.d));
     bool bad = false;
     cplx pp = one, qlast = zero; // product of (-q) over this chunk's rows except the block's last interior row
 #pragma unroll
@@ -187,7 +190,7 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
         if (j < nrow) {
             cplx p = cmake(-g[j] - qin.x, rho - qin.y);
             if (!cfinite_nonzero(p)) bad = true;
-            qin = crecip(p);
+            qin = crecip_fast(p);
             q[8 * c + j] = qin;
             if (!(isLast && j == 6)) pp = cmul(pp, cneg(qin));
             qlast = qin;
@@ -220,7 +223,7 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
         if (w > 0) redSupU[w - 1] = cneg(Zn1);
     }
     if (isFirst && w > 0) {
-        const cplx quf = cmul(U.b, crecip(U.d)); // with LOGC == 0 isFirst == isLast and U is already the constant map
+        const cplx quf = cmul(U.b, crecip_fast(U.d)); // with LOGC == 0 isFirst == isLast and U is already the constant map
         if (!cfinite_nonzero(U.d)) bad = true;
         redDiagU[w - 1] = cneg(quf);
     }

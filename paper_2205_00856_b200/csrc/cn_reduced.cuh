@@ -779,7 +779,7 @@ k_rs_factor_level_smem(int64_t n, const cplx *__restrict__ sub, const cplx *__re
             cplx li = cmul(sS[i], prp);
             cplx piv = cfnma(li, psup, sD[i]);
             if (!cfinite_nonzero(piv)) bad = true;
-            cplx r = crecip(piv);
+            cplx r = crecip_fast(piv);
             sS[i] = li;
             sD[i] = r;
             sU[i] = cmul(supi, r);
@@ -854,7 +854,7 @@ k_rs_factor_top_scan(int64_t n, const cplx *__restrict__ sub, const cplx *__rest
         if (lane >= dd) M = mob_scale(mob_mul(M, S));
     }
     cn_mob Pm = mob_shfl(M, lane == 0 ? 0 : lane - 1);
-    cplx rqprev = (lane == 0) ? zero : cmul(Pm.b, crecip(Pm.d));
+    cplx rqprev = (lane == 0) ? zero : cmul(Pm.b, crecip_fast(Pm.d));
     bool bad = false;
     supprev = sup0;
     for (int64_t i = i0; i < i1; ++i) {
@@ -862,7 +862,7 @@ k_rs_factor_top_scan(int64_t n, const cplx *__restrict__ sub, const cplx *__rest
         cplx lq = (i > 0) ? cmul(sub[i], rqprev) : zero;
         cplx piv = cfnma(lq, supprev, diag[i]);
         if (!cfinite_nonzero(piv)) bad = true;
-        cplx r = crecip(piv);
+        cplx r = crecip_fast(piv);
         lw[i] = lq;
         rq[i] = r;
         uw[i] = cmul(si, r);
