@@ -84,8 +84,9 @@ __global__ void k_factor_blocks(cn_geom g, double two_dx2, double rho, const dou
 // matrices of its 8 rows, a segmented Kogge-Stone scan over the lanes of the block composes them (a block's first
 // chunk is entered by q = 0, so its map is the CONSTANT b / d and everything downstream of it is constant too), and
 // each thread then recomputes its own 8 pivots serially from its true inflow.  The upward pivots (only Z_{1,1} is
-// needed) are the same scan in the other direction.  Matrices are rescaled by their largest component after every
-// product (a Moebius map does not change when its matrix is scaled), so |mu|^m never overflows.
+// needed) are the same scan in the other direction.  The matrix of a chunk is rescaled by a power of two (a Moebius
+// map does not change when its matrix is scaled), so |mu|^8 never overflows; the scan then multiplies at most 2^LOGC
+// matrices with components below 2, which needs no further rescaling.
 // Memory: a thread reads 64 contiguous bytes of V and writes 128 of q and 64 of gamma -- whole sectors, against one
 // 8-byte access per row and per thread in k_factor_blocks (619 us at C2, P = 2^17; this kernel: see DESIGN.md 8c).
 struct cn_mob {
@@ -179,7 +180,7 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
     for (int k = 0; k < LOGC; ++k) {
         const int dd = 1 << k;
         cn_mob S = mob_shfl(M, lane - dd < 0 ? 0 : lane - dd);
-        if (pos >= dd) M = mob_scale(mob_mul(M, S));
+        if (pos >= dd) M = mob_mul(M, S); // scaled chunk maps: <= 2 * 16^LOGC after the scan, no rescaling needed
     }
     cn_mob Pm = mob_shfl(M, lane == 0 ? 0 : lane - 1); // inclusive map of the chunk above: a constant inside a block
     cplx qin = isFirst ? zero : cmul(Pm.b, crecip_fast(Pm.d));
@@ -214,7 +215,7 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
     for (int k = 0; k < LOGC; ++k) {
         const int dd = 1 << k;
         cn_mob S = mob_shfl(U, lane + dd > 31 ? 31 : lane + dd);
-        if (pos + dd < CPB) U = mob_scale(mob_mul(U, S));
+        if (pos + dd < CPB) U = mob_mul(U, S);
     }
     if (isLast) {
         const cplx Zn1 = cmul(qlast, pp);
