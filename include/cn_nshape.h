@@ -69,7 +69,9 @@ typedef enum {
     CN_OPT_RS_FUSED = 9,    /* 1 = the last two RS levels (group reduction, last-level solve, group
                                substitution; Eq. 6) run as one kernel when the last level has at
                                most 1024 rows and the grid fits the device; 0 (default) = one kernel per stage, which is
-                               1-2 % faster at C2 under programmatic dependent launch */
+                               1-2 % faster at C2 under programmatic dependent launch.  The fused
+                               kernel's CTAs wait for one another: use it only when nothing else runs on the device
+                               concurrently (another stream's kernels could keep its last CTA from being scheduled) */
     CN_OPT_RS_GROUP = 10,   /* joint lines per group of a nested RS level (2..2^20, default 256): the fan-out
                                n_bl(i) / n_bl(i+1) of PAPER.md:239-247 Eq. 8; any value but 256 selects the
                                paper-shaped kernels in which one thread serves one group */
