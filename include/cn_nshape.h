@@ -75,14 +75,14 @@ typedef enum {
     CN_OPT_RS_GROUP = 10,   /* joint lines per group of a nested RS level (2..2^20, default 256): the fan-out
                                n_bl(i) / n_bl(i+1) of PAPER.md:239-247 Eq. 8; any value but 256 selects the
                                paper-shaped kernels in which one thread serves one group */
+    CN_OPT_RS_SERIAL_TOP = 11, /* 1 = the LAST level is solved serially by one thread (the beta n_bl term of Eq. 8)
+                               whatever the number of nested levels; default 0 = one CTA in parallel */
     CN_OPT_RS_TOP_IN_SUBST = 12, /* 1 (default) = a last level of at most 256 rows is solved inside the substitution
                                kernel of the level below it, redundantly by every CTA (one launch less per step);
                                a value v > 1 sets the row limit to min(v, 1024); 0 = always by its own kernel */
-    CN_OPT_KEEP_P = 13,     /* 0 (default) = the tiled path partitions caller blocks of more than 256 rows again into
+    CN_OPT_KEEP_P = 13      /* 0 (default) = the tiled path partitions caller blocks of more than 256 rows again into
                                blocks of 256 rows (cn_plan_info.P_effective; psi does not depend on the partition);
                                1 = blocks of up to 4096 rows are kept as given (slower: a block then spans warps) */
-    CN_OPT_RS_SERIAL_TOP = 11 /* 1 = the LAST level is solved serially by one thread (the beta n_bl term of Eq. 8)
-                               whatever the number of nested levels; default 0 = one CTA in parallel */
 } cn_option;
 
 typedef struct {
@@ -95,8 +95,8 @@ typedef struct {
     size_t device_bytes;     /* device memory owned by the plan */
     int64_t launches;        /* kernels launched by this plan so far (all entry points) */
     double bytes_per_point_step; /* algorithmic HBM bytes per point per fused step of the chosen path */
-    int64_t P_effective;     /* blocks the kernels work with: P, or N / 256 when a block of P exceeds one CTA tile
-                                (4096 rows) and the tiled path partitions it again */
+    int64_t P_effective;     /* blocks the kernels work with: P, or N / 256 when the tiled path partitions the caller's
+                                blocks again (blocks of more than 256 rows, CN_OPT_KEEP_P) */
 } cn_plan_info;
 
 /*
