@@ -281,3 +281,32 @@ def test_config_c2_full_size(name):
     assert abs(np.vdot(out, out).real * cfg.dx - 1.0) <= 1e-12
     out1, _ = gpu_step(cfg.N, cfg.P, cfg.dx, cfg.dt, V, psi, 1)
     assert residual(cfg.dx, cfg.dt, V, psi, out1) <= TOL_RES
+
+
+def test_config_c2_full_step_count():
+    """C2 at full size for the config's FULL step count (1000 steps, 10 calls of 100 as bench.py issues them): the
+    oracle needs ~5 minutes for that, so the check is by properties that hold at any size -- the norm (CN is unitary:
+    1e-12 per 1000 steps is the oracle's own pin), time reversal with a plan of -dt, and the oracle element by
+    element on the last 5 steps restarted from the GPU state after 995."""
+    torch = torch_()
+    cfg = W.CONFIGS["C2dense"]
+    V, psi = W.potential(cfg), W.psi0(cfg)
+    d = torch.from_numpy(psi).cuda()
+    with B.Plan(cfg.N, cfg.P, cfg.dx, cfg.dt, V) as plan:
+        plan.factorize()
+        for _ in range(9):
+            plan.step(d, 100)
+        plan.step(d, 95)
+        torch.cuda.synchronize()
+        mid = d.cpu().numpy()
+        plan.step(d, 5)
+        torch.cuda.synchronize()
+        out = d.cpu().numpy()
+    assert abs(np.vdot(out, out).real * cfg.dx - 1.0) <= 1e-11
+    assert np.max(np.abs(out - O.step(cfg.dx, cfg.dt, V, mid, 5))) <= TOL_PSI
+    with B.Plan(cfg.N, cfg.P, cfg.dx, -cfg.dt, V) as back:
+        back.factorize()
+        for _ in range(10):
+            back.step(d, 100)
+        torch.cuda.synchronize()
+    assert np.max(np.abs(d.cpu().numpy() - psi)) <= 1e-9   # 2000 steps of rounding, forward and back
