@@ -1064,7 +1064,6 @@ extern "C" cn_status cn_step_td(cn_plan *p, void *psi_, int64_t nsteps, const do
         p->tmPsiFor = psi_;
     }
     const int64_t m = (p->N % p->P == 0) ? p->N / p->P : 0;
-    const int T = 256;
     for (int64_t k = 0; k < nsteps; ++k) {
         if ((st = factor_compute(p, p->dV, p->tdRed, m, stream, false, p->tdG, field[k])) != CN_OK) return st;
         if ((st = launch_pass(p, psi, 0, /*cur=*/1, stream)) != CN_OK) return st;
