@@ -995,7 +995,10 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
         const int64_t chunks = (p->N + 7) / 8;
         const bool pdl = p->opt_pdl != 0;
         cudaError_t e;
-#define CN_ONCHIP(T) launch_k(k_onchip_steps<T>, 1u, (unsigned)T, 0, stream, pdl, p->N, nsteps, p->rho, psi, (const cplx *)p->qB, (const double *)p->gam)
+#define CN_ONCHIP(T)                                                                                                             \
+    (cudaFuncSetAttribute((const void *)k_onchip_steps<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)onchip_smem_bytes<T>()), \
+     launch_k(k_onchip_steps<T>, 1u, (unsigned)T, onchip_smem_bytes<T>(), stream, pdl, p->N, nsteps, p->rho, psi,                     \
+              (const cplx *)p->qB, (const double *)p->gam))
         if (chunks <= 32) e = CN_ONCHIP(32);
         else if (chunks <= 64) e = CN_ONCHIP(64);
         else if (chunks <= 128) e = CN_ONCHIP(128);
