@@ -52,10 +52,10 @@ typedef enum {
 typedef enum {
     CN_OPT_PATH = 1,        /* 0 = auto (default), 1 = force the generic thread-per-block kernels,
                                2 = force the tiled TMA kernels (CN_EINVAL at factorize if the shape does not fit) */
-    CN_OPT_TILE_THREADS = 2,/* threads per CTA of the tiled kernels: 0 = auto, else 64/128/256/512 (8 points per thread) */
+    CN_OPT_TILE_THREADS = 2,/* threads per CTA of the tiled kernels: 0 = auto, else 128/256/512 (8 points per thread) */
     CN_OPT_RS_TOPMAX = 3,   /* largest reduced system solved by the single-CTA RS kernel (1..8192, default 4096);
                                a larger one is partitioned again into groups of 256 joint lines (next RS level) */
-    CN_OPT_USE_GRAPH = 4,   /* reserved: accepted, no effect (small systems are stepped on chip, CN_OPT_ONCHIP) */
+                            /* 4: not used (CN_EINVAL) */
     CN_OPT_RS_LEVELS = 5,   /* 0 = auto (levels added while the system exceeds RS_TOPMAX), k >= 1 = exactly k nested
                                levels where possible (Eq. 6; CN_EINVAL at factorize if the last
                                level exceeds 8192 rows), -1 = paper-literal serial RS by one thread */
@@ -66,12 +66,7 @@ typedef enum {
     CN_OPT_ONCHIP = 8,      /* 1 (default) = a system of N <= 4096 points whose plan forces neither a path nor an RS
                                structure is stepped by ONE single-CTA launch per cn_step call that keeps psi in
                                registers and loops over the steps on chip (cn_plan_info.path = 3); 0 = never */
-    CN_OPT_RS_FUSED = 9,    /* 1 = the last two RS levels (group reduction, last-level solve, group
-                               substitution; Eq. 6) run as one kernel when the last level has at
-                               most 1024 rows and the grid fits the device; 0 (default) = one kernel per stage, which is
-                               1-2 % faster at C2 under programmatic dependent launch.  The fused
-                               kernel's CTAs wait for one another: use it only when nothing else runs on the device
-                               concurrently (another stream's kernels could keep its last CTA from being scheduled) */
+                            /* 9: not used (CN_EINVAL) */
     CN_OPT_RS_GROUP = 10,   /* joint lines per group of a nested RS level (2..2^20, default 256): the fan-out
                                n_bl(i) / n_bl(i+1) of PAPER.md:239-247 Eq. 8; any value but 256 selects the
                                paper-shaped kernels in which one thread serves one group */
@@ -80,9 +75,12 @@ typedef enum {
     CN_OPT_RS_TOP_IN_SUBST = 12, /* 1 (default) = a last level of at most 256 rows is solved inside the substitution
                                kernel of the level below it, redundantly by every CTA (one launch less per step);
                                a value v > 1 sets the row limit to min(v, 1024); 0 = always by its own kernel */
-    CN_OPT_KEEP_P = 13      /* 0 (default) = the tiled path partitions caller blocks of more than 256 rows again into
-                               blocks of 256 rows (cn_plan_info.P_effective; psi does not depend on the partition);
-                               1 = blocks of up to 4096 rows are kept as given (slower: a block then spans warps) */
+    CN_OPT_KEEP_P = 13      /* 0 (default) = unless the caller's blocks already have 8 * 2^k <= 256 rows, the tiled path
+                               partitions the system itself: blocks of the largest 8 * 2^k <= 256 rows that divides N
+                               (cn_plan_info.P_effective; psi does not depend on the partition);
+                               1 = the caller's P is the partition: equal blocks of 8 * 2^k <= 4096 rows run on the tiled
+                               kernels as given (slower above 256 rows: a block then spans warps), any other shape on
+                               the generic thread-per-block kernels */
 } cn_option;
 
 typedef struct {
@@ -95,14 +93,18 @@ typedef struct {
     size_t device_bytes;     /* device memory owned by the plan */
     int64_t launches;        /* kernels launched by this plan so far (all entry points) */
     double bytes_per_point_step; /* algorithmic HBM bytes per point per fused step of the chosen path */
-    int64_t P_effective;     /* blocks the kernels work with: P, or N / 256 when the tiled path partitions the caller's
-                                blocks again (blocks of more than 256 rows, CN_OPT_KEEP_P) */
+    int64_t P_effective;     /* blocks the kernels work with: P, or N / (8 * 2^k) when the tiled path chooses the
+                                partition itself (see cn_plan_create, CN_OPT_KEEP_P) */
 } cn_plan_info;
 
 /*
  * cn_plan_create -- describe one Hamiltonian / time step.
  *   out : HOST, receives the plan.            N : number of grid points (rows of T), N >= 2.
- *   P   : number of blocks n_bl, 1 <= P <= N.  Blocks need not be equal.
+ *   P   : number of blocks n_bl, 1 <= P <= N.  Blocks need not be equal.  P is the partition the
+ *         kernels use ONLY under CN_OPT_PATH = 1 (generic kernels) or CN_OPT_KEEP_P = 1; by default it is a hint:
+ *         psi does not depend on the partition (direct solver), so when N is a multiple of 8 the library runs the
+ *         tiled kernels on blocks of 8 * 2^k <= 256 rows of its own choosing (the caller's blocks if they already
+ *         have that shape) and reports the count as cn_plan_info.P_effective.
  *   dx, dt : grid spacing (> 0) and time step (!= 0, negative = backward propagation).
  *   V   : N real potential values, HOST or DEVICE pointer (detected); copied, caller keeps ownership.
  * Allocates nothing on the device yet except the copy of V.

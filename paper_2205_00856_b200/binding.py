@@ -14,7 +14,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(PKG, "libcn_nshape.so")
 
 CN_OK, CN_EINVAL, CN_ENOMEM, CN_ECUDA, CN_ENOTFACTORIZED, CN_EBREAKDOWN = range(6)
-CN_OPT_PATH, CN_OPT_TILE_THREADS, CN_OPT_RS_TOPMAX, CN_OPT_USE_GRAPH, CN_OPT_RS_LEVELS, CN_OPT_PROFILE, CN_OPT_PDL, CN_OPT_ONCHIP, CN_OPT_RS_FUSED = 1, 2, 3, 4, 5, 6, 7, 8, 9
+CN_OPT_PATH, CN_OPT_TILE_THREADS, CN_OPT_RS_TOPMAX, CN_OPT_RS_LEVELS, CN_OPT_PROFILE, CN_OPT_PDL, CN_OPT_ONCHIP = 1, 2, 3, 5, 6, 7, 8
 CN_OPT_RS_GROUP, CN_OPT_RS_SERIAL_TOP, CN_OPT_RS_TOP_IN_SUBST, CN_OPT_KEEP_P = 10, 11, 12, 13
 PATH_AUTO, PATH_GENERIC, PATH_TILED, PATH_ONCHIP = 0, 1, 2, 3
 
@@ -232,9 +232,9 @@ class Plan:
         if device_budget:
             cn_plan_set_device_budget(self.h, device_budget)
         for k, v in opts.items():
-            cn_plan_set_option(self.h, {"rs_topmax": CN_OPT_RS_TOPMAX, "use_graph": CN_OPT_USE_GRAPH,
+            cn_plan_set_option(self.h, {"rs_topmax": CN_OPT_RS_TOPMAX,
                                         "rs_levels": CN_OPT_RS_LEVELS, "profile": CN_OPT_PROFILE,
-                                        "pdl": CN_OPT_PDL, "onchip": CN_OPT_ONCHIP, "rs_fused": CN_OPT_RS_FUSED, "rs_group": CN_OPT_RS_GROUP,
+                                        "pdl": CN_OPT_PDL, "onchip": CN_OPT_ONCHIP, "rs_group": CN_OPT_RS_GROUP,
                                         "rs_serial_top": CN_OPT_RS_SERIAL_TOP, "rs_top_in_subst": CN_OPT_RS_TOP_IN_SUBST, "keep_p": CN_OPT_KEEP_P}[k], v)
 
     def factorize(self, stream=None):

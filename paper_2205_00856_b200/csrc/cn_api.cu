@@ -61,12 +61,9 @@ struct cn_plan {
     };
     std::vector<rs_level> lv;
     // configuration
-    int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_graph = 0, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
-    int opt_pdl = 1, opt_rs_fused = 0, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0, opt_rs_top_in_subst = 1, opt_keep_p = 0;
+    int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
+    int opt_pdl = 1, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0, opt_rs_top_in_subst = 1, opt_keep_p = 0;
     int64_t opt_rs_top_in_subst_max = 256; // measured at C2: faster up to 256 rows (160.8 vs 163.0 us), slower from 512 on
-    // fused last-two-levels RS kernel (cn_reduced.cuh k_rs_fused): arrival counter + published epoch, launch number
-    unsigned long long *rs_sync = nullptr, rs_epoch = 0;
-    bool rs_fused = false;
     // time-dependent H (cn_step_td): spatial shape g of the driving term, the potential of the current step and the
     // temporaries of the factorization kept alive so that cn_step_td never allocates
     double *tdG = nullptr, *tdV = nullptr;
@@ -134,7 +131,6 @@ static void free_factors(cn_plan *p)
     p->q = nullptr; p->gam = nullptr; p->lw = p->rq = p->uw = nullptr;
     p->slotD = p->slotU = nullptr; p->sup[0] = p->sup[1] = nullptr; p->work = nullptr; p->derr = nullptr;
     p->qB = nullptr;
-    p->rs_sync = nullptr; p->rs_epoch = 0; p->rs_fused = false;
     p->gamJ = nullptr;
     for (int b = 0; b < cn_plan::NB; ++b) { p->bPsi[b] = nullptr; p->bQ[b] = nullptr; p->bV[b] = nullptr; }
     p->factorized = false;
@@ -264,9 +260,6 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
     case CN_OPT_PDL:
         plan->opt_pdl = value ? 1 : 0;
         return CN_OK;
-    case CN_OPT_USE_GRAPH:
-        plan->opt_graph = value ? 1 : 0;
-        return CN_OK;
     case CN_OPT_ONCHIP:
         plan->opt_onchip = value ? 1 : 0;
         return CN_OK;
@@ -285,10 +278,6 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
         return CN_OK;
     case CN_OPT_KEEP_P:
         plan->opt_keep_p = value ? 1 : 0;
-        plan->factorized = false;
-        return CN_OK;
-    case CN_OPT_RS_FUSED:
-        plan->opt_rs_fused = value ? 1 : 0;
         plan->factorized = false;
         return CN_OK;
     case CN_OPT_RS_LEVELS:
@@ -434,6 +423,11 @@ static cn_status ooc_setup(cn_plan *p, int64_t m)
         if ((st = dev_alloc(p, &p->bPsi[b], (size_t)pts)) != CN_OK) return st;
         if ((st = dev_alloc(p, &p->bQ[b], (size_t)pts)) != CN_OK) return st;
         if ((st = dev_alloc(p, &p->bV[b], (size_t)pts)) != CN_OK) return st;
+        // a last part shorter than the buffers leaves the tail of its last tile untouched: the inactive lanes of that
+        // tile must read finite values (0 * garbage in the unpredicated scans would be NaN for Inf / NaN garbage)
+        CN_CUDA(p, cudaMemset(p->bPsi[b], 0, sizeof(cplx) * (size_t)pts));
+        CN_CUDA(p, cudaMemset(p->bQ[b], 0, sizeof(cplx) * (size_t)pts));
+        CN_CUDA(p, cudaMemset(p->bV[b], 0, sizeof(double) * (size_t)pts));
         if ((st = make_map(p, &p->tmPsiB[b], p->bPsi[b], 16, box_rows, pts / 8)) != CN_OK) return st;
         if ((st = make_map(p, &p->tmQB[b], p->bQ[b], 16, box_rows, pts / 8)) != CN_OK) return st;
         if ((st = make_map(p, &p->tmGamB[b], p->bV[b], 8, box_rows, pts / 8)) != CN_OK) return st;
@@ -471,8 +465,6 @@ static cn_status ooc_setup(cn_plan *p, int64_t m)
     p->grid_tiled = (int)(tiles < slots ? tiles : slots);
     return CN_OK;
 }
-
-static cn_status rs_fused_setup(cn_plan *p, cudaStream_t stream);
 
 // The arithmetic of the factorization: every matrix-side quantity of RD/RU/JD/JU from the potential
 // `Vsrc`, the reduced matrices of all RS levels and their factors.  Launches only (no allocation, no synchronisation):
@@ -560,6 +552,8 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
     return CN_OK;
 }
 
+static cn_status td_scratch(cn_plan *p);
+
 // ---- factorize ----------------------------------------------------------------------------------------
 extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
 {
@@ -567,15 +561,23 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     cudaStream_t stream = (cudaStream_t)stream_;
     free_factors(p);
     const int64_t N = p->N;
-    // A caller's block of more than 4096 rows does not fit one CTA tile, and a block of 512..4096 rows spans several
-    // warps (shared-memory scans and CTA barriers: 189-235 us per C2 step against 158).  The tiled path therefore
-    // partitions every block of more than 256 rows again into sub-blocks of 256 rows -- the same method one level down
-    // (PAPER.md:128-149); psi does not depend on the partition.  CN_OPT_KEEP_P = 1 keeps blocks of up to 4096 rows as
-    // the caller gave them; the generic path (CN_OPT_PATH = 1) always takes the caller's P literally.
+    // The partition the kernels work with.  psi does not depend on it (direct solver), and the tiled kernels want equal
+    // blocks of 8 * 2^k rows: up to 256 rows a block lives inside one warp (shuffle scans only), 512..4096 rows span
+    // several warps (shared-memory scans and CTA barriers: 189-235 us per C2 step against 158), more does not fit a
+    // CTA tile, and any other shape (N % P != 0, m = 300, m = 768 ...) would fall to the generic thread-per-block
+    // kernels (10-500 times slower at C2).  So unless the caller's blocks already have 8 * 2^k <= 256 rows, the auto
+    // and the forced-tiled paths partition the system themselves into blocks of the largest 8 * 2^k <= 256 rows that
+    // divides N -- the same method one level down.  CN_OPT_KEEP_P = 1 and the generic path
+    // (CN_OPT_PATH = 1) take the caller's P literally.
     p->P = p->Pu;
-    if (p->opt_path != 1 && N % p->Pu == 0) {
-        const int64_t mu = N / p->Pu;
-        if (mu > (p->opt_keep_p ? 4096 : 256) && (mu & (mu - 1)) == 0) p->P = N / 256;
+    if (p->opt_path != 1 && !p->opt_keep_p && N % 8 == 0) {
+        const int64_t mu = (N % p->Pu == 0) ? N / p->Pu : 0;
+        const bool fits = mu >= 8 && mu <= 256 && (mu & (mu - 1)) == 0;
+        if (!fits) {
+            int64_t me = 8;
+            while (me < 256 && N % (2 * me) == 0) me *= 2;
+            p->P = N / me;
+        }
     }
     const int64_t P = p->P;
 
@@ -698,9 +700,15 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
         CN_CUDA(p, cudaGetDevice(&dev));
         CN_CUDA(p, cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, dev));
     }
-    if ((st = rs_fused_setup(p, stream)) != CN_OK) return st;
+    if (p->qB && N <= CN_ONCHIP_NMAX) { // the on-chip stepper's dynamic shared memory, once per plan (not per cn_step)
+        CN_CUDA(p, cudaFuncSetAttribute((const void *)k_onchip_steps<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)onchip_smem_bytes<32>()));
+        CN_CUDA(p, cudaFuncSetAttribute((const void *)k_onchip_steps<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)onchip_smem_bytes<64>()));
+        CN_CUDA(p, cudaFuncSetAttribute((const void *)k_onchip_steps<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)onchip_smem_bytes<128>()));
+        CN_CUDA(p, cudaFuncSetAttribute((const void *)k_onchip_steps<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)onchip_smem_bytes<256>()));
+        CN_CUDA(p, cudaFuncSetAttribute((const void *)k_onchip_steps<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)onchip_smem_bytes<512>()));
+    }
     p->factorized = true;
-    return CN_OK;
+    return td_scratch(p);
 }
 
 // ---- profiling aid ---------------------------------------------------------------------------------------
@@ -802,38 +810,6 @@ static cudaError_t launch_top_k(cn_plan *p, const cn_plan::rs_level &L, cplx *X,
                     (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw, X);
 }
 
-typedef void (*rs_fused_t)(int64_t, const cplx *, const cplx *, const cplx *, const cplx *, const cplx *, const cplx *,
-                           const cplx *, cplx *, cplx *, int64_t, const cplx *, const cplx *, const cplx *, cplx *, cplx *,
-                           unsigned long long *, unsigned long long);
-static rs_fused_t rs_fused_kernel(int64_t ntop)
-{
-    const int64_t T = 32 * CN_RS_WARPS;
-    if (ntop <= T) return k_rs_fused<1>;
-    if (ntop <= 2 * T) return k_rs_fused<2>;
-    if (ntop <= 4 * T) return k_rs_fused<4>;
-    return k_rs_fused<8>;
-}
-
-// the last two RS levels run as ONE kernel when the last level is small and every CTA of the group level can be
-// resident at once (its CTAs wait for the one that solves the last level)
-static cn_status rs_fused_setup(cn_plan *p, cudaStream_t stream)
-{
-    p->rs_fused = false;
-    const int nlv = (int)p->lv.size();
-    if (!p->opt_rs_fused || p->opt_rs_levels < 0 || p->opt_rs_serial_top || p->opt_rs_group != CN_RS_G || nlv < 2 || p->lv.back().n > CN_RS_FUSED_TOPMAX) return CN_OK;
-    int per_sm = 0;
-    CN_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)rs_fused_kernel(p->lv.back().n),
-                                                             32 * CN_RS_WARPS, 0));
-    const int64_t grid = (p->lv[nlv - 1].n + CN_RS_WARPS - 1) / CN_RS_WARPS;
-    if (per_sm < 1 || grid > (int64_t)per_sm * p->sms) return CN_OK;
-    cn_status st;
-    if ((st = dev_alloc(p, &p->rs_sync, 2)) != CN_OK) return st;
-    CN_CUDA(p, cudaMemsetAsync(p->rs_sync, 0, 2 * sizeof(unsigned long long), stream));
-    p->rs_epoch = 0;
-    p->rs_fused = true;
-    return CN_OK;
-}
-
 // RS of one step: (RD+RU+JD+JU) level by level, RS of the last level, SS level by level (Eq. 6)
 static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
 {
@@ -842,10 +818,10 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
     const int pi = prof_begin(p, 1, stream);
     cudaError_t e = cudaSuccess;
     p->lv[0].X = p->sup[out];
-    const int nsep = p->rs_fused ? nlv - 2 : nlv - 1; // group levels that run as separate reduce / subst kernels
+    const int nsep = nlv - 1; // group levels: one reduce and one substitute kernel each
     const bool tg = p->opt_rs_group != CN_RS_G; // one thread per group of any size (paper-shaped, cn_reduced.cuh)
     // the last level is solved inside the substitution kernel of the level below it (one launch less per step)
-    const bool tis = !tg && !p->rs_fused && p->opt_rs_top_in_subst && p->opt_rs_levels >= 0 && !p->opt_rs_serial_top &&
+    const bool tis = !tg && p->opt_rs_top_in_subst && p->opt_rs_levels >= 0 && !p->opt_rs_serial_top &&
                      nlv >= 2 && p->lv.back().n <= p->opt_rs_top_in_subst_max;
     const int64_t G = p->opt_rs_group;
     for (int i = 0; i < nsep && e == cudaSuccess; ++i) {
@@ -860,15 +836,7 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
                      (const cplx *)L.sup, U.rD, U.rU);
         p->launches += 1;
     }
-    if (e == cudaSuccess && p->rs_fused) {
-        const cn_plan::rs_level &L = p->lv[nlv - 2], &U = p->lv[nlv - 1];
-        p->rs_epoch += 1;
-        e = launch_k(rs_fused_kernel(U.n), (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl,
-                     L.n, (const cplx *)L.rD, (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u,
-                     (const cplx *)L.sub, (const cplx *)L.sup, U.rD, U.rU, U.n, (const cplx *)p->lw, (const cplx *)p->rq,
-                     (const cplx *)p->uw, U.X, L.X, p->rs_sync, p->rs_epoch);
-        p->launches += 1;
-    } else if (e == cudaSuccess && !tis) {
+    if (e == cudaSuccess && !tis) {
         const cn_plan::rs_level &L = p->lv.back();
         if (p->opt_rs_levels < 0 || p->opt_rs_serial_top)
             e = launch_k(k_rs_serial, 1u, 32u, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU,
@@ -995,10 +963,9 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
         const int64_t chunks = (p->N + 7) / 8;
         const bool pdl = p->opt_pdl != 0;
         cudaError_t e;
-#define CN_ONCHIP(T)                                                                                                             \
-    (cudaFuncSetAttribute((const void *)k_onchip_steps<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)onchip_smem_bytes<T>()), \
-     launch_k(k_onchip_steps<T>, 1u, (unsigned)T, onchip_smem_bytes<T>(), stream, pdl, p->N, nsteps, p->rho, psi,                     \
-              (const cplx *)p->qB, (const double *)p->gam))
+#define CN_ONCHIP(T)                                                                                              \
+    launch_k(k_onchip_steps<T>, 1u, (unsigned)T, onchip_smem_bytes<T>(), stream, pdl, p->N, nsteps, p->rho, psi, \
+             (const cplx *)p->qB, (const double *)p->gam)
         if (chunks <= 32) e = CN_ONCHIP(32);
         else if (chunks <= 64) e = CN_ONCHIP(64);
         else if (chunks <= 128) e = CN_ONCHIP(128);
@@ -1032,6 +999,19 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
 // no allocation, no synchronisation -- and a step is prologue (RHS + RD/RU/JD/JU) -> RS -> epilogue (SS) with the
 // factors of that step.  SS(k) cannot be fused with RD/RU(k+1) here: the two use different matrices.
 
+// scratch of the per-step factorization of cn_step_td, sized for the partition in use; called by whichever of
+// cn_plan_set_td_shape / cn_factorize comes second, so that cn_step_td itself never allocates
+static cn_status td_scratch(cn_plan *p)
+{
+    if (!p->tdG || !p->factorized || (p->tdRed && p->tdRedP == p->P)) return CN_OK;
+    if (p->tdRed) cudaFree(p->tdRed);
+    p->tdRed = nullptr;
+    p->tdRedP = 0;
+    CN_CUDA(p, cudaMalloc((void **)&p->tdRed, sizeof(cplx) * 6 * (size_t)p->P));
+    p->tdRedP = p->P;
+    return CN_OK;
+}
+
 extern "C" cn_status cn_plan_set_td_shape(cn_plan *p, const double *g)
 {
     if (!p || !g) return CN_EINVAL;
@@ -1042,7 +1022,7 @@ extern "C" cn_status cn_plan_set_td_shape(cn_plan *p, const double *g)
         CN_CUDA(p, cudaMalloc((void **)&p->tdV, vb));
     }
     CN_CUDA(p, cudaMemcpy(p->tdG, g, vb, cudaMemcpyDefault));
-    return CN_OK;
+    return td_scratch(p);
 }
 
 extern "C" cn_status cn_step_td(cn_plan *p, void *psi_, int64_t nsteps, const double *field, void *stream_)
@@ -1052,32 +1032,37 @@ extern "C" cn_status cn_step_td(cn_plan *p, void *psi_, int64_t nsteps, const do
     if (!p->factorized) return CN_ENOTFACTORIZED;
     if (p->ooc || !p->tdG) return CN_EINVAL;
     if (nsteps == 0) return CN_OK;
+    for (int64_t k = 0; k < nsteps; ++k)
+        if (!std::isfinite(field[k])) return CN_EINVAL; // nothing has been enqueued yet
     cudaStream_t stream = (cudaStream_t)stream_;
     cplx *psi = (cplx *)psi_;
     cn_status st;
-    if (p->tdRedP != p->P) { // scratch of the factorization, sized for this partition (first call only)
-        if (p->tdRed) cudaFree(p->tdRed);
-        p->tdRed = nullptr;
-        CN_CUDA(p, cudaMalloc((void **)&p->tdRed, sizeof(cplx) * 6 * (size_t)p->P));
-        p->tdRedP = p->P;
-    }
+    if (!p->tdRed || p->tdRedP != p->P) return CN_EINVAL; // td_scratch() ran at set_td_shape / factorize: cannot happen
     if (p->path == 2 && p->tmPsiFor != psi_) {
         const int box_rows = p->tpb < 256 ? p->tpb : 256;
         if ((st = make_map(p, &p->tmPsi, psi_, 16, box_rows)) != CN_OK) return st;
         p->tmPsiFor = psi_;
     }
     const int64_t m = (p->N % p->P == 0) ? p->N / p->P : 0;
-    for (int64_t k = 0; k < nsteps; ++k) {
-        if ((st = factor_compute(p, p->dV, p->tdRed, m, stream, false, p->tdG, field[k])) != CN_OK) return st;
-        if ((st = launch_pass(p, psi, 0, /*cur=*/1, stream)) != CN_OK) return st;
-        if ((st = launch_rs(p, 1, stream)) != CN_OK) return st;
-        if ((st = launch_pass(p, psi, 2, /*cur=*/1, stream)) != CN_OK) return st;
-    }
-    // leave the plan with the factors of the static H again, so that cn_step keeps its meaning
-    if ((st = factor_compute(p, p->dV, p->tdRed, m, stream, false)) != CN_OK) return st;
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(p, e);
-    return CN_OK;
+    // a launch that fails mid-loop leaves the plan with the factors of that step: the plan is then marked
+    // unfactorized, so that a later cn_step cannot silently use the wrong matrix
+    auto run = [&]() -> cn_status {
+        cn_status s;
+        for (int64_t k = 0; k < nsteps; ++k) {
+            if ((s = factor_compute(p, p->dV, p->tdRed, m, stream, false, p->tdG, field[k])) != CN_OK) return s;
+            if ((s = launch_pass(p, psi, 0, /*cur=*/1, stream)) != CN_OK) return s;
+            if ((s = launch_rs(p, 1, stream)) != CN_OK) return s;
+            if ((s = launch_pass(p, psi, 2, /*cur=*/1, stream)) != CN_OK) return s;
+        }
+        // leave the plan with the factors of the static H again, so that cn_step keeps its meaning
+        if ((s = factor_compute(p, p->dV, p->tdRed, m, stream, false)) != CN_OK) return s;
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(p, e);
+        return CN_OK;
+    };
+    st = run();
+    if (st != CN_OK) p->factorized = false;
+    return st;
 }
 
 // ---- general complex tridiagonal front end (Eq. 5) ---------------------------------------

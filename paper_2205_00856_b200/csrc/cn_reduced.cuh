@@ -414,199 +414,6 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
     rs_store_rows(X + g0, ng, sbuf, lane, R);
 }
 
-// ---- (RD+RU+JD+JU)[M_i] + RS[M_last] + SS[M_i] of the last two levels in ONE launch -----------------------------
-// Eq. 6 for the level below the last one, without the two kernel boundaries: every warp reduces
-// its group and keeps the group's factors and right-hand sides in registers; the CTA that arrives LAST (a
-// monotonic arrival counter, no reset: launch number `epoch` ends at epoch * gridDim.x) solves the last level
-// (ntop <= 128 KT rows, KT rows per thread) and publishes `epoch` in sync[1]; the other CTAs spin on it and then
-// substitute.  All CTAs are co-resident by construction (the host launches this kernel only when the grid fits the
-// device, cn_api.cu), so the spin cannot deadlock.
-#define CN_RS_FUSED_TOPMAX (32 * CN_RS_WARPS * 8)
-
-CN_DEVINL unsigned long long ld_volatile_u64(const unsigned long long *p)
-{
-    unsigned long long v;
-    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
-}
-
-template <int KT>
-__global__ void __launch_bounds__(32 * CN_RS_WARPS)
-k_rs_fused(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
-           const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ sub,
-           const cplx *__restrict__ sup, cplx *outD, cplx *outU, int64_t ntop, const cplx *__restrict__ lw,
-           const cplx *__restrict__ rq, const cplx *__restrict__ uw, cplx *Xup, cplx *__restrict__ X,
-           unsigned long long *sync, unsigned long long epoch)
-{
-    constexpr int K = CN_RS_K;
-    __shared__ cplx sA[2][32], sB[2][32];
-    __shared__ int sLast;
-    const int lane = threadIdx.x & 31;
-    const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
-    const int64_t g = (int64_t)blockIdx.x * CN_RS_WARPS + (threadIdx.x >> 5);
-    const bool live = g < ngroups;
-    const int64_t g0 = g * CN_RS_G;
-    const int ng = live ? (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G) : 0;
-    const int r0 = lane * K;
-    const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
-    cplx lk[K], rpk[K], uk[K], R[K];
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-        const bool interior = r0 + k < ng - 1;
-        lk[k] = interior ? l[g0 + r0 + k] : zero;
-        rpk[k] = interior ? rp[g0 + r0 + k] : zero;
-        uk[k] = interior ? u[g0 + r0 + k] : zero;
-    }
-    cplx subJ = zero, supAbove = zero;
-    if (live && lane == 0) {
-        subJ = sub[g0 + ng - 1];
-        if (g > 0) supAbove = sup[g0 - 1];
-    }
-    pdl_wait();
-#pragma unroll
-    for (int k = 0; k < K; ++k) R[k] = (r0 + k < ng) ? cadd(ld_dep(rD + g0 + r0 + k), ld_dep(rU + g0 + r0 + k)) : zero;
-    pdl_launch_dependents();
-
-    // ---- phase 1: reduce the group (as k_rs_reduce; R stays intact for phase 3) ---------------------------
-    {
-        cplx Rj = zero;
-#pragma unroll
-        for (int k = 0; k < K; ++k)
-            if (r0 + k == ng - 1) Rj = R[k];
-        Rj = shfl_c(Rj, ng > 0 ? (ng - 1) / K : 0);
-        cplx T[K];
-        cplx A = one, B = zero;
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-            B = (r0 + k < ng - 1) ? cfnma(lk[k], B, R[k]) : zero;
-            A = cmul(cneg(lk[k]), A);
-        }
-        warp_scan_affine<+1, 5>(A, B, lane);
-        cplx in = shfl_up_c(B, 1);
-        if (lane == 0) in = zero;
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-            in = (r0 + k < ng - 1) ? cfnma(lk[k], in, R[k]) : zero;
-            T[k] = cmul(rpk[k], in);
-        }
-        A = one;
-        B = zero;
-#pragma unroll
-        for (int k = K - 1; k >= 0; --k) {
-            B = cfnma(uk[k], B, T[k]);
-            A = cmul(cneg(uk[k]), A);
-        }
-        warp_scan_affine<-1, 5>(A, B, lane);
-        in = shfl_down_c(B, 1);
-        if (lane == 31) in = zero;
-        cplx yN = zero, y0 = zero;
-#pragma unroll
-        for (int k = K - 1; k >= 0; --k) {
-            in = cfnma(uk[k], in, T[k]);
-            if (r0 + k == ng - 2) yN = in;
-            if (k == 0) y0 = in;
-        }
-        yN = shfl_c(yN, ng > 1 ? (ng - 2) / K : 0);
-        if (live && lane == 0) {
-            outD[g] = (ng >= 2) ? cfnma(subJ, yN, Rj) : Rj;
-            if (g > 0) outU[g - 1] = (ng >= 2) ? cneg(cmul(supAbove, y0)) : zero;
-        }
-    }
-    // ---- arrival; the last CTA solves the last level -------------------------------------------------------
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const unsigned long long old = atomicAdd(sync, 1ULL);
-        sLast = (old + 1 == epoch * (unsigned long long)gridDim.x) ? 1 : 0;
-    }
-    __syncthreads();
-    if (sLast) {
-        __threadfence();
-        const int t = threadIdx.x;
-        const int64_t w0 = (int64_t)t * KT;
-        cplx tl[KT], tr[KT], tu[KT], tR[KT];
-#pragma unroll
-        for (int k = 0; k < KT; ++k) {
-            const bool in = w0 + k < ntop;
-            tl[k] = in ? lw[w0 + k] : zero;
-            tr[k] = in ? rq[w0 + k] : zero;
-            tu[k] = in ? uw[w0 + k] : zero;
-            tR[k] = in ? cadd(ld_dep(outD + w0 + k), ld_dep(outU + w0 + k)) : zero;
-        }
-        cplx A = one, B = zero;
-#pragma unroll
-        for (int k = 0; k < KT; ++k) {
-            B = cfnma(tl[k], B, tR[k]);
-            A = cmul(cneg(tl[k]), A);
-        }
-        cplx in = cta_scan_excl<+1>(A, B, zero, sA[0], sB[0]);
-#pragma unroll
-        for (int k = 0; k < KT; ++k) {
-            in = cfnma(tl[k], in, tR[k]);
-            tR[k] = cmul(tr[k], in);
-        }
-        A = one;
-        B = zero;
-#pragma unroll
-        for (int k = KT - 1; k >= 0; --k) {
-            B = cfnma(tu[k], B, tR[k]);
-            A = cmul(cneg(tu[k]), A);
-        }
-        in = cta_scan_excl<-1>(A, B, zero, sA[1], sB[1]);
-#pragma unroll
-        for (int k = KT - 1; k >= 0; --k) {
-            in = cfnma(tu[k], in, tR[k]);
-            if (w0 + k < ntop) Xup[w0 + k] = in;
-        }
-        __threadfence();
-        __syncthreads();
-        if (threadIdx.x == 0) atomicExch(sync + 1, epoch);
-    } else {
-        if (threadIdx.x == 0)
-            while (ld_volatile_u64(sync + 1) < epoch) {}
-        __syncthreads();
-        __threadfence();
-    }
-    // ---- phase 3: substitute (as k_rs_subst) -----------------------------------------------------------------
-    cplx XL = zero, XJ = zero;
-    if (live) {
-        if (g > 0) XL = ld_dep(Xup + g - 1);
-        XJ = ld_dep(Xup + g);
-    }
-#pragma unroll
-    for (int k = 0; k < K; ++k)
-        if (!(r0 + k < ng - 1)) R[k] = zero; // the joint line's right-hand side is not part of the substitution
-    cplx A = one, B = (lane == 0) ? XL : zero;
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-        B = cfnma(lk[k], B, R[k]);
-        A = cmul(cneg(lk[k]), A);
-    }
-    warp_scan_affine<+1, 5>(A, B, lane);
-    cplx in = shfl_up_c(B, 1);
-    if (lane == 0) in = XL;
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-        in = cfnma(lk[k], in, R[k]);
-        R[k] = cmul(rpk[k], in);
-    }
-    A = one;
-    B = zero;
-#pragma unroll
-    for (int k = K - 1; k >= 0; --k) {
-        B = (r0 + k == ng - 1) ? XJ : cfnma(uk[k], B, R[k]);
-        A = cmul(cneg(uk[k]), A);
-    }
-    warp_scan_affine<-1, 5>(A, B, lane);
-    in = shfl_down_c(B, 1);
-    if (lane == 31) in = zero;
-#pragma unroll
-    for (int k = K - 1; k >= 0; --k) {
-        in = (r0 + k == ng - 1) ? XJ : cfnma(uk[k], in, R[k]);
-        if (r0 + k < ng) X[g0 + r0 + k] = in;
-    }
-}
-
 // ---- paper-shaped group kernels: ONE THREAD serves one group of G joint lines (any G) ------------------------
 // The multi-iteration GPU program of PAPER.md:276 ("interleaving" the block kernels for the nested method): the same
 // stages as k_rs_reduce / k_rs_subst by serial sweeps straight in global memory.  X of the level is the scratch for

@@ -96,6 +96,35 @@ def test_tiled_path_random(N, P, tt, keep_p):
     assert residual(dx, dt, V, psi, out1) <= TOL_RES
 
 
+AUTO_PARTITION_CASES = [
+    # (N, P, expected block size): by default P is a hint, the tiled kernels run on blocks of the largest 8 * 2^k <= 256
+    # rows that divides N unless the caller's blocks already have such a shape (m = 300, m = 768, N % P != 0
+    # used to fall to the thread-per-block kernels)
+    (3 << 15, 128, 256),       # m = 768
+    (300000, 1000, 32),        # m = 300; 300000 = 2^5 * 9375
+    (300000, 7, 32),           # N % P != 0
+    (8 * 4097, 4097 * 2, 8),   # m = 4 -> blocks of 8 rows (N / 8 odd)
+    (1 << 16, 1 << 10, 64),    # the caller's blocks of 64 rows are kept
+    (1 << 16, 3, 256),
+]
+
+
+@pytest.mark.parametrize("N,P,m_eff", AUTO_PARTITION_CASES)
+def test_auto_partition(N, P, m_eff):
+    cfg = W.scaled(W.CONFIGS["C2dense"], N=N)
+    V, psi = W.potential(cfg), W.psi0(cfg)
+    dx, dt = 0.01, 0.005
+    ref = O.step(dx, dt, V, psi, 3)
+    out, info = gpu_step(N, P, dx, dt, V, psi, 3, onchip=0)
+    assert info["path"] == B.PATH_TILED and info["P"] == P and info["P_effective"] == N // m_eff, info
+    err = np.max(np.abs(out - ref))
+    assert err <= TOL_PSI, (N, P, err)
+    # the caller's partition taken literally (generic kernels unless the shape fits the tiled ones) gives the same psi
+    out2, info2 = gpu_step(N, P, dx, dt, V, psi, 3, onchip=0, keep_p=1)
+    assert info2["P_effective"] == P
+    assert np.max(np.abs(out2 - ref)) <= TOL_PSI
+
+
 ONCHIP_SHAPES = [2, 3, 8, 9, 64, 100, 255, 256, 257, 777, 1000, 2048, 4095, 4096]
 
 
@@ -133,11 +162,6 @@ RS_CASES = [
     (1 << 13, 1 << 10, dict(rs_levels=-1)),             # paper-literal serial RS
     (1 << 13, 1 << 10, dict(pdl=0)),
     (5000, 700, dict(rs_topmax=16)),                    # generic path + nested RS
-    # the same structures with one kernel per RS stage instead of the fused last-two-levels kernel
-    (1 << 13, 1 << 10, dict(rs_topmax=64, rs_fused=0)),
-    (8 * 1000, 1000, dict(rs_topmax=64, rs_fused=0)),
-    (8 * 513, 513, dict(rs_topmax=2, rs_fused=0)),
-    (1 << 17, 1 << 14, dict(rs_fused=0)),
     # last level by its own kernel instead of inside the substitution kernel
     (1 << 13, 1 << 10, dict(rs_topmax=64, rs_top_in_subst=0)),
     (8 * 1000, 1000, dict(rs_topmax=64, rs_top_in_subst=0)),
@@ -152,13 +176,6 @@ RS_CASES = [
     (5000, 700, dict(rs_group=7, rs_levels=3, rs_serial_top=1)),
     (300000, 4489, dict(rs_group=67, rs_levels=2, rs_serial_top=1)),
     (300000, 12167, dict(rs_group=23, rs_levels=3, rs_serial_top=1)),
-    # fused kernel with 2, 4 and 8 last-level rows per thread (last level of 160 / 384 / 1024 rows)
-    (8 * 40960, 40960, dict(rs_fused=1)),
-    (8 * 98304, 98304, dict(rs_fused=1)),
-    (1 << 21, 1 << 18, dict(rs_fused=1)),
-    (1 << 13, 1 << 10, dict(rs_topmax=64, rs_fused=1)),
-    (8 * 1000, 1000, dict(rs_topmax=64, rs_fused=1)),
-    (8 * 513, 513, dict(rs_topmax=2, rs_fused=1)),
 ]
 
 
@@ -179,7 +196,7 @@ def test_rs_levels(N, P, opts):
 
 
 @pytest.mark.parametrize("N,P,opts", [(1 << 21, 1 << 18, dict()), (1 << 21, 1 << 18, dict(pdl=0)),
-                                       (8 * 98304, 98304, dict()), (8 * 98304, 98304, dict(rs_fused=1))])
+                                       (8 * 98304, 98304, dict())])
 def test_refill_race_stress(N, P, opts):
     """Repeated fresh plans on L2-resident systems with m = 8: the shapes on which the TMA refill of the input tile
     overtook shared-memory loads still queued behind the CTA barrier (about 1 call in 10 before the
@@ -250,6 +267,21 @@ def test_errors_on_device():
     with pytest.raises(B.CnError) as ei:
         B.cn_step(plan.h, psi.data_ptr() + 8, 1)
     assert ei.value.status == B.CN_EINVAL
+    # every option value the header documents is accepted, everything else is CN_EINVAL (include/cn_nshape.h)
+    good = {B.CN_OPT_PATH: (0, 1, 2), B.CN_OPT_TILE_THREADS: (0, 128, 256, 512), B.CN_OPT_RS_TOPMAX: (1, 4096, 8192),
+            B.CN_OPT_RS_LEVELS: (-1, 0, 1, 8), B.CN_OPT_PROFILE: (0, 1), B.CN_OPT_PDL: (0, 1), B.CN_OPT_ONCHIP: (0, 1),
+            B.CN_OPT_RS_GROUP: (2, 256, 1 << 20), B.CN_OPT_RS_SERIAL_TOP: (0, 1), B.CN_OPT_RS_TOP_IN_SUBST: (0, 1, 1024),
+            B.CN_OPT_KEEP_P: (0, 1)}
+    bad = {B.CN_OPT_PATH: (-1, 3), B.CN_OPT_TILE_THREADS: (64, 1024), B.CN_OPT_RS_TOPMAX: (0, 8193),
+           B.CN_OPT_RS_LEVELS: (-2, 9), B.CN_OPT_RS_GROUP: (1, (1 << 20) + 1), 4: (0, 1), 9: (0, 1), 0: (0,), 14: (0,)}
+    for key, vals in good.items():
+        for v in vals:
+            plan.set_option(key, v)
+    for key, vals in bad.items():
+        for v in vals:
+            with pytest.raises(B.CnError) as ei:
+                plan.set_option(key, v)
+            assert ei.value.status == B.CN_EINVAL, (key, v)
     plan.close()
     # V given as a device tensor
     dV = torch.zeros(64, dtype=torch.float64, device="cuda")
@@ -284,10 +316,10 @@ def test_config_c2_full_size(name):
 
 
 def test_config_c2_full_step_count():
-    """C2 at full size for the config's FULL step count (1000 steps, 10 calls of 100 as bench.py issues them): the
-    oracle needs ~5 minutes for that, so the check is by properties that hold at any size -- the norm (CN is unitary:
-    1e-12 per 1000 steps is the oracle's own pin), time reversal with a plan of -dt, and the oracle element by
-    element on the last 5 steps restarted from the GPU state after 995."""
+    """C2 at full size for the config's FULL step count (1000 steps, 10 calls of 100 as bench.py issues them) by
+    properties that hold at any size -- the norm (CN is unitary: 1e-12 per 1000 steps is the oracle's own pin), time
+    reversal with a plan of -dt, and the oracle on the last 5 steps restarted from the GPU state after 995.  The
+    element-by-element comparison with 1000 ORACLE steps is tests/test_gpu_zz_fullsteps.py::test_config_c2_all_steps."""
     torch = torch_()
     cfg = W.CONFIGS["C2dense"]
     V, psi = W.potential(cfg), W.psi0(cfg)
@@ -302,7 +334,7 @@ def test_config_c2_full_step_count():
         plan.step(d, 5)
         torch.cuda.synchronize()
         out = d.cpu().numpy()
-    assert abs(np.vdot(out, out).real * cfg.dx - 1.0) <= 1e-11
+    assert abs(np.vdot(out, out).real * cfg.dx - 1.0) <= 1e-12
     assert np.max(np.abs(out - O.step(cfg.dx, cfg.dt, V, mid, 5))) <= TOL_PSI
     with B.Plan(cfg.N, cfg.P, cfg.dx, -cfg.dt, V) as back:
         back.factorize()

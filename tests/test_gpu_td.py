@@ -40,7 +40,7 @@ CASES = [
     (4096, 64, dict(path=B.PATH_GENERIC)),
     (4096, 64, dict()),                              # auto: the on-chip stepper is NOT used for driven steps
     (5000, 123, dict()),                             # ragged blocks -> generic kernels
-    (1 << 16, 1 << 13, dict(rs_fused=1)),            # nested RS, fused last two levels
+    (1 << 16, 1 << 13, dict()),                      # nested RS
     (1 << 16, 1 << 13, dict(pdl=0)),
     (1 << 18, 1 << 10, dict()),
 ]
