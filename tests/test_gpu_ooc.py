@@ -24,7 +24,7 @@ OOC_CASES = [
     (1 << 18, 1 << 6, 3 << 20, 3),      # m = 4096: tile = block = 4096 points
     (1 << 15, 1 << 7, 400000, 5),       # parts of a single tile
     (3 << 15, 3 << 7, 1 << 20, 3),      # N not a power of two
-    ((1 << 15) + 256, 129, 2200000, 3), # 3 parts; the last one (256 points, not a whole tile) lands in a buffer that never held a full part
+    ((1 << 15) + 256, 129, 1000000, 3), # the last part (256 points) is not a whole tile: its tail reads the zeroed / stale buffer rows
 ]
 
 
