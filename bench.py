@@ -40,6 +40,15 @@ CN_PER_STEP = 100            # CN steps per bench step (one cn_step call)
 BYTES_PER_POINT_STEP = 56.0  # algorithmic: psi in 16 + q 16 + gamma 8 + psi out 16
 METRIC = "cn_grid_point_steps_per_sec_complex128"
 UNIT = "Gpoint-steps/s"
+WORKLOAD = ("C2 (N=2^24 complex128, dx=0.05, dt=0.005, soft-Coulomb V, Gaussian x random phase + 1e-3 dense noise, "
+            "1000 CN steps)")
+
+
+def bench_config(cfg, P, world):
+    """`config` of the JSON line: the workload only, identical for both arms (--impl ours / reference)."""
+    return {"workload": WORKLOAD, "N": cfg.N, "P": P, "dx": cfg.dx, "dt": cfg.dt, "cn_steps": cfg.steps,
+            "l2_policy": "inputs_larger_than_L2 (psi 268 MB + factors 403 MB per pass vs 126 MB L2)",
+            "parallelism": "replicas x%d" % world}
 
 
 def measured_peaks():
@@ -54,16 +63,22 @@ def measured_peaks():
 
 
 def ncu_traffic_per_launch():
-    """dram bytes per fused-pass launch from the committed ncu --set full capture, if any (profiles/)."""
-    path = os.path.join(ROOT, "profiles", "pass_kernel_traffic.txt")
+    """(dram bytes per fused-pass launch, where the figure comes from): the committed ncu --set full capture under
+    profiles/ -- ncu cannot run inside a timed bench, so the line says which capture (file, commit) it quotes."""
+    rel = os.path.join("profiles", "pass_kernel_traffic.txt")
+    val, src = None, None
     try:
-        with open(path) as f:
+        with open(os.path.join(ROOT, rel)) as f:
             for line in f:
                 if line.startswith("dram_bytes_per_launch_at_N_2^24="):
-                    return float(line.split("=")[1])
+                    val = float(line.split("=")[1])
+                elif line.startswith("source="):
+                    src = line.split("=", 1)[1].strip()
     except Exception:
         pass
-    return None
+    if val is None:
+        return None, None
+    return val, "%s (%s)" % (rel, src or "ncu --set full capture, see the file")
 
 
 class ClockSampler:
@@ -122,6 +137,117 @@ class ClockSampler:
 
 dist_env = R.dist_env
 
+def per_config_report(torch, peak, full, with_cpu):
+    """Every other BASELINE.json config (and the two "next" front ends at C2's shape) under the same clock as the headline:
+    a few ms of GPU time each through the C-ABI (paper_2205_00856_b200/report.py holds the timing loops), each with
+    the oracle timed on a bounded sample of the same workload on this box's host cores.  C3 (2^30 points, 85 GB of
+    host memory, minutes of input generation) and C5 (2^29 points streamed from pinned host memory) only with --full.
+    `frac` = algorithmic bytes / time / measured copy peak; the algorithmic bytes per unit are DESIGN.md's."""
+    from paper_2205_00856_b200 import report as RP
+    out = {}
+
+    def cpu(value, unit, cores, sample):
+        return {"value": value, "unit": unit, "cores": cores, "kind": "oracle", "host_cores_available": os.cpu_count(),
+                "sample": sample}
+
+    O = None
+    if with_cpu:
+        from oracle import cn_oracle as O  # noqa: N811  (cpu_baseline leg only)
+
+    # ---- C1: N = 4096 lives on one SM; latency bound, no HBM roofline -------------------------------------------
+    cfg = W.CONFIGS["C1"]
+    r = RP.run_1d(torch, "C1", peak)
+    r3 = RP.run_1d(torch, "C1", peak, onchip=0)
+    c1 = {"workload": "C1 (N=4096, P=64, dx=0.1, dt=0.01, harmonic V, 100 CN steps)", "us_per_cn_step": r["us_per_cn_step_best"],
+          "Gpoint_steps_per_s": r["Gpoint_steps_per_s"], "path": r["path"],
+          "us_per_cn_step_three_launches": r3["us_per_cn_step_best"],
+          "roofline": "none: psi (64 KB) stays in the registers of one CTA for the whole call; latency / FP64-issue bound"}
+    if O:
+        V, psi = W.potential(cfg), W.psi0(cfg)
+        sec = sum(O.step(cfg.dx, cfg.dt, V, psi, cfg.steps, return_seconds=True)[1] for _ in range(20))
+        c1["cpu_baseline"] = cpu(cfg.N * cfg.steps * 20 / sec / 1e9, UNIT, 1, "20 x the config's 100 steps, serial Thomas")
+    out["C1"] = c1
+
+    # ---- C4: many-systems sweeps, 32 B per point per sweep -----------------------------------------------------
+    cfg = W.CONFIGS["C4"]
+    r = RP.run_c4(torch, peak)
+    c4 = {"workload": "C4 (8192 x 8192, dx=dy=0.05, dt=0.002, V=0.5(x^2+y^2), x-sweep then y-sweep, 20 steps)",
+          "bytes_per_point_sweep": 32, "x": r["x"], "y": r["y"], "xy": r["xy"],
+          "Gpoint_steps_per_s": r["Gpoint_steps_per_s"], "frac": r["xy"]["hbm_frac_measured_peak"]}
+    if O:
+        psi2 = W.psi0_2d(cfg)
+        Vx, Vy = W.potential(cfg), W.potential_y(cfg)
+        _, sec = O.step_2d(cfg.dx, cfg.dt, Vx, Vy, psi2, 1, return_seconds=True)
+        c4["cpu_baseline"] = cpu(cfg.N * cfg.N / sec / 1e9, UNIT, 1, "1 of the 20 2-D steps at full size, serial loops over the systems")
+        _, sec, nth = O.step_2d_omp(cfg.dx, cfg.dt, Vx, Vy, psi2, 2)
+        c4["cpu_baseline_all_cores"] = cpu(2 * cfg.N * cfg.N / sec / 1e9, UNIT, nth,
+                                           "2 of the 20 2-D steps at full size, OpenMP over the independent systems of a sweep")
+        del psi2
+    out["C4"] = c4
+
+    # ---- time-dependent H at C2's shape (row f-2) ---------------------------------------------------------------
+    cfg = W.CONFIGS["C2dense"]
+    r = RP.run_td(torch, peak)
+    td_bytes = RP.TD_BYTES_PER_POINT
+    td = {"workload": "C2 shape, H(t) = H0 + f(t) x: factorization redone on the device in every step",
+          "us_per_driven_step": r["us_per_driven_step"], "Gpoint_steps_per_s": r["Gpoint_steps_per_s"],
+          "bytes_per_point": td_bytes, "frac": td_bytes * cfg.N / (r["us_per_driven_step"] * 1e-6) / 1e9 / peak}
+    if O:
+        V, psi = W.potential(cfg), W.psi0(cfg)
+        t0 = time.time()
+        O.step_td(cfg.dx, cfg.dt, V, W.grid(cfg), [0.01, -0.02], psi)
+        td["cpu_baseline"] = cpu(2 * cfg.N / (time.time() - t0) / 1e9, UNIT, 1,
+                                 "2 driven steps at full N=2^24 (each a full Thomas solve with its own pivots)")
+    out["TD"] = td
+
+    # ---- general complex tridiagonal front end (row f-3) ------------------------------------------------------------
+    r = RP.run_tridiag(torch, peak)
+    tri = {"workload": "random diagonally dominant complex tridiagonal system, N=2^24, one right-hand side per solve",
+           "us_per_solve": r["us_per_solve"], "Grows_per_s": r["Grows_per_s"], "bytes_per_row": r["bytes_per_row"],
+           "frac": r["hbm_frac_measured_peak"]}
+    if O:
+        n = 1 << 22
+        rng = np.random.default_rng(2205)
+        z = lambda: rng.normal(size=n) + 1j * rng.normal(size=n)  # noqa: E731
+        b, c, d = z(), z(), z()
+        a = (np.abs(b) + np.abs(c)) * 2.5 * np.exp(1j * rng.uniform(0, 2 * np.pi, n))
+        t0 = time.time()
+        O.thomas(b, a, c, d)
+        tri["cpu_baseline"] = cpu(n / (time.time() - t0) / 1e9, "Grows/s", 1, "one Thomas solve of 2^22 rows of the same distribution")
+    out["TRI"] = tri
+
+    if full:
+        # ---- C3: 2^30 points resident (psi 17 GB + factors 26 GB) -----------------------------------------------------
+        cfg = W.CONFIGS["C3"]
+        r = RP.run_1d(torch, "C3", peak)
+        c3 = {"workload": "C3 (N=2^30, dx=0.01, dt=0.001, 32 seeded Gaussians, 50 CN steps)",
+              "us_per_cn_step": r["us_per_cn_step_best"], "Gpoint_steps_per_s": r["Gpoint_steps_per_s"],
+              "bytes_per_point": 56, "frac": r["hbm_frac_measured_peak"], "P_effective": r["P_effective"],
+              "rs_levels": r["rs_levels"]}
+        if O:
+            n = 1 << 26
+            sub = W.scaled(cfg, N=n)
+            V, psi = RP._inputs(sub)
+            sec = O.step_inplace(sub.dx, sub.dt, V, psi, 4, lean=True)
+            c3["cpu_baseline"] = cpu(4 * n / sec / 1e9, UNIT, 1, "4 lean-Thomas steps on 2^26 points with C3's parameters")
+        out["C3"] = c3
+        # ---- C5: out of core, bound by the host link --------------------------------------------------------------------
+        r = RP.run_c5(torch)
+        c5 = {"workload": "C5 (N=2^29 in pinned host memory, device budget 2 GB, harmonic V, 10 CN steps)",
+              "s_per_cn_step": r["s_per_cn_step"], "Gpoint_steps_per_s": r["Gpoint_steps_per_s"], "h2d_GBps": r["h2d_GBps"],
+              "d2h_GBps": r["d2h_GBps"], "link_GBps": r["link_GBps"], "frac_of_link": r["h2d_frac_of_link"],
+              "bytes_per_point": "24 in + 16 out over the host link", "device_bytes": r["device_bytes"]}
+        if O:
+            cfg = W.CONFIGS["C5"]
+            n = 1 << 26
+            sub = W.scaled(cfg, N=n)
+            V, psi = RP._inputs(sub)
+            sec = O.step_inplace(sub.dx, sub.dt, V, psi, 4, lean=True)
+            c5["cpu_baseline"] = cpu(4 * n / sec / 1e9, UNIT, 1, "4 lean-Thomas steps on 2^26 points with C5's parameters")
+        out["C5"] = c5
+    return out
+
+
 
 def oracle_timed(cfg, V, psi, cn_steps: int):
     from oracle import cn_oracle as O
@@ -150,10 +276,11 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "C2 (N=2^24, dx=0.05, dt=0.005, soft-Coulomb V, Gaussian x random phase + 1e-3 noise)",
-                   "cn_steps_per_bench_step": cn_per},
+        "config": bench_config(cfg, cfg.P, max(1, world)),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
-                         "sample": "%d CN steps at full N=2^24 per bench step, serial Thomas, 1 thread" % cn_per},
+                         "host_cores_available": os.cpu_count(),
+                         "sample": "%d CN steps at full N=2^24 per bench step (of the config's 1000), serial Thomas, "
+                                   "1 thread" % cn_per},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -173,6 +300,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--clock-interval-ms", type=int, default=20, help="nvidia-smi sampling period during the timed region")
     ap.add_argument("--sweep", action="store_true", help="also time the P sweep 2^8..2^16 (extra JSON key)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (C1, C4, TD, TRI)")
+    ap.add_argument("--full", action="store_true", help="per_config also runs C3 (2^30, 85 GB host) and C5 (2^29, streamed)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -256,9 +385,9 @@ def main():
     peak, peak_src = measured_peaks()
     pass_ms = prof["pass_ms"] / max(1, prof["pass_count"])
     achieved = BYTES_PER_POINT_STEP * cfg.N / (pass_ms * 1e-3) / 1e9 if prof["pass_count"] else None
-    traffic = ncu_traffic_per_launch()
+    traffic, traffic_src = ncu_traffic_per_launch()
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": (achieved / peak) if achieved else None, "traffic": traffic,
+                "frac": (achieved / peak) if achieved else None, "traffic": traffic, "traffic_source": traffic_src,
                 "kernel": "k_pass_tiled<TPB,LOGC,P1=1,P2=1> (fused SS(k) + RHS/RD/RU/JD/JU(k+1))",
                 "kernel_ms": pass_ms, "launches_timed": prof["pass_count"],
                 "rs_chain_ms": prof["rs_ms"] / max(1, prof["rs_count"]),
@@ -341,18 +470,22 @@ def main():
                "host_cores_available": os.cpu_count(),
                "sample": "first %d of the 1000 CN steps of C2 at full N=2^24 (serial Thomas, 1 thread)" % nsamp}
 
+    # ---- the other configs under the same clock (rank 0, N = 1): a few ms of GPU time each ------------------
+    info = plan.info()
+    per_config = None
+    if rank == 0 and world == 1 and not args.no_per_config:
+        per_config = per_config_report(torch, peak, args.full, not args.no_cpu_baseline)
+
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "C2 (N=2^24 complex128, dx=0.05, dt=0.005, soft-Coulomb V, Gaussian x random "
-                                   "phase + 1e-3 dense noise)", "N": cfg.N, "P": P, "cn_steps_per_bench_step": cn_per,
-                       "l2_policy": "inputs_larger_than_L2 (psi 268 MB + factors 403 MB per pass vs 126 MB L2)",
-                       "parallelism": "replicas x%d" % world, "path": plan.info()["path"],
-                       "tile_threads": plan.info()["tile_threads"], "factorize_ms": factor_ms},
+            "config": bench_config(cfg, P, world),
+            "launch": {"cn_steps_per_bench_step": cn_per, "path": info["path"], "P_effective": info["P_effective"],
+                       "tile_threads": info["tile_threads"], "rs_levels": info["rs_levels"], "factorize_ms": factor_ms},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-            "cpu_baseline": cpu,
+            "cpu_baseline": cpu, "per_config": per_config,
         }
         if sweep is not None:
             line["p_sweep"] = sweep

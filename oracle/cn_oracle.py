@@ -24,7 +24,10 @@ _SO = os.path.join(_HERE, "libcn_oracle.so")
 # no -ffast-math, no FTZ/DAZ; see the header of cn_thomas.c for -fcx-limited-range
 CFLAGS = ["-O2", "-std=c11", "-fPIC", "-shared", "-ffp-contract=off", "-fcx-limited-range", "-Wall"]
 
+_SO_OMP = os.path.join(_HERE, "libcn_oracle_omp.so")  # the same source + -fopenmp: adds cn_oracle_step_2d_omp (timing aid)
+
 _lib = None
+_lib_omp = None
 _lock = threading.Lock()
 
 
@@ -34,7 +37,25 @@ def build(force: bool = False) -> str:
         tmp = _SO + ".tmp%d" % os.getpid()
         subprocess.check_call(["gcc", *CFLAGS, "-o", tmp, _SRC, "-lm"])
         os.replace(tmp, _SO)
+    if force or not os.path.exists(_SO_OMP) or os.path.getmtime(_SO_OMP) < os.path.getmtime(_SRC):
+        tmp = _SO_OMP + ".tmp%d" % os.getpid()
+        subprocess.check_call(["gcc", *CFLAGS, "-fopenmp", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _SO_OMP)
     return _SO
+
+
+def _load_omp():
+    global _lib_omp
+    with _lock:
+        if _lib_omp is None:
+            build()
+            lib = ctypes.CDLL(_SO_OMP)
+            i64, dbl, ptr = ctypes.c_int64, ctypes.c_double, ctypes.c_void_p
+            lib.cn_oracle_step_2d_omp.restype = i64
+            lib.cn_oracle_step_2d_omp.argtypes = [i64, i64, dbl, dbl, ptr, ptr, ptr, i64, ctypes.POINTER(dbl),
+                                                  ctypes.POINTER(i64)]
+            _lib_omp = lib
+    return _lib_omp
 
 
 def _load():
@@ -150,6 +171,23 @@ def step_2d(dx: float, dt: float, Vx, Vy, psi, nsteps: int = 1, return_seconds: 
     if rc:
         raise RuntimeError("oracle failed rc=%d" % rc)
     return (out, sec.value) if return_seconds else out
+
+
+def step_2d_omp(dx: float, dt: float, Vx, Vy, psi, nsteps: int = 1):
+    """`step_2d` with the independent systems of every sweep shared out over all host cores by OpenMP (the multi-core
+    C4 CPU baseline of BASELINE.md section 3).  Each thread runs the unchanged serial per-system step, so the result
+    is bit-identical to `step_2d` (pinned in tests/test_oracle_pins.py).  Returns (psi, seconds, threads used)."""
+    Vx = np.ascontiguousarray(Vx, dtype=np.float64)
+    Vy = np.ascontiguousarray(Vy, dtype=np.float64)
+    out = _z(psi).copy()
+    ny, nx = out.shape
+    assert Vx.size == nx and Vy.size == ny
+    sec, nth = ctypes.c_double(0.0), ctypes.c_int64(0)
+    rc = _load_omp().cn_oracle_step_2d_omp(nx, ny, dx, dt, _p(Vx), _p(Vy), _p(out), nsteps, ctypes.byref(sec),
+                                           ctypes.byref(nth))
+    if rc:
+        raise RuntimeError("oracle failed rc=%d" % rc)
+    return out, sec.value, int(nth.value)
 
 
 def dense_T(dx: float, dt: float, V) -> np.ndarray:

@@ -215,3 +215,52 @@ int64_t cn_oracle_step_2d(int64_t nx, int64_t ny, double dx, double dt, const do
     if (seconds_out) *seconds_out = acc;
     return 0;
 }
+
+/* ---- C4 timed on all host cores (SURVEY 8d "Oracle timing") ------------------------
+ * The SAME 2-D step with the independent systems of a sweep shared out over OpenMP threads (static schedule);
+ * compiled only with -fopenmp into libcn_oracle_omp.so.  Every thread runs the unchanged serial sys_step on its
+ * systems with a scratch vector of its own, so the result is bit-identical to cn_oracle_step_2d
+ * (tests/test_oracle_pins.py::test_step_2d_omp_is_bitwise_serial).  A CPU-baseline timing aid: parity tests use the
+ * serial function above. */
+#ifdef _OPENMP
+#include <omp.h>
+int64_t cn_oracle_step_2d_omp(int64_t nx, int64_t ny, double dx, double dt, const double *Vx, const double *Vy,
+                              zc *psi, int64_t nsteps, double *seconds_out, int64_t *threads_out)
+{
+    cn_oracle_sys Sx, Sy;
+    int64_t rc = sys_init(&Sx, nx, dx, dt, Vx);
+    if (rc) return rc;
+    rc = sys_init(&Sy, ny, dx, dt, Vy);
+    if (rc) { sys_free(&Sx); return rc; }
+    int64_t bad = 0, nthreads = 1;
+    double t0 = now_s();
+#pragma omp parallel
+    {
+        cn_oracle_sys Lx = Sx, Ly = Sy; /* shared read-only coefficients, private right-hand-side scratch */
+        Lx.d = malloc(sizeof(zc) * nx);
+        Ly.d = malloc(sizeof(zc) * ny);
+        if (!Lx.d || !Ly.d) {
+#pragma omp atomic write
+            bad = 1;
+        }
+#pragma omp single
+        nthreads = omp_get_num_threads();
+#pragma omp barrier
+        if (!bad) {
+            for (int64_t k = 0; k < nsteps; ++k) {
+#pragma omp for schedule(static)
+                for (int64_t y = 0; y < ny; ++y) sys_step(&Lx, psi + y * nx, 1);
+#pragma omp for schedule(static)
+                for (int64_t x = 0; x < nx; ++x) sys_step(&Ly, psi + x, nx);
+            }
+        }
+        free(Lx.d);
+        free(Ly.d);
+    }
+    double acc = now_s() - t0;
+    sys_free(&Sx); sys_free(&Sy);
+    if (seconds_out) *seconds_out = acc;
+    if (threads_out) *threads_out = nthreads;
+    return bad ? -1 : 0;
+}
+#endif

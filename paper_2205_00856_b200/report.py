@@ -198,6 +198,11 @@ def p_sweep(torch, peak, name="C2dense"):
     return {"config": name + " P sweep", "N": cfg.N, "sqrtN": math.isqrt(cfg.N), "rows": rows, "fit": fits}
 
 
+# algorithmic HBM bytes per point of one driven step: factor kernel V 8 + g 8 in, q 16 + gamma 8
+# out; prologue pass psi 16 + q 16 + gamma 8 in; epilogue pass the same in + psi 16 out
+TD_BYTES_PER_POINT = 136
+
+
 def run_td(torch, peak, name="C2dense", nsteps=20):
     """Driven steps (H(t) = H0 + f(t) x, cn_step_td): factorization inside the step loop, two passes per step."""
     cfg = W.CONFIGS[name]
@@ -263,10 +268,11 @@ def levels_study(torch, N=300000):
     V, psi = _inputs(cfg)
     d = torch.from_numpy(psi).cuda()
     rows = []
+    big = N > (1 << 20)  # at 2^24 the far ends of the curves cost seconds per step: start at 2^8, cap the serial RS
     for n_it in (1, 2, 3):
-        for k in range(4, 18):
+        for k in range(8 if big else 4, 23 if big else 18):
             P0 = 1 << k
-            if P0 > N // 2:
+            if P0 > N // 2 or (big and n_it == 1 and k > 17):
                 break
             if n_it == 1:
                 opts = dict(path=B.PATH_GENERIC, rs_levels=-1)
@@ -277,7 +283,7 @@ def levels_study(torch, N=300000):
                 opts = dict(path=B.PATH_GENERIC, rs_levels=n_it, rs_group=r, rs_serial_top=1)
             with B.Plan(cfg.N, P0, cfg.dx, cfg.dt, V, **opts) as plan:
                 plan.factorize()
-                best, _ = time_plan(torch, plan, d, 10, reps=3)
+                best, _ = time_plan(torch, plan, d, 4 if big else 10, reps=2 if big else 3)
             rows.append({"n_it": n_it, "P0": P0, "fanout": r, "us_per_cn_step": 1e3 * best})
     summary = {}
     for n_it in (1, 2, 3):
@@ -292,7 +298,8 @@ def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", default="C1,C2,C3,C4,C5")
     ap.add_argument("--sweep", action="store_true")
-    ap.add_argument("--levels", action="store_true", help="nested multi-iteration study at n_tot = 3e5")
+    ap.add_argument("--levels", action="store_true", help="nested multi-iteration study (PAPER.md Fig. 2, Eq. 8-9)")
+    ap.add_argument("--levels-n", default="300000", help="comma list of system sizes for --levels (paper: 3e5)")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
     import torch
@@ -327,7 +334,8 @@ def main(argv=None):
     if args.sweep:
         emit(p_sweep(torch, peak))
     if args.levels:
-        emit(levels_study(torch))
+        for n in args.levels_n.split(","):
+            emit(levels_study(torch, int(n)))
     return 0
 
 

@@ -114,6 +114,25 @@ def test_step_2d_vs_dense():
     assert np.max(np.abs(out - ref)) <= 1e-13
 
 
+def test_step_2d_omp_is_bitwise_serial():
+    # the multi-core timing copy (bench.py's C4 cpu_baseline) runs the unchanged per-system step: same bits, and the
+    # dense reference of the test above pins it independently
+    nx, ny, dx, dt = 37, 29, 0.3, 0.07
+    rng = np.random.default_rng(5)
+    Vx, Vy = rng.uniform(-1, 1, nx), rng.uniform(-1, 1, ny)
+    psi = rng.standard_normal((ny, nx)) + 1j * rng.standard_normal((ny, nx))
+    out, sec, threads = O.step_2d_omp(dx, dt, Vx, Vy, psi, 4)
+    assert threads >= 1 and sec >= 0.0
+    assert np.array_equal(out, O.step_2d(dx, dt, Vx, Vy, psi, 4))
+    Tx = np.eye(nx) + 0.5j * dt * hamiltonian_dense(dx, Vx)
+    Ty = np.eye(ny) + 0.5j * dt * hamiltonian_dense(dx, Vy)
+    ref = psi.copy()
+    for _ in range(4):
+        ref = np.linalg.solve(Tx, Tx.conj().T @ ref.T).T
+        ref = np.linalg.solve(Ty, Ty.conj().T @ ref)
+    assert np.max(np.abs(out - ref)) <= 1e-13
+
+
 # ---- invariants -----------------------------------------------------------------------------------
 def test_norm_conservation_c1():
     cfg = W.CONFIGS["C1"]
