@@ -191,6 +191,47 @@ cn_status cn_tridiag_create(cn_tridiag **out, int64_t N, const void *b, const vo
 cn_status cn_tridiag_solve(cn_tridiag *t, const void *d, void *x, void *stream);
 cn_status cn_tridiag_destroy(cn_tridiag *t);
 
+/*
+ * Sharded mode: ONE system of N_total rows spread over `nshards` processes / GPUs, the wave function
+ * never gathered ("neither the matrix nor the wavefunction ever need to be placed entirely on a
+ * single process ... the only data that needs to be gathered is on the joint lines"), one small exchange around the
+ * RS stage per step (section 5.2.1; process layout of PAPER.md:282-288 section 6.2).
+ *
+ * Shard r (0 <= r < nshards, in row order) owns N_local consecutive rows -- the same N_local (a multiple of 256) and
+ * the same options on every shard -- with its own factors, slots and nested RS levels over its own joint lines.
+ * Its last row is a joint line of every level, so the shard is one block of the partition method applied once more
+ * on top (Eq. 6).  What crosses shards, as opaque records of complex128 values that the CALLER
+ * all-gathers in rank order (any transport: NCCL, MPI, peer copies; the library never communicates):
+ *   - once per (H, dt), the matrix side:  cn_shard_factorize_local writes this shard's record of
+ *     `matrix_count` values, cn_shard_factorize_finish reads the nshards records and factors the last RS level of the
+ *     whole system, replicated on every shard (no root process; PAPER.md:207 names the alternative);
+ *   - per step, the d side: a record of `step_count` = nt + 1 values -- the JU contribution to the last row of the
+ *     preceding shard and the right-hand sides of this shard's nt last-level rows; with nt = 1 these are the two
+ *     values per process of PAPER.md:175 for a pre-factored matrix.  The two support values a process gets back
+ *      are computed locally from the gathered records;
+ *   - once per run, psi^0 on the last row of every shard (1 value; cn_shard_edge), which the first explicit half-step
+ *     of the next shard needs (Eq. 3).
+ * A run of n steps on one vector:  cn_shard_edge -> gather -> cn_shard_prologue -> [gather -> cn_shard_advance] x (n-1)
+ * -> gather -> cn_shard_epilogue.   Stages: prologue = RHS + RD/RU/JD/JU of step 1 and the local reductions; advance =
+ * last-level RS + substitutions + SS of step k fused with RHS + RD/RU/JD/JU of step k+1 + local
+ * reductions; epilogue = last-level RS + substitutions + SS.  All records are DEVICE pointers, 16-byte aligned; every
+ * call is asynchronous on `stream` except the two factorize calls, which synchronise it once.  psi is the shard's
+ * N_local complex128 DEVICE vector, updated in place.  nshards = 1 is allowed (records unused).
+ * Errors: CN_EINVAL for shapes the sharded mode does not take (N_local not a multiple of 256, forced generic path,
+ * device budget, RS options other than CN_OPT_RS_TOPMAX) and for gathered matrix records that are not nshards records
+ * of equal-shaped shards in rank order.  cn_factorize / cn_step / cn_step_td on a plan with nshards > 1: CN_EINVAL.
+ */
+cn_status cn_shard_plan_create(cn_plan **out, int64_t N_local, int64_t P_local, double dx, double dt,
+                               const double *V_local, int32_t shard, int32_t nshards);
+/* complex128 values per shard record: matrix_count (factorize), step_count (every step) */
+cn_status cn_shard_counts(const cn_plan *plan, int64_t *matrix_count, int64_t *step_count);
+cn_status cn_shard_factorize_local(cn_plan *plan, void *matrix_send, void *stream);
+cn_status cn_shard_factorize_finish(cn_plan *plan, const void *matrix_all, void *stream);
+cn_status cn_shard_edge(cn_plan *plan, const void *psi, void *edge_send, void *stream);
+cn_status cn_shard_prologue(cn_plan *plan, void *psi, const void *edges_all, void *step_send, void *stream);
+cn_status cn_shard_advance(cn_plan *plan, void *psi, const void *step_all, void *step_send, void *stream);
+cn_status cn_shard_epilogue(cn_plan *plan, void *psi, const void *step_all, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

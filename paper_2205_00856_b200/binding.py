@@ -21,7 +21,9 @@ PATH_AUTO, PATH_GENERIC, PATH_TILED, PATH_ONCHIP = 0, 1, 2, 3
 EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", "cn_factorize", "cn_step",
            "cn_batched_sweep", "cn_destroy", "cn_plan_get_info", "cn_plan_get_profile", "cn_status_string",
            "cn_last_cuda_error", "cn_version", "cn_plan_set_td_shape", "cn_step_td",
-           "cn_tridiag_create", "cn_tridiag_solve", "cn_tridiag_destroy"]
+           "cn_tridiag_create", "cn_tridiag_solve", "cn_tridiag_destroy",
+           "cn_shard_plan_create", "cn_shard_counts", "cn_shard_factorize_local", "cn_shard_factorize_finish",
+           "cn_shard_edge", "cn_shard_prologue", "cn_shard_advance", "cn_shard_epilogue"]
 
 
 class CnError(RuntimeError):
@@ -73,6 +75,14 @@ def lib():
         L.cn_tridiag_destroy.argtypes = [vp]
         L.cn_batched_sweep.restype = i32
         L.cn_batched_sweep.argtypes = [vp, vp, i64, i64, i64, i64, vp]
+        L.cn_shard_plan_create.restype = i32
+        L.cn_shard_plan_create.argtypes = [ctypes.POINTER(vp), i64, i64, dbl, dbl, vp, ctypes.c_int32, ctypes.c_int32]
+        L.cn_shard_counts.restype = i32
+        L.cn_shard_counts.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64)]
+        for name, n in (("cn_shard_factorize_local", 3), ("cn_shard_factorize_finish", 3), ("cn_shard_edge", 4),
+                        ("cn_shard_prologue", 5), ("cn_shard_advance", 5), ("cn_shard_epilogue", 4)):
+            getattr(L, name).restype = i32
+            getattr(L, name).argtypes = [vp] * n
         L.cn_destroy.restype = i32
         L.cn_destroy.argtypes = [vp]
         L.cn_plan_get_info.restype = i32
@@ -204,6 +214,65 @@ class Tridiag:
     def close(self):
         if self.h:
             lib().cn_tridiag_destroy(self.h)
+            self.h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class ShardPlan:
+    """One shard of a system spread over several processes (cn_shard_*): marshalling only.  The records are device
+    tensors owned by the caller; `paper_2205_00856_b200.sharded` holds the protocol that moves them."""
+
+    def __init__(self, N_local, P_local, dx, dt, V_local, shard, nshards, **opts):
+        h = ctypes.c_void_p()
+        st = lib().cn_shard_plan_create(ctypes.byref(h), N_local, P_local, dx, dt, _ptr(V_local), shard, nshards)
+        _check(None, st, "cn_shard_plan_create")
+        self.h, self.N, self.shard, self.nshards = h, N_local, shard, nshards
+        for k, v in opts.items():
+            cn_plan_set_option(self.h, {"rs_topmax": CN_OPT_RS_TOPMAX, "pdl": CN_OPT_PDL, "keep_p": CN_OPT_KEEP_P,
+                                        "tile_threads": CN_OPT_TILE_THREADS}[k], v)
+
+    def counts(self):
+        m, s = ctypes.c_int64(0), ctypes.c_int64(0)
+        _check(self.h, lib().cn_shard_counts(self.h, ctypes.byref(m), ctypes.byref(s)), "cn_shard_counts")
+        return int(m.value), int(s.value)
+
+    def factorize_local(self, matrix_send, stream=None):
+        _check(self.h, lib().cn_shard_factorize_local(self.h, _ptr(matrix_send), _stream(stream)), "cn_shard_factorize_local")
+
+    def factorize_finish(self, matrix_all, stream=None):
+        _check(self.h, lib().cn_shard_factorize_finish(self.h, _ptr(matrix_all), _stream(stream)), "cn_shard_factorize_finish")
+
+    def edge(self, psi, edge_send, stream=None):
+        _check(self.h, lib().cn_shard_edge(self.h, _ptr(psi), _ptr(edge_send), _stream(stream)), "cn_shard_edge")
+
+    def prologue(self, psi, edges_all, step_send, stream=None):
+        _check(self.h, lib().cn_shard_prologue(self.h, _ptr(psi), _ptr(edges_all), _ptr(step_send), _stream(stream)),
+               "cn_shard_prologue")
+
+    def advance(self, psi, step_all, step_send, stream=None):
+        _check(self.h, lib().cn_shard_advance(self.h, _ptr(psi), _ptr(step_all), _ptr(step_send), _stream(stream)),
+               "cn_shard_advance")
+
+    def epilogue(self, psi, step_all, stream=None):
+        _check(self.h, lib().cn_shard_epilogue(self.h, _ptr(psi), _ptr(step_all), _stream(stream)), "cn_shard_epilogue")
+
+    def info(self):
+        return cn_plan_get_info(self.h)
+
+    def close(self):
+        if self.h:
+            cn_destroy(self.h)
             self.h = None
 
     def __enter__(self):

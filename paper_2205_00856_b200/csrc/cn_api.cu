@@ -18,6 +18,7 @@
 #include "cn_reduced.cuh"
 #include "cn_batched.cuh"
 #include "cn_onchip.cuh"
+#include "cn_shard.cuh"
 
 typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                     const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
@@ -69,6 +70,15 @@ struct cn_plan {
     double *tdG = nullptr, *tdV = nullptr;
     cplx *tdRed = nullptr;
     int64_t tdRedP = 0;
+    // sharded mode (cn_shard_*; cn_shard.cuh): this plan holds rows of ONE system that nshards processes share
+    int shard = 0, nshards = 1;
+    bool above = false, below = false; // a shard precedes / follows this one
+    int64_t nt = 0;                    // rows of this shard's last RS level (equal on all shards)
+    cplx *topX[2] = {nullptr, nullptr}; // support values of the whole last level (nshards * nt), ping-pong like sup[]
+    cplx *gsub = nullptr, *gdiag = nullptr, *gsup = nullptr; // the whole last-level matrix, assembled from the records
+    cplx *diagAcc = nullptr;           // what this shard adds to the diagonal of the row above it, summed over the levels
+    int sh_out = 1;                    // sup[] / topX[] buffer the pending RS writes
+    bool sh_local_done = false;        // cn_shard_factorize_local has run, cn_shard_factorize_finish is due
     // profiling (CN_OPT_PROFILE): event pairs around fused-pass (kind 0) and RS (kind 1) launches
     struct ev_pair { cudaEvent_t a, b; int kind; };
     std::vector<ev_pair> ev_pool;
@@ -121,6 +131,20 @@ static cn_status dev_alloc(cn_plan *p, T **ptr, size_t count)
     return CN_OK;
 }
 
+// the same with one guard element in front (index -1), zeroed: sharded plans keep there what belongs to the row above
+// the shard (cn_shard.cuh); `guard` = false is plain dev_alloc
+template <typename T>
+static cn_status dev_alloc_g(cn_plan *p, T **ptr, size_t count, bool guard)
+{
+    if (!guard) return dev_alloc(p, ptr, count);
+    T *raw = nullptr;
+    cn_status st = dev_alloc(p, &raw, count + 1);
+    if (st != CN_OK) return st;
+    if (cudaMemset(raw, 0, sizeof(T)) != cudaSuccess) return CN_ECUDA;
+    *ptr = raw + 1;
+    return CN_OK;
+}
+
 static void free_factors(cn_plan *p)
 {
     for (void *x : p->owned) cudaFree(x);
@@ -132,6 +156,8 @@ static void free_factors(cn_plan *p)
     p->slotD = p->slotU = nullptr; p->sup[0] = p->sup[1] = nullptr; p->work = nullptr; p->derr = nullptr;
     p->qB = nullptr;
     p->gamJ = nullptr;
+    p->topX[0] = p->topX[1] = nullptr; p->gsub = p->gdiag = p->gsup = nullptr; p->diagAcc = nullptr;
+    p->sh_local_done = false;
     for (int b = 0; b < cn_plan::NB; ++b) { p->bPsi[b] = nullptr; p->bQ[b] = nullptr; p->bV[b] = nullptr; }
     p->factorized = false;
     p->tmPsiFor = nullptr;
@@ -468,16 +494,21 @@ static cn_status ooc_setup(cn_plan *p, int64_t m)
 
 // The arithmetic of the factorization: every matrix-side quantity of RD/RU/JD/JU from the potential
 // `Vsrc`, the reduced matrices of all RS levels and their factors.  Launches only (no allocation, no synchronisation):
-// cn_factorize calls it once, cn_step_td once per step with the potential of that step.  `red`: 6 P complex scratch.
+// cn_factorize calls it once, cn_step_td once per step with the potential of that step.  `red`: CN_RED_COUNT(P) complex
+// scratch = six arrays of P values, each with a guard element in front (used by sharded plans only).
+#define CN_RED_COUNT(P) (6 * ((size_t)(P) + 1))
 static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64_t m, cudaStream_t stream, bool whole = true,
                                 const double *tdG = nullptr, double tdF = 0.0)
 {
     const int64_t N = p->N, P = p->P;
     const int nlv = (int)p->lv.size();
     cn_status st;
-    cplx *redSubD = red, *redDiagD = red + P, *redSupU = red + 2 * P, *redDiagU = red + 3 * P;
-    cplx *tmpA = red + 4 * P, *tmpB = red + 5 * P;
-    CN_CUDA(p, cudaMemsetAsync(red, 0, sizeof(cplx) * 6 * (size_t)P, stream));
+    const int64_t Pg = P + 1;
+    cplx *redSubD = red + 1, *redDiagD = red + Pg + 1, *redSupU = red + 2 * Pg + 1, *redDiagU = red + 3 * Pg + 1;
+    cplx *tmpA = red + 4 * Pg + 1, *tmpB = red + 5 * Pg + 1;
+    const int above = p->above ? 1 : 0;
+    const bool sharded = p->nshards > 1;
+    CN_CUDA(p, cudaMemsetAsync(red, 0, sizeof(cplx) * CN_RED_COUNT(P), stream));
     CN_CUDA(p, cudaMemsetAsync(p->derr, 0, sizeof(int), stream));
     CN_CUDA(p, cudaMemsetAsync(p->slotU, 0, sizeof(cplx) * (size_t)P, stream));
 
@@ -492,7 +523,7 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
         }
         const int64_t nch = N / 8;
         const unsigned gridc = (unsigned)((nch + 127) / 128);
-#define CN_FB(L) k_factor_blocks_chunked<L><<<gridc, 128, 0, stream>>>(nch, p->two_dx2, p->rho, Vsrc, tdG, tdF, p->q, p->gam, redSubD, redDiagD, redSupU, redDiagU, p->derr)
+#define CN_FB(L) k_factor_blocks_chunked<L><<<gridc, 128, 0, stream>>>(nch, p->two_dx2, p->rho, Vsrc, tdG, tdF, p->q, p->gam, redSubD, redDiagD, redSupU, redDiagU, p->derr, above)
         switch (logc) {
         case 0: CN_FB(0); break;
         case 1: CN_FB(1); break;
@@ -501,6 +532,7 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
         case 4: CN_FB(4); break;
         case 5: CN_FB(5); break;
         default:
+            if (sharded) return CN_EINVAL; // sharded plans: blocks of 8 * 2^k <= 256 rows, whole warps of chunks
             if (tdG) { // the thread-per-block kernel takes the potential of the step ready-made
                 k_td_potential<<<(unsigned)((N + 255) / 256), 256, 0, stream>>>(N, Vsrc, tdG, tdF, p->tdV);
                 Vsrc = p->tdV;
@@ -527,7 +559,8 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
         }
     }
     k_rs_assemble0<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(P, N, p->rho, p->gam, p->gamJ, redSubD, redDiagD, redSupU,
-                                                                 redDiagU, p->lv[0].sub, p->lv[0].diag, p->lv[0].sup);
+                                                                 redDiagU, p->lv[0].sub, p->lv[0].diag, p->lv[0].sup, above,
+                                                                 p->diagAcc);
     p->launches += 2;
     if (p->qB && whole) { // one block per system: the factors of cn_batched_sweep and of the on-chip stepper
         k_factor_whole<<<1, 32, 0, stream>>>(N, p->rho, p->gam, p->qB, p->derr);
@@ -537,14 +570,14 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
         cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
         if (p->opt_rs_group == CN_RS_G)
             k_rs_factor_level_smem<<<(unsigned)((U.n + CN_RS_FL_WARPS - 1) / CN_RS_FL_WARPS), 32 * CN_RS_FL_WARPS, 0, stream>>>(
-                L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr);
+                L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr, above);
         else
         k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, (int64_t)p->opt_rs_group, L.sub, L.diag, L.sup, L.l, L.rp, L.u, tmpA,
                                                                          U.sub, U.diag, tmpB, U.sup, p->derr);
-        k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB);
+        k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB, above ? p->diagAcc : nullptr);
         p->launches += 2;
     }
-    {
+    if (!sharded) { // (a sharded plan's last level is factored from the gathered records, cn_shard_factorize_finish)
         cn_plan::rs_level &L = p->lv.back();
         k_rs_factor_top_scan<<<1, 32, 0, stream>>>(L.n, L.sub, L.diag, L.sup, p->lw, p->rq, p->uw, p->derr);
         p->launches += 1;
@@ -555,12 +588,45 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
 static cn_status td_scratch(cn_plan *p);
 
 // ---- factorize ----------------------------------------------------------------------------------------
+// the partition the kernels work with (see cn_factorize) and, for a sharded plan, the rows nt of its last RS level
+static void choose_partition(const cn_plan *p, int64_t *Peff, int64_t *nt)
+{
+    const int64_t N = p->N;
+    int64_t P = p->Pu;
+    if (p->opt_path != 1 && !p->opt_keep_p && N % 8 == 0) {
+        const int64_t mu = (N % p->Pu == 0) ? N / p->Pu : 0;
+        const bool fits = mu >= 8 && mu <= 256 && (mu & (mu - 1)) == 0;
+        if (!fits) {
+            int64_t me = 8;
+            while (me < 256 && N % (2 * me) == 0) me *= 2;
+            P = N / me;
+        }
+    }
+    *Peff = P;
+    if (nt) { // levels are added while the shard's system exceeds its share of what one CTA solves (8192 rows in all)
+        int64_t topmax = 8 * CN_RS_TOP_THREADS / p->nshards;
+        if (topmax > p->opt_rs_topmax) topmax = p->opt_rs_topmax;
+        int64_t n = P;
+        while (n > topmax && n > 1) n = (n + CN_RS_G - 1) / CN_RS_G;
+        *nt = n;
+    }
+}
+
+static cn_status factorize_impl(cn_plan *p, cudaStream_t stream, cplx *msend);
+
 extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
 {
     if (!p) return CN_EINVAL;
-    cudaStream_t stream = (cudaStream_t)stream_;
+    if (p->nshards > 1) return CN_EINVAL; // a sharded plan is factored by cn_shard_factorize_local / _finish
+    return factorize_impl(p, (cudaStream_t)stream_, nullptr);
+}
+
+// msend != NULL: sharded plan; everything but the last RS level, whose rows go to the matrix record msend (DEVICE)
+static cn_status factorize_impl(cn_plan *p, cudaStream_t stream, cplx *msend)
+{
     free_factors(p);
     const int64_t N = p->N;
+    const bool sharded = p->nshards > 1;
     // The partition the kernels work with.  psi does not depend on it (direct solver), and the tiled kernels want equal
     // blocks of 8 * 2^k rows: up to 256 rows a block lives inside one warp (shuffle scans only), 512..4096 rows span
     // several warps (shared-memory scans and CTA barriers: 189-235 us per C2 step against 158), more does not fit a
@@ -569,16 +635,7 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     // and the forced-tiled paths partition the system themselves into blocks of the largest 8 * 2^k <= 256 rows that
     // divides N -- the same method one level down.  CN_OPT_KEEP_P = 1 and the generic path
     // (CN_OPT_PATH = 1) take the caller's P literally.
-    p->P = p->Pu;
-    if (p->opt_path != 1 && !p->opt_keep_p && N % 8 == 0) {
-        const int64_t mu = (N % p->Pu == 0) ? N / p->Pu : 0;
-        const bool fits = mu >= 8 && mu <= 256 && (mu & (mu - 1)) == 0;
-        if (!fits) {
-            int64_t me = 8;
-            while (me < 256 && N % (2 * me) == 0) me *= 2;
-            p->P = N / me;
-        }
-    }
+    choose_partition(p, &p->P, sharded ? &p->nt : nullptr);
     const int64_t P = p->P;
 
     // choose the path
@@ -596,6 +653,10 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
         if (p->opt_tile_threads && p->opt_tile_threads < cpb) tiled_ok = false;
     }
     if (p->opt_path == 2 && !tiled_ok) return CN_EINVAL;
+    // sharded: the tiled kernels on blocks inside one warp, resident, warp-per-group RS levels chosen by the library
+    if (sharded && (!tiled_ok || p->opt_path == 1 || logc > 5 || (N / 8) % 32 != 0 || p->hV || p->opt_rs_levels != 0 ||
+                    p->opt_rs_group != CN_RS_G || p->opt_rs_serial_top))
+        return CN_EINVAL;
     p->path = (p->opt_path == 1 || !tiled_ok) ? 1 : 2;
     p->tpb = (p->path == 2) ? tpb : 0;
     p->logc = logc;
@@ -609,19 +670,18 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
     } else {
         if ((st = dev_alloc(p, &p->gamJ, (size_t)P)) != CN_OK) return st;
     }
-    if ((st = dev_alloc(p, &p->slotD, (size_t)P)) != CN_OK) return st;
-    if ((st = dev_alloc(p, &p->slotU, (size_t)P)) != CN_OK) return st;
-    if ((st = dev_alloc(p, &p->sup[0], (size_t)P)) != CN_OK) return st;
-    if ((st = dev_alloc(p, &p->sup[1], (size_t)P)) != CN_OK) return st;
+    if ((st = dev_alloc_g(p, &p->slotD, (size_t)P, sharded)) != CN_OK) return st;
+    if ((st = dev_alloc_g(p, &p->slotU, (size_t)P, sharded)) != CN_OK) return st;
     if ((st = dev_alloc(p, &p->derr, 1)) != CN_OK) return st;
     if (p->path == 1)
         if ((st = dev_alloc(p, &p->work, (size_t)N)) != CN_OK) return st;
-    if (N <= CN_BATCHED_NMAX && !p->ooc)
+    if (N <= CN_BATCHED_NMAX && !p->ooc && !sharded)
         if ((st = dev_alloc(p, &p->qB, (size_t)N)) != CN_OK) return st;
 
     // RS levels: lv[0] has P rows; add levels of ceil(n / G) rows until the last one fits the single CTA
     {
-        const int64_t topmax = (p->opt_rs_levels < 0) ? INT64_MAX : p->opt_rs_topmax;
+        int64_t topmax = (p->opt_rs_levels < 0) ? INT64_MAX : p->opt_rs_topmax;
+        if (sharded && topmax > 8 * CN_RS_TOP_THREADS / p->nshards) topmax = 8 * CN_RS_TOP_THREADS / p->nshards;
         int64_t n = P;
         for (;;) {
             cn_plan::rs_level L;
@@ -629,7 +689,7 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
             p->lv.push_back(L);
             const int nl = (int)p->lv.size();
             const bool want_more = (p->opt_rs_levels > 0) ? (nl < p->opt_rs_levels) : (n > topmax);
-            if (!want_more || n <= 2) break;
+            if (!want_more || n <= (sharded ? 1 : 2)) break;
             n = (n + p->opt_rs_group - 1) / p->opt_rs_group;
         }
         if (p->opt_rs_levels >= 0 && !p->opt_rs_serial_top && p->lv.back().n > 8 * CN_RS_TOP_THREADS) return CN_EINVAL;
@@ -640,7 +700,7 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
         const size_t n = (size_t)L.n;
         if ((st = dev_alloc(p, &L.sub, n)) != CN_OK) return st;
         if ((st = dev_alloc(p, &L.diag, n)) != CN_OK) return st;
-        if ((st = dev_alloc(p, &L.sup, n)) != CN_OK) return st;
+        if ((st = dev_alloc_g(p, &L.sup, n, sharded)) != CN_OK) return st;
         if (i < nlv - 1) {
             if ((st = dev_alloc(p, &L.l, n)) != CN_OK) return st;
             if ((st = dev_alloc(p, &L.rp, n)) != CN_OK) return st;
@@ -651,20 +711,46 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
             L.rU = p->slotU;
         } else {
             if ((st = dev_alloc(p, &L.rD, n)) != CN_OK) return st;
-            if ((st = dev_alloc(p, &L.rU, n)) != CN_OK) return st;
-            if ((st = dev_alloc(p, &L.X, n)) != CN_OK) return st;
+            if ((st = dev_alloc_g(p, &L.rU, n, sharded)) != CN_OK) return st;
+            if (!(sharded && i == nlv - 1)) // (a sharded plan's last level lives in topX[], see below)
+                if ((st = dev_alloc(p, &L.X, n)) != CN_OK) return st;
             CN_CUDA(p, cudaMemsetAsync(L.rU, 0, sizeof(cplx) * n, stream)); // rU[last] stays 0
         }
     }
-    const size_t ntop = (size_t)p->lv.back().n;
+    // last level: its factors; for a sharded plan the whole last level of all shards (nshards * nt rows, replicated)
+    const size_t ntop = sharded ? (size_t)p->nshards * (size_t)p->nt : (size_t)p->lv.back().n;
+    if (sharded && p->lv.back().n != p->nt) return CN_EINVAL; // choose_partition and the loop above must agree
     if ((st = dev_alloc(p, &p->lw, ntop)) != CN_OK) return st;
     if ((st = dev_alloc(p, &p->rq, ntop)) != CN_OK) return st;
     if ((st = dev_alloc(p, &p->uw, ntop)) != CN_OK) return st;
+    if (sharded) {
+        for (int b = 0; b < 2; ++b) {
+            if ((st = dev_alloc(p, &p->topX[b], ntop)) != CN_OK) return st;
+            CN_CUDA(p, cudaMemsetAsync(p->topX[b], 0, sizeof(cplx) * ntop, stream));
+        }
+        if ((st = dev_alloc(p, &p->gsub, ntop)) != CN_OK || (st = dev_alloc(p, &p->gdiag, ntop)) != CN_OK ||
+            (st = dev_alloc(p, &p->gsup, ntop)) != CN_OK || (st = dev_alloc(p, &p->diagAcc, 1)) != CN_OK)
+            return st;
+        CN_CUDA(p, cudaMemsetAsync(p->diagAcc, 0, sizeof(cplx), stream));
+    }
+    // support values on the joint lines, old and new (ping-pong).  Sharded: with one guard element in front (the row
+    // above the shard); when level 0 is the last level they are this shard's window of topX[]
+    const int64_t toff = (int64_t)p->shard * p->nt;
+    for (int b = 0; b < 2; ++b) {
+        if (sharded && nlv == 1) p->sup[b] = p->topX[b] + toff;
+        else if ((st = dev_alloc_g(p, &p->sup[b], (size_t)P, sharded)) != CN_OK) return st;
+    }
 
     // temporaries of the factorization (freed below)
     cplx *red = nullptr;
-    CN_CUDA(p, cudaMalloc((void **)&red, sizeof(cplx) * 6 * (size_t)P));
+    CN_CUDA(p, cudaMalloc((void **)&red, sizeof(cplx) * CN_RED_COUNT(P)));
     if ((st = factor_compute(p, p->dV, red, m, stream)) != CN_OK) { cudaFree(red); return st; }
+    if (sharded) {
+        const cn_plan::rs_level &L = p->lv.back();
+        k_shard_pack_matrix<<<(unsigned)((p->nt + 127) / 128), 128, 0, stream>>>(p->nt, L.sub, L.diag, L.sup, p->diagAcc,
+                                                                             p->above ? 1 : 0, p->shard, msend);
+        p->launches += 1;
+    }
     int herr = 0;
     cudaError_t e = cudaMemcpyAsync(&herr, p->derr, sizeof(int), cudaMemcpyDeviceToHost, stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
@@ -706,6 +792,10 @@ extern "C" cn_status cn_factorize(cn_plan *p, void *stream_)
         CN_CUDA(p, cudaFuncSetAttribute((const void *)k_onchip_steps<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)onchip_smem_bytes<128>()));
         CN_CUDA(p, cudaFuncSetAttribute((const void *)k_onchip_steps<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)onchip_smem_bytes<256>()));
         CN_CUDA(p, cudaFuncSetAttribute((const void *)k_onchip_steps<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)onchip_smem_bytes<512>()));
+    }
+    if (sharded) { // the last level is still to come (cn_shard_factorize_finish)
+        p->sh_local_done = true;
+        return CN_OK;
     }
     p->factorized = true;
     return td_scratch(p);
@@ -784,6 +874,15 @@ static cn_status launch_pass(cn_plan *p, cplx *psi, int mode, int cur, cudaStrea
         prm.slotD = p->slotD;
         prm.slotU = p->slotU;
         prm.supInit = p->sup[0];
+        if (p->above) {
+            // a shard with a predecessor: its blocks are numbered from 1, so that "the joint line above block w" is
+            // index w - 1 >= 0 for every block -- for the first one the guard element in front of the arrays, which
+            // holds what belongs to the last row of the preceding shard (the same mechanism as a streamed part)
+            prm.chunk0 = (int64_t)1 << p->logc;
+            prm.supOld -= 1; prm.supNew -= 1; prm.slotD -= 1; prm.slotU -= 1; prm.supInit -= 1;
+            prm.P += 1;
+        }
+        if (p->below) prm.P = 0; // the last block of this shard is not the last block of the system
         tiled_kernel_t k = tiled_kernel(p->tpb, p->logc, mode);
         e = launch_k(k, (unsigned)p->grid_tiled, (unsigned)p->tpb, tiled_smem(p->tpb), stream, pdl, p->tmPsi, p->tmQ,
                      p->tmGam, prm);
@@ -811,20 +910,27 @@ static cudaError_t launch_top_k(cn_plan *p, const cn_plan::rs_level &L, cplx *X,
 }
 
 // RS of one step: (RD+RU+JD+JU) level by level, RS of the last level, SS level by level (Eq. 6)
-static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
+// Sharded plans (cn_shard.cuh) run it in two halves around the exchange: phase 1 = the reductions and the record `rec`
+// to send, phase 2 = the replicated last level from the gathered records `rec`, then the substitutions.
+static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase = 0, cplx *rec = nullptr)
 {
     const bool pdl = p->opt_pdl && !p->opt_profile;
     const int nlv = (int)p->lv.size();
     const int pi = prof_begin(p, 1, stream);
     cudaError_t e = cudaSuccess;
+    const bool sharded = p->nshards > 1;
+    const int above = p->above ? 1 : 0;
+    const int64_t toff = (int64_t)p->shard * p->nt;
     p->lv[0].X = p->sup[out];
+    if (sharded) p->lv.back().X = p->topX[out] + toff; // (nlv == 1: sup[out] is that window already)
+    const cplx *Xabove = (sharded && above) ? p->topX[out] + toff - 1 : nullptr;
     const int nsep = nlv - 1; // group levels: one reduce and one substitute kernel each
     const bool tg = p->opt_rs_group != CN_RS_G; // one thread per group of any size (paper-shaped, cn_reduced.cuh)
     // the last level is solved inside the substitution kernel of the level below it (one launch less per step)
-    const bool tis = !tg && p->opt_rs_top_in_subst && p->opt_rs_levels >= 0 && !p->opt_rs_serial_top &&
+    const bool tis = !tg && !sharded && p->opt_rs_top_in_subst && p->opt_rs_levels >= 0 && !p->opt_rs_serial_top &&
                      nlv >= 2 && p->lv.back().n <= p->opt_rs_top_in_subst_max;
     const int64_t G = p->opt_rs_group;
-    for (int i = 0; i < nsep && e == cudaSuccess; ++i) {
+    for (int i = 0; i < nsep && e == cudaSuccess && phase != 2; ++i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
         if (tg)
             e = launch_k(k_rs_reduce_thread, (unsigned)((U.n + 63) / 64), 64u, 0, stream, pdl, L.n, G, (const cplx *)L.rD,
@@ -833,10 +939,42 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
         else
         e = launch_k(k_rs_reduce, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
                      (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
-                     (const cplx *)L.sup, U.rD, U.rU);
+                     (const cplx *)L.sup, U.rD, U.rU, above);
         p->launches += 1;
     }
-    if (e == cudaSuccess && !tis) {
+    if (sharded && phase == 1 && e == cudaSuccess) { // the record of this step: JU guards of all levels + last-level rhs
+        cn_shard_guards gs;
+        gs.n = nlv;
+        for (int i = 0; i < nlv; ++i) gs.g[i] = p->lv[i].rU - 1;
+        const cn_plan::rs_level &L = p->lv.back();
+        e = launch_k(k_shard_pack_step, (unsigned)((p->nt + 127) / 128), 128u, 0, stream, pdl, p->nt, (const cplx *)L.rD,
+                     (const cplx *)L.rU, gs, above, rec);
+        p->launches += 1;
+    }
+    if (phase == 1) {
+        prof_end(p, pi, stream);
+        return e == cudaSuccess ? CN_OK : cuda_fail(p, e);
+    }
+    if (sharded && e == cudaSuccess) {
+        // RS of the whole last level, replicated; launched WITHOUT programmatic serialization: the kernel before it on
+        // the stream is the caller's exchange, which must be complete
+        const int64_t n = (int64_t)p->nshards * p->nt;
+        cplx *guard0 = (above && nlv >= 2) ? p->sup[out] - 1 : nullptr;
+        int T = CN_RS_TOP_THREADS;
+#define CN_STOP(K)                                                                                                     \
+    {                                                                                                                  \
+        while (T > 32 && (int64_t)(T / 2) * K >= n) T /= 2;                                                            \
+        e = launch_k(k_shard_top<K>, 1u, (unsigned)T, 0, stream, false, (int64_t)p->nshards, p->nt, (const cplx *)rec, \
+                     (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw, p->topX[out], toff, guard0);       \
+    }
+        if (n <= CN_RS_TOP_THREADS) CN_STOP(1)
+        else if (n <= 2 * CN_RS_TOP_THREADS) CN_STOP(2)
+        else if (n <= 4 * CN_RS_TOP_THREADS) CN_STOP(4)
+        else CN_STOP(8)
+#undef CN_STOP
+        p->launches += 1;
+    }
+    if (e == cudaSuccess && !tis && !sharded) {
         const cn_plan::rs_level &L = p->lv.back();
         if (p->opt_rs_levels < 0 || p->opt_rs_serial_top)
             e = launch_k(k_rs_serial, 1u, 32u, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU,
@@ -858,7 +996,8 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream)
             const int kt = (tis && i == nlv - 2) ? (U.n <= T ? 1 : (U.n <= 2 * T ? 2 : (U.n <= 4 * T ? 4 : 8))) : 0;
 #define CN_SUBST(KT) launch_k(k_rs_subst<KT>, gr, 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU, \
                               (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X, U.n,                 \
-                              (const cplx *)U.rD, (const cplx *)U.rU, (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw)
+                              (const cplx *)U.rD, (const cplx *)U.rU, (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw, \
+                              Xabove)
             e = kt == 0 ? CN_SUBST(0) : (kt == 1 ? CN_SUBST(1) : (kt == 2 ? CN_SUBST(2) : (kt == 4 ? CN_SUBST(4) : CN_SUBST(8))));
 #undef CN_SUBST
         }
@@ -1007,7 +1146,7 @@ static cn_status td_scratch(cn_plan *p)
     if (p->tdRed) cudaFree(p->tdRed);
     p->tdRed = nullptr;
     p->tdRedP = 0;
-    CN_CUDA(p, cudaMalloc((void **)&p->tdRed, sizeof(cplx) * 6 * (size_t)p->P));
+    CN_CUDA(p, cudaMalloc((void **)&p->tdRed, sizeof(cplx) * CN_RED_COUNT(p->P)));
     p->tdRedP = p->P;
     return CN_OK;
 }
@@ -1395,4 +1534,140 @@ extern "C" cn_status cn_batched_sweep(cn_plan *p, void *psi_, int64_t nsys, int6
     }
     if (e != cudaSuccess) return cuda_fail(p, e);
     return CN_OK;
+}
+
+// ---- sharded mode (kernels and record layout in cn_shard.cuh) ------
+extern "C" cn_status cn_shard_plan_create(cn_plan **out, int64_t N_local, int64_t P_local, double dx, double dt,
+                                          const double *V_local, int32_t shard, int32_t nshards)
+{
+    if (!out) return CN_EINVAL;
+    *out = nullptr;
+    if (nshards < 1 || nshards > 1024 || shard < 0 || shard >= nshards) return CN_EINVAL;
+    if (N_local % 256 != 0 || N_local < 256) return CN_EINVAL; // whole warps of 8-row chunks (tiled kernels only)
+    cn_status st = cn_plan_create(out, N_local, P_local, dx, dt, V_local);
+    if (st != CN_OK) return st;
+    cn_plan *p = *out;
+    p->shard = shard;
+    p->nshards = nshards;
+    p->above = shard > 0;
+    p->below = shard < nshards - 1;
+    return CN_OK;
+}
+
+extern "C" cn_status cn_shard_counts(const cn_plan *p, int64_t *matrix_count, int64_t *step_count)
+{
+    if (!p || !matrix_count || !step_count) return CN_EINVAL;
+    int64_t Peff = 0, nt = 0;
+    choose_partition(p, &Peff, &nt);
+    *matrix_count = CN_SHARD_MREC(nt);
+    *step_count = nt + 1;
+    return CN_OK;
+}
+
+extern "C" cn_status cn_shard_factorize_local(cn_plan *p, void *matrix_send, void *stream_)
+{
+    if (!p || !matrix_send || (((uintptr_t)matrix_send) & 15) != 0) return CN_EINVAL;
+    if (p->nshards == 1) { // one shard is the whole system: nothing to exchange, the record stays unused
+        cn_status st = factorize_impl(p, (cudaStream_t)stream_, nullptr);
+        if (st == CN_OK) p->sh_local_done = true;
+        return st;
+    }
+    return factorize_impl(p, (cudaStream_t)stream_, (cplx *)matrix_send);
+}
+
+extern "C" cn_status cn_shard_factorize_finish(cn_plan *p, const void *matrix_all, void *stream_)
+{
+    if (!p || !p->sh_local_done) return CN_EINVAL;
+    if (p->nshards == 1) return CN_OK;
+    if (!matrix_all || (((uintptr_t)matrix_all) & 15) != 0) return CN_EINVAL;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int64_t n = (int64_t)p->nshards * p->nt;
+    CN_CUDA(p, cudaMemsetAsync(p->derr, 0, sizeof(int), stream));
+    k_shard_assemble_top<<<(unsigned)((n + 127) / 128), 128, 0, stream>>>((int64_t)p->nshards, p->nt, (const cplx *)matrix_all,
+                                                                         p->gsub, p->gdiag, p->gsup, p->derr);
+    k_rs_factor_top_scan<<<1, 32, 0, stream>>>(n, p->gsub, p->gdiag, p->gsup, p->lw, p->rq, p->uw, p->derr);
+    p->launches += 2;
+    int herr = 0;
+    CN_CUDA(p, cudaMemcpyAsync(&herr, p->derr, sizeof(int), cudaMemcpyDeviceToHost, stream));
+    CN_CUDA(p, cudaStreamSynchronize(stream));
+    if (herr >= 2) return CN_EINVAL; // records of shards with another shape, or not in rank order
+    if (herr) return CN_EBREAKDOWN;
+    p->factorized = true;
+    return CN_OK;
+}
+
+extern "C" cn_status cn_shard_edge(cn_plan *p, const void *psi, void *edge_send, void *stream_)
+{
+    if (!p || !psi || !edge_send) return CN_EINVAL;
+    CN_CUDA(p, cudaMemcpyAsync(edge_send, (const cplx *)psi + (p->N - 1), sizeof(cplx), cudaMemcpyDeviceToDevice,
+                               (cudaStream_t)stream_));
+    return CN_OK;
+}
+
+static cn_status shard_map_psi(cn_plan *p, void *psi_)
+{
+    if (p->tmPsiFor == psi_) return CN_OK;
+    const int box_rows = p->tpb < 256 ? p->tpb : 256;
+    cn_status st = make_map(p, &p->tmPsi, psi_, 16, box_rows);
+    if (st == CN_OK) p->tmPsiFor = psi_;
+    return st;
+}
+
+extern "C" cn_status cn_shard_prologue(cn_plan *p, void *psi_, const void *edges_all, void *step_send, void *stream_)
+{
+    if (!p || !psi_ || (((uintptr_t)psi_) & 15) != 0) return CN_EINVAL;
+    if (!p->factorized) return CN_ENOTFACTORIZED;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    cn_status st;
+    if (p->nshards == 1) { // degenerate: behaves like the first third of cn_step
+        if ((st = shard_map_psi(p, psi_)) != CN_OK) return st;
+        if ((st = launch_pass(p, (cplx *)psi_, 0, 1, stream)) != CN_OK) return st;
+        p->sh_out = 1;
+        return CN_OK;
+    }
+    if (!step_send || (p->above && !edges_all)) return CN_EINVAL;
+    if ((st = shard_map_psi(p, psi_)) != CN_OK) return st;
+    if (p->above) // psi^0 on the last row of the preceding shard: the old value of "the joint line above" for block 0
+        CN_CUDA(p, cudaMemcpyAsync(p->sup[0] - 1, (const cplx *)edges_all + (p->shard - 1), sizeof(cplx),
+                                   cudaMemcpyDeviceToDevice, stream));
+    if ((st = launch_pass(p, (cplx *)psi_, 0, /*cur=*/1, stream)) != CN_OK) return st;
+    p->sh_out = 1;
+    return launch_rs(p, p->sh_out, stream, 1, (cplx *)step_send);
+}
+
+extern "C" cn_status cn_shard_advance(cn_plan *p, void *psi_, const void *step_all, void *step_send, void *stream_)
+{
+    if (!p || !psi_) return CN_EINVAL;
+    if (!p->factorized) return CN_ENOTFACTORIZED;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    cn_status st;
+    if (p->tmPsiFor != psi_) return CN_EINVAL; // cn_shard_prologue starts a run on this vector
+    if (p->nshards == 1) {
+        if ((st = launch_rs(p, p->sh_out, stream)) != CN_OK) return st;
+        const int cur = p->sh_out;
+        p->sh_out = cur ^ 1;
+        return launch_pass(p, (cplx *)psi_, 1, cur, stream);
+    }
+    if (!step_all || !step_send) return CN_EINVAL;
+    if ((st = launch_rs(p, p->sh_out, stream, 2, (cplx *)step_all)) != CN_OK) return st;
+    const int cur = p->sh_out;
+    if ((st = launch_pass(p, (cplx *)psi_, 1, cur, stream)) != CN_OK) return st;
+    p->sh_out = cur ^ 1;
+    return launch_rs(p, p->sh_out, stream, 1, (cplx *)step_send);
+}
+
+extern "C" cn_status cn_shard_epilogue(cn_plan *p, void *psi_, const void *step_all, void *stream_)
+{
+    if (!p || !psi_) return CN_EINVAL;
+    if (!p->factorized) return CN_ENOTFACTORIZED;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    cn_status st;
+    if (p->tmPsiFor != psi_) return CN_EINVAL;
+    if (p->nshards == 1) {
+        if ((st = launch_rs(p, p->sh_out, stream)) != CN_OK) return st;
+    } else {
+        if (!step_all) return CN_EINVAL;
+        if ((st = launch_rs(p, p->sh_out, stream, 2, (cplx *)step_all)) != CN_OK) return st;
+    }
+    return launch_pass(p, (cplx *)psi_, 2, p->sh_out, stream);
 }

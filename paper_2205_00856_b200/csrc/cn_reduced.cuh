@@ -199,8 +199,9 @@ CN_DEVINL void rs_load_rows_n(const cplx *const (&src)[NA], const int (&lim)[NA]
 __global__ void __launch_bounds__(32 * CN_RS_WARPS)
 k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
             const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ sub,
-            const cplx *__restrict__ sup, cplx *__restrict__ outD, cplx *__restrict__ outU)
-{
+            const cplx *__restrict__ sup, cplx *__restrict__ outD, cplx *__restrict__ outU, int above = 0)
+{   // above: the rows of a shard that another shard precedes (cn_shard.cuh): group 0 has a real joint line above it,
+    // whose coupling sup[-1] and slot outU[-1] are the guard elements of the arrays
     constexpr int K = CN_RS_K;
     const int lane = threadIdx.x & 31;
     const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
@@ -222,7 +223,7 @@ k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
     cplx subJ = zero, supAbove = zero;
     if (live && lane == 0) {
         subJ = sub[g0 + ng - 1];
-        if (g > 0) supAbove = sup[g0 - 1];
+        if (g > 0 || above) supAbove = sup[g0 - 1];
     }
     pdl_wait();
     {
@@ -277,7 +278,7 @@ k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
     yN = shfl_c(yN, ng > 1 ? (ng - 2) / K : 0);
     if (live && lane == 0) {
         outD[g] = (ng >= 2) ? cfnma(subJ, yN, Rj) : Rj;                        // JD
-        if (g > 0) outU[g - 1] = (ng >= 2) ? cneg(cmul(supAbove, y0)) : zero; // JU
+        if (g > 0 || above) outU[g - 1] = (ng >= 2) ? cneg(cmul(supAbove, y0)) : zero; // JU
     }
 }
 
@@ -290,8 +291,8 @@ __global__ void __launch_bounds__(32 * CN_RS_WARPS)
 k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
            const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ Xup,
            cplx *__restrict__ X, int64_t ntop, const cplx *topD, const cplx *topU, const cplx *__restrict__ lw,
-           const cplx *__restrict__ rq, const cplx *__restrict__ uw)
-{
+           const cplx *__restrict__ rq, const cplx *__restrict__ uw, const cplx *Xabove = nullptr)
+{   // Xabove (KT == 0 only): support value of the joint line above group 0 when a shard precedes this one (cn_shard.cuh)
     constexpr int K = CN_RS_K;
     const int lane = threadIdx.x & 31;
     const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
@@ -375,6 +376,7 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
         pdl_wait();
         if (live) {
             if (g > 0) XL = ld_dep(Xup + g - 1);
+            else if (Xabove) XL = ld_dep(Xabove);
             XJ = ld_dep(Xup + g);
         }
         pdl_launch_dependents();
@@ -476,10 +478,16 @@ __global__ void k_rs_assemble0(int64_t P, int64_t N, double rho, const double *_
                                const double *__restrict__ gamJ,
                                const cplx *__restrict__ redSubD, const cplx *__restrict__ redDiagD,
                                const cplx *__restrict__ redSupU, const cplx *__restrict__ redDiagU,
-                               cplx *__restrict__ sub, cplx *__restrict__ diag, cplx *__restrict__ sup)
-{
+                               cplx *__restrict__ sub, cplx *__restrict__ diag, cplx *__restrict__ sup,
+                               int above = 0, cplx *__restrict__ diagAboveAcc = nullptr)
+{   // above (cn_shard.cuh): row 0 keeps its coupling to the last row of the preceding shard; that row's coupling to row 0
+    // goes to the guard sup[-1] and the diagonal term this shard's first block adds to it opens the sum *diagAboveAcc
     int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= P) return;
+    if (above && w == 0) {
+        sup[-1] = redSupU[-1];
+        *diagAboveAcc = redDiagU[-1];
+    }
     const int64_t J = ((N % P == 0) ? (w + 1) * (N / P) : (int64_t)(((__int128)(w + 1) * N) / P)) - 1;
     const double gJ = gamJ ? gamJ[w] : gam[J];
     cplx d = cmake(-gJ + redDiagD[w].x, rho + redDiagD[w].y);
@@ -488,7 +496,7 @@ __global__ void k_rs_assemble0(int64_t P, int64_t N, double rho, const double *_
         d = cadd(d, redDiagU[w]);
         s = redSupU[w];
     }
-    sub[w] = (w > 0) ? redSubD[w] : cmake(0.0, 0.0);
+    sub[w] = (w > 0 || above) ? redSubD[w] : cmake(0.0, 0.0);
     diag[w] = d;
     sup[w] = s;
 }
@@ -559,8 +567,8 @@ __global__ void __launch_bounds__(32 * CN_RS_FL_WARPS)
 k_rs_factor_level_smem(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
                        const cplx *__restrict__ sup, cplx *__restrict__ l, cplx *__restrict__ rp, cplx *__restrict__ u,
                        cplx *__restrict__ sub2, cplx *__restrict__ diag2, cplx *__restrict__ diag2U,
-                       cplx *__restrict__ sup2, int *__restrict__ err)
-{
+                       cplx *__restrict__ sup2, int *__restrict__ err, int above = 0)
+{   // above (cn_shard.cuh): group 0 is treated like any later group; its JU matrix side goes to the guards [-1]
     __shared__ cplx sm[CN_RS_FL_WARPS][4][CN_RS_G]; // sub -> l, diag -> rp, sup -> u, tmp
     const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
     const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
@@ -608,9 +616,9 @@ k_rs_factor_level_smem(int64_t n, const cplx *__restrict__ sub, const cplx *__re
                 beLast = be;
             }
         }
-        sub2[g] = (g == 0) ? zero : (has ? cmul(subJ, alLast) : subJ);
+        sub2[g] = (g == 0 && !above) ? zero : (has ? cmul(subJ, alLast) : subJ);
         diag2[g] = has ? cfma(subJ, beLast, diagJ) : diagJ;
-        if (g > 0) {
+        if (g > 0 || above) {
             const cplx sa = sup[g0 - 1];
             diag2U[g - 1] = has ? cmul(sa, al) : zero;
             sup2[g - 1] = has ? cmul(sa, be) : sa;
@@ -676,13 +684,16 @@ k_rs_factor_top_scan(int64_t n, const cplx *__restrict__ sub, const cplx *__rest
         rqprev = r;
         supprev = si;
     }
-    if (bad) atomicExch(err, 1);
+    if (bad) atomicMax(err, 1); // (max: keeps the 2 of k_shard_assemble_top)
 }
 
 // diag += diagU (the two-writer accumulation of the next level's diagonal)
-__global__ void k_rs_add(int64_t n, cplx *__restrict__ diag, const cplx *__restrict__ diagU)
+// (diagAboveAcc: a shard with a predecessor also sums what its first groups add to the diagonal of the row above it)
+__global__ void k_rs_add(int64_t n, cplx *__restrict__ diag, const cplx *__restrict__ diagU,
+                         cplx *__restrict__ diagAboveAcc = nullptr)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) diag[i] = cadd(diag[i], diagU[i]);
+    if (i == 0 && diagAboveAcc) *diagAboveAcc = cadd(*diagAboveAcc, diagU[-1]);
 }
 
