@@ -259,6 +259,41 @@ def run_tridiag(torch, peak, N=1 << 24):
             "bytes_per_row": 176, "GBps": gbs, "hbm_frac_measured_peak": gbs / peak, "create_ms": fms}
 
 
+def run_shards(torch, peak, name="C2dense", S=8, nsteps=50, **opts):
+    """Sharded mode (cn_shard_*, row f-4) on ONE device: the S shards of one system stepped in-process, their records
+    "gathered" by concatenation (sharded.LocalShards).  The shards' kernels run one after the other on the one GPU,
+    so this is NOT a scaling figure: it measures what the sharded protocol adds per step in kernel time and launches
+    (S x (pack + last-level solve + one launch more on the RS chain), smaller tiles per launch) over the unsharded
+    plan on the same rows.  The network leg of a real job (one all-gather of step_count values per shard) is absent."""
+    from . import sharded as SH
+    cfg = W.CONFIGS[name]
+    V, psi = _inputs(cfg)
+    n = cfg.N // S
+    plans = [B.ShardPlan(n, max(1, n // 256), cfg.dx, cfg.dt, V[r * n:(r + 1) * n], r, S, **opts) for r in range(S)]
+    grp = SH.LocalShards(plans, lambda c: torch.zeros(c, dtype=torch.complex128, device="cuda"), torch.cat)
+    grp.factorize()
+    parts = [torch.from_numpy(psi[r * n:(r + 1) * n].copy()).cuda() for r in range(S)]
+    grp.step(parts, 3)
+    torch.cuda.synchronize()
+    ms = []
+    for _ in range(3):
+        e0, e1 = _events(torch)
+        e0.record()
+        grp.step(parts, nsteps)
+        e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1) / nsteps)
+    counts = plans[0].counts()
+    launches = sum(p.info()["launches"] for p in plans)
+    for p in plans:
+        p.close()
+    best = min(ms)
+    return {"config": name + " sharded in-process", "N": cfg.N, "shards": S, "N_local": n, "record_values_per_step": counts[1],
+            "record_values_matrix": counts[0], "us_per_cn_step_all_shards_serialised": 1e3 * best,
+            "us_per_cn_step_per_shard": 1e3 * best / S, "Gpoint_steps_per_s_one_device": cfg.N / best / 1e6,
+            "launches_total": launches}
+
+
 def levels_study(torch, N=300000):
     """Nested multi-iteration study (Eq. 8-9, Fig. 2) with the paper-shaped kernels:
     one thread per block, one thread per group at every nested level, serial last level.  n_it = number of
@@ -331,6 +366,9 @@ def main(argv=None):
             emit(run_td(torch, peak))
         elif name == "TRI":
             emit(run_tridiag(torch, peak))
+        elif name == "SHARD":
+            for S, opts in ((1, {}), (2, {}), (8, {}), (8, {"rs_topmax": 1})):
+                emit(dict(run_shards(torch, peak, S=S, **opts), options=opts))
     if args.sweep:
         emit(p_sweep(torch, peak))
     if args.levels:
