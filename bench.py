@@ -216,6 +216,12 @@ def per_config_report(torch, peak, full, with_cpu):
         tri["cpu_baseline"] = cpu(n / (time.time() - t0) / 1e9, "Grows/s", 1, "one Thomas solve of 2^22 rows of the same distribution")
     out["TRI"] = tri
 
+    # ---- many systems with a potential of their own each at C4's shape (row f-3) ---------------------------------------
+    r = RP.run_systems(torch, peak)
+    out["C4V"] = {"workload": "C4 shape (8192 x 8192), non-separable V(x, y): every line of a sweep has its own matrix",
+                  "bytes_per_point_sweep": 56, "contiguous": r["contiguous"], "interleaved": r["interleaved"],
+                  "frac": r["contiguous"]["hbm_frac_measured_peak"]}
+
     if full:
         # ---- C3: 2^30 points resident (psi 17 GB + factors 26 GB) -----------------------------------------------------
         cfg = W.CONFIGS["C3"]

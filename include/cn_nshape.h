@@ -162,6 +162,24 @@ cn_status cn_step_td(cn_plan *plan, void *psi, int64_t nsteps, const double *fie
 cn_status cn_batched_sweep(cn_plan *plan, void *psi, int64_t nsys, int64_t elem_stride, int64_t sys_stride,
                            int64_t nsteps, void *stream);
 
+/*
+ * Many systems with a potential of their own each (operator splitting turns an N-D
+ * problem into series of 1-D problems, and with a non-separable V(x, y) every line of a sweep has its own matrix).
+ *   cn_plan_set_systems : declares, before cn_factorize, that the plan's N rows (its V, and psi alike) are `nsys`
+ *       independent systems of N / nsys rows with Dirichlet ends each; row j of system k lives at
+ *       [k * sys_stride + j * elem_stride].  Dense layouts only: contiguous systems (elem_stride = 1, sys_stride =
+ *       N / nsys) or interleaved systems (elem_stride = nsys, sys_stride = 1).  cn_factorize then stores per-point
+ *       factors of every system.  Contiguous systems of 8 * 2^k rows run on the tiled kernels of cn_step -- a system
+ *       boundary is a joint line above which "psi = 0", like the top of a single system, so the whole array is one
+ *       fused pass: 56 B per point and step (psi 16 + q 16 + gamma 8 in, psi 16 out; 32 B in cn_batched_sweep, whose
+ *       systems share one matrix that stays on chip), SS(k) fused with RD/RU(k+1) over the steps of a call.
+ *       Any other dense layout runs on one thread per system (correctness path).
+ *   cn_batched_sweep_v  : nsteps CN steps of all systems in place (the same call as cn_step on such a plan).
+ * Not available for out-of-core, sharded or time-dependent use (CN_EINVAL); cn_batched_sweep refuses such a plan.
+ */
+cn_status cn_plan_set_systems(cn_plan *plan, int64_t nsys, int64_t elem_stride, int64_t sys_stride);
+cn_status cn_batched_sweep_v(cn_plan *plan, void *psi, int64_t nsteps, void *stream);
+
 cn_status cn_destroy(cn_plan *plan);
 
 cn_status cn_plan_get_info(const cn_plan *plan, cn_plan_info *info);
@@ -185,9 +203,18 @@ const char *cn_version(void);
  *                       CN_EBREAKDOWN if a zero or non-finite pivot is met; diagonally dominant matrices are safe.
  *   cn_tridiag_solve  : d, x = N complex128 DEVICE vectors (x may alias d); asynchronous on `stream`, no allocation.
  *   cn_tridiag_destroy: frees everything.
+ *   cn_tridiag_create_blocks : the same with CALLER-PLACED joint lines ("the blocks may differ in
+ *                       size"): joints = P strictly increasing HOST row indices (0-based), joints[P-1] = N - 1; block w =
+ *                       rows (joints[w-1], joints[w]], its last row is its joint line, blocks of one row (joint line
+ *                       only) and two rows allowed.  The ragged first level runs on one thread per block straight in
+ *                       global memory -- the shape of the paper's own kernels -- and the reduced
+ *                       system on the P joint lines on the nested warp-per-group levels.  CN_EINVAL for joints that
+ *                       are not increasing or do not end at N - 1.  The solution does not depend on the joints.
  */
 typedef struct cn_tridiag cn_tridiag;
 cn_status cn_tridiag_create(cn_tridiag **out, int64_t N, const void *b, const void *a, const void *c, void *stream);
+cn_status cn_tridiag_create_blocks(cn_tridiag **out, int64_t N, const void *b, const void *a, const void *c, int64_t P,
+                                   const int64_t *joints, void *stream);
 cn_status cn_tridiag_solve(cn_tridiag *t, const void *d, void *x, void *stream);
 cn_status cn_tridiag_destroy(cn_tridiag *t);
 

@@ -22,6 +22,7 @@ EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", 
            "cn_batched_sweep", "cn_destroy", "cn_plan_get_info", "cn_plan_get_profile", "cn_status_string",
            "cn_last_cuda_error", "cn_version", "cn_plan_set_td_shape", "cn_step_td",
            "cn_tridiag_create", "cn_tridiag_solve", "cn_tridiag_destroy",
+           "cn_tridiag_create_blocks", "cn_plan_set_systems", "cn_batched_sweep_v",
            "cn_shard_plan_create", "cn_shard_counts", "cn_shard_factorize_local", "cn_shard_factorize_finish",
            "cn_shard_edge", "cn_shard_prologue", "cn_shard_advance", "cn_shard_epilogue"]
 
@@ -69,6 +70,12 @@ def lib():
         L.cn_step_td.argtypes = [vp, vp, i64, vp, vp]
         L.cn_tridiag_create.restype = i32
         L.cn_tridiag_create.argtypes = [ctypes.POINTER(vp), i64, vp, vp, vp, vp]
+        L.cn_tridiag_create_blocks.restype = i32
+        L.cn_tridiag_create_blocks.argtypes = [ctypes.POINTER(vp), i64, vp, vp, vp, i64, vp, vp]
+        L.cn_plan_set_systems.restype = i32
+        L.cn_plan_set_systems.argtypes = [vp, i64, i64, i64]
+        L.cn_batched_sweep_v.restype = i32
+        L.cn_batched_sweep_v.argtypes = [vp, vp, i64, vp]
         L.cn_tridiag_solve.restype = i32
         L.cn_tridiag_solve.argtypes = [vp, vp, vp, vp]
         L.cn_tridiag_destroy.restype = i32
@@ -173,6 +180,14 @@ def cn_batched_sweep(plan, psi, nsys: int, elem_stride: int, sys_stride: int, ns
            "cn_batched_sweep")
 
 
+def cn_plan_set_systems(plan, nsys: int, elem_stride: int, sys_stride: int):
+    _check(plan, lib().cn_plan_set_systems(plan, nsys, elem_stride, sys_stride), "cn_plan_set_systems")
+
+
+def cn_batched_sweep_v(plan, psi, nsteps: int = 1, stream=None):
+    _check(plan, lib().cn_batched_sweep_v(plan, _ptr(psi), nsteps, _stream(stream)), "cn_batched_sweep_v")
+
+
 def cn_destroy(plan):
     _check(None, lib().cn_destroy(plan), "cn_destroy")
 
@@ -196,10 +211,16 @@ def cn_version() -> str:
 class Tridiag:
     """General complex tridiagonal system (cn_tridiag_*): marshalling only."""
 
-    def __init__(self, b, a, c, stream=None):
+    def __init__(self, b, a, c, stream=None, joints=None):
+        """joints: optional caller-placed joint lines (increasing 0-based row indices, the last one N - 1)."""
         n = int(a.shape[0])
         h = ctypes.c_void_p()
-        st = lib().cn_tridiag_create(ctypes.byref(h), n, _ptr(b), _ptr(a), _ptr(c), _stream(stream))
+        if joints is None:
+            st = lib().cn_tridiag_create(ctypes.byref(h), n, _ptr(b), _ptr(a), _ptr(c), _stream(stream))
+        else:
+            J = (ctypes.c_int64 * len(joints))(*[int(j) for j in joints])
+            st = lib().cn_tridiag_create_blocks(ctypes.byref(h), n, _ptr(b), _ptr(a), _ptr(c), len(joints),
+                                                ctypes.cast(J, ctypes.c_void_p), _stream(stream))
         if st != CN_OK:
             raise CnError(st, "cn_tridiag_create")
         self.h, self.N = h, n
@@ -321,6 +342,13 @@ class Plan:
 
     def batched_sweep(self, psi, nsys, elem_stride, sys_stride, nsteps=1, stream=None):
         cn_batched_sweep(self.h, psi, nsys, elem_stride, sys_stride, nsteps, stream)
+
+    def set_systems(self, nsys, elem_stride, sys_stride):
+        cn_plan_set_systems(self.h, nsys, elem_stride, sys_stride)
+        return self
+
+    def batched_sweep_v(self, psi, nsteps=1, stream=None):
+        cn_batched_sweep_v(self.h, psi, nsteps, stream)
 
     def info(self):
         return cn_plan_get_info(self.h)

@@ -61,6 +61,9 @@ struct cn_plan {
         cplx *rD = nullptr, *rU = nullptr, *X = nullptr;      // two rhs slots per row, solution (levels >= 1)
     };
     std::vector<rs_level> lv;
+    int64_t *off0 = nullptr; // caller-placed joint lines of level 0 (cn_tridiag_create_blocks): group g = rows [off0[g], off0[g+1])
+    int64_t noff0 = 0;       // number of such groups
+    cplx *scratch0 = nullptr; // their reduction's scratch (the solution vector may alias the right-hand side)
     // configuration
     int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
     int opt_pdl = 1, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0, opt_rs_top_in_subst = 1, opt_keep_p = 0;
@@ -70,6 +73,10 @@ struct cn_plan {
     double *tdG = nullptr, *tdV = nullptr;
     cplx *tdRed = nullptr;
     int64_t tdRedP = 0;
+    // many systems with a potential of their own each (cn_plan_set_systems): the plan's N rows are nsys systems
+    int sysMode = 0;        // 0 one system; 1 contiguous systems on the tiled kernels (cuts, cn_pass_tiled.cuh); 2 generic
+    int sysWant = 0;        // what cn_plan_set_systems asked for (cn_factorize settles sysMode)
+    int64_t sysN = 0, sysCount = 0, sysEs = 0, sysSs = 0; // rows per system, systems, strides (complex elements)
     // sharded mode (cn_shard_*; cn_shard.cuh): this plan holds rows of ONE system that nshards processes share
     int shard = 0, nshards = 1;
     bool above = false, below = false; // a shard precedes / follows this one
@@ -156,6 +163,8 @@ static void free_factors(cn_plan *p)
     p->slotD = p->slotU = nullptr; p->sup[0] = p->sup[1] = nullptr; p->work = nullptr; p->derr = nullptr;
     p->qB = nullptr;
     p->gamJ = nullptr;
+    p->off0 = nullptr;
+    p->scratch0 = nullptr;
     p->topX[0] = p->topX[1] = nullptr; p->gsub = p->gdiag = p->gsup = nullptr; p->diagAcc = nullptr;
     p->sh_local_done = false;
     for (int b = 0; b < cn_plan::NB; ++b) { p->bPsi[b] = nullptr; p->bQ[b] = nullptr; p->bV[b] = nullptr; }
@@ -321,7 +330,7 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
 // the whole system is stepped on chip by one CTA (cn_onchip.cuh) when nothing asks for a particular kernel family
 static bool onchip_active(const cn_plan *p)
 {
-    return p->opt_onchip && p->opt_path == 0 && p->opt_rs_levels == 0 && !p->opt_profile && !p->ooc && p->qB &&
+    return p->opt_onchip && p->opt_path == 0 && p->opt_rs_levels == 0 && !p->opt_profile && !p->ooc && p->qB && !p->sysMode &&
            p->N <= CN_ONCHIP_NMAX;
 }
 
@@ -508,6 +517,7 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
     cplx *tmpA = red + 4 * Pg + 1, *tmpB = red + 5 * Pg + 1;
     const int above = p->above ? 1 : 0;
     const bool sharded = p->nshards > 1;
+    const int64_t cutMask = (p->sysMode == 1) ? p->sysN / m - 1 : ~(int64_t)0; // blocks per system - 1 (a power of two)
     CN_CUDA(p, cudaMemsetAsync(red, 0, sizeof(cplx) * CN_RED_COUNT(P), stream));
     CN_CUDA(p, cudaMemsetAsync(p->derr, 0, sizeof(int), stream));
     CN_CUDA(p, cudaMemsetAsync(p->slotU, 0, sizeof(cplx) * (size_t)P, stream));
@@ -523,7 +533,7 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
         }
         const int64_t nch = N / 8;
         const unsigned gridc = (unsigned)((nch + 127) / 128);
-#define CN_FB(L) k_factor_blocks_chunked<L><<<gridc, 128, 0, stream>>>(nch, p->two_dx2, p->rho, Vsrc, tdG, tdF, p->q, p->gam, redSubD, redDiagD, redSupU, redDiagU, p->derr, above)
+#define CN_FB(L) k_factor_blocks_chunked<L><<<gridc, 128, 0, stream>>>(nch, p->two_dx2, p->rho, Vsrc, tdG, tdF, p->q, p->gam, redSubD, redDiagD, redSupU, redDiagU, p->derr, above, cutMask)
         switch (logc) {
         case 0: CN_FB(0); break;
         case 1: CN_FB(1); break;
@@ -532,7 +542,7 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
         case 4: CN_FB(4); break;
         case 5: CN_FB(5); break;
         default:
-            if (sharded) return CN_EINVAL; // sharded plans: blocks of 8 * 2^k <= 256 rows, whole warps of chunks
+            if (sharded || p->sysMode) return CN_EINVAL; // these need blocks of 8 * 2^k <= 256 rows, whole warps of chunks
             if (tdG) { // the thread-per-block kernel takes the potential of the step ready-made
                 k_td_potential<<<(unsigned)((N + 255) / 256), 256, 0, stream>>>(N, Vsrc, tdG, tdF, p->tdV);
                 Vsrc = p->tdV;
@@ -560,7 +570,7 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
     }
     k_rs_assemble0<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(P, N, p->rho, p->gam, p->gamJ, redSubD, redDiagD, redSupU,
                                                                  redDiagU, p->lv[0].sub, p->lv[0].diag, p->lv[0].sup, above,
-                                                                 p->diagAcc);
+                                                                 p->diagAcc, cutMask);
     p->launches += 2;
     if (p->qB && whole) { // one block per system: the factors of cn_batched_sweep and of the on-chip stepper
         k_factor_whole<<<1, 32, 0, stream>>>(N, p->rho, p->gam, p->qB, p->derr);
@@ -593,7 +603,11 @@ static void choose_partition(const cn_plan *p, int64_t *Peff, int64_t *nt)
 {
     const int64_t N = p->N;
     int64_t P = p->Pu;
-    if (p->opt_path != 1 && !p->opt_keep_p && N % 8 == 0) {
+    if (p->sysMode == 1) { // blocks of the largest 8 * 2^k <= 256 rows that divides a SYSTEM
+        int64_t me = 8;
+        while (me < 256 && p->sysN % (2 * me) == 0) me *= 2;
+        P = N / me;
+    } else if (p->opt_path != 1 && !p->opt_keep_p && N % 8 == 0) {
         const int64_t mu = (N % p->Pu == 0) ? N / p->Pu : 0;
         const bool fits = mu >= 8 && mu <= 256 && (mu & (mu - 1)) == 0;
         if (!fits) {
@@ -627,6 +641,37 @@ static cn_status factorize_impl(cn_plan *p, cudaStream_t stream, cplx *msend)
     free_factors(p);
     const int64_t N = p->N;
     const bool sharded = p->nshards > 1;
+    p->sysMode = 0;
+    if (p->sysWant) {
+        if (sharded || p->hV) return CN_EINVAL;
+        // contiguous systems of 8 * 2^k rows made of a power-of-two number of blocks: the tiled kernels with cuts
+        int64_t me = 8;
+        while (me < 256 && p->sysN % (2 * me) == 0) me *= 2;
+        const int64_t k = (p->sysN % me == 0) ? p->sysN / me : 0;
+        const bool fast = p->sysWant == 1 && p->opt_path != 1 && k >= 1 && (k & (k - 1)) == 0 && (N / 8) % 32 == 0;
+        if (p->opt_path == 2 && !fast) return CN_EINVAL;
+        p->sysMode = fast ? 1 : 2;
+    }
+    if (p->sysMode == 2) { // any dense layout: per-system pivots by one thread per system (cn_batched.cuh)
+        cn_status st;
+        if ((st = dev_alloc(p, &p->q, (size_t)N)) != CN_OK) return st;
+        if ((st = dev_alloc(p, &p->gam, (size_t)N)) != CN_OK) return st;
+        if ((st = dev_alloc(p, &p->derr, 1)) != CN_OK) return st;
+        CN_CUDA(p, cudaMemsetAsync(p->derr, 0, sizeof(int), stream));
+        const int T = 64;
+        k_batched_v_factor<<<(unsigned)((p->sysCount + T - 1) / T), T, 0, stream>>>(p->sysN, p->sysCount, p->sysEs, p->sysSs,
+                                                                                   p->two_dx2, p->rho, p->dV, p->q, p->gam,
+                                                                                   p->derr);
+        p->launches += 1;
+        int herr = 0;
+        CN_CUDA(p, cudaMemcpyAsync(&herr, p->derr, sizeof(int), cudaMemcpyDeviceToHost, stream));
+        CN_CUDA(p, cudaStreamSynchronize(stream));
+        if (herr) return CN_EBREAKDOWN;
+        p->P = p->sysCount;
+        p->path = 1;
+        p->factorized = true;
+        return CN_OK;
+    }
     // The partition the kernels work with.  psi does not depend on it (direct solver), and the tiled kernels want equal
     // blocks of 8 * 2^k rows: up to 256 rows a block lives inside one warp (shuffle scans only), 512..4096 rows span
     // several warps (shared-memory scans and CTA barriers: 189-235 us per C2 step against 158), more does not fit a
@@ -654,6 +699,7 @@ static cn_status factorize_impl(cn_plan *p, cudaStream_t stream, cplx *msend)
     }
     if (p->opt_path == 2 && !tiled_ok) return CN_EINVAL;
     // sharded: the tiled kernels on blocks inside one warp, resident, warp-per-group RS levels chosen by the library
+    if (p->sysMode == 1 && (!tiled_ok || logc > 5)) return CN_EINVAL; // cannot happen: choose_partition picked the blocks
     if (sharded && (!tiled_ok || p->opt_path == 1 || logc > 5 || (N / 8) % 32 != 0 || p->hV || p->opt_rs_levels != 0 ||
                     p->opt_rs_group != CN_RS_G || p->opt_rs_serial_top))
         return CN_EINVAL;
@@ -675,7 +721,7 @@ static cn_status factorize_impl(cn_plan *p, cudaStream_t stream, cplx *msend)
     if ((st = dev_alloc(p, &p->derr, 1)) != CN_OK) return st;
     if (p->path == 1)
         if ((st = dev_alloc(p, &p->work, (size_t)N)) != CN_OK) return st;
-    if (N <= CN_BATCHED_NMAX && !p->ooc && !sharded)
+    if (N <= CN_BATCHED_NMAX && !p->ooc && !sharded && !p->sysMode)
         if ((st = dev_alloc(p, &p->qB, (size_t)N)) != CN_OK) return st;
 
     // RS levels: lv[0] has P rows; add levels of ceil(n / G) rows until the last one fits the single CTA
@@ -867,6 +913,7 @@ static cn_status launch_pass(cn_plan *p, cplx *psi, int mode, int cur, cudaStrea
         prm.nchunks = p->N / 8;
         prm.chunk0 = 0;
         prm.P = p->P;
+        prm.cutMask = (p->sysMode == 1) ? p->sysN / (p->N / p->P) - 1 : ~(int64_t)0;
         prm.rho = p->rho;
         prm.psi_raw = psi;
         prm.supOld = supOld;
@@ -928,14 +975,15 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase =
     const bool tg = p->opt_rs_group != CN_RS_G; // one thread per group of any size (paper-shaped, cn_reduced.cuh)
     // the last level is solved inside the substitution kernel of the level below it (one launch less per step)
     const bool tis = !tg && !sharded && p->opt_rs_top_in_subst && p->opt_rs_levels >= 0 && !p->opt_rs_serial_top &&
-                     nlv >= 2 && p->lv.back().n <= p->opt_rs_top_in_subst_max;
+                     nlv >= 2 && p->lv.back().n <= p->opt_rs_top_in_subst_max && !(p->off0 && nlv == 2);
     const int64_t G = p->opt_rs_group;
     for (int i = 0; i < nsep && e == cudaSuccess && phase != 2; ++i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        if (tg)
+        const int64_t *off = (i == 0) ? p->off0 : nullptr; // caller-placed joint lines: one thread per (ragged) block
+        if (tg || off)
             e = launch_k(k_rs_reduce_thread, (unsigned)((U.n + 63) / 64), 64u, 0, stream, pdl, L.n, G, (const cplx *)L.rD,
                          (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
-                         (const cplx *)L.sup, L.X, U.rD, U.rU);
+                         (const cplx *)L.sup, (off && p->scratch0) ? p->scratch0 : L.X, U.rD, U.rU, off, p->noff0);
         else
         e = launch_k(k_rs_reduce, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
                      (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
@@ -987,9 +1035,11 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase =
     }
     for (int i = nsep - 1; i >= 0 && e == cudaSuccess; --i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        if (tg)
+        const int64_t *off = (i == 0) ? p->off0 : nullptr;
+        if (tg || off)
             e = launch_k(k_rs_subst_thread, (unsigned)((U.n + 63) / 64), 64u, 0, stream, pdl, L.n, G, (const cplx *)L.rD,
-                         (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X);
+                         (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X,
+                         off, p->noff0);
         else {
             const unsigned gr = (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS);
             const int64_t T = 32 * CN_RS_WARPS;
@@ -1032,6 +1082,7 @@ static cn_status ooc_pass(cn_plan *p, cplx *hpsi, int mode, int cur, bool first)
         prm.nchunks = n / 8;
         prm.chunk0 = r0 / 8;
         prm.P = p->P;
+        prm.cutMask = ~(int64_t)0;
         prm.rho = p->rho;
         prm.psi_raw = p->bPsi[b];
         prm.supOld = p->sup[cur ^ 1];
@@ -1096,7 +1147,19 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
     cudaStream_t stream = (cudaStream_t)stream_;
     cplx *psi = (cplx *)psi_;
     cn_status st;
+    if (p->nshards > 1) return CN_EINVAL; // a sharded plan is stepped by cn_shard_prologue / _advance / _epilogue
     if (p->ooc) return ooc_step(p, psi, nsteps, stream);
+    if (p->sysMode == 2) {
+        const int T = 64;
+        for (int64_t k = 0; k < nsteps; ++k) {
+            cudaError_t e = launch_k(k_batched_v_sweep, (unsigned)((p->sysCount + T - 1) / T), (unsigned)T, 0, stream, false,
+                                     p->sysN, p->sysCount, p->sysEs, p->sysSs, p->rho, psi, (const cplx *)p->q,
+                                     (const double *)p->gam);
+            p->launches += 1;
+            if (e != cudaSuccess) return cuda_fail(p, e);
+        }
+        return CN_OK;
+    }
     if (onchip_active(p)) {
         // one launch for the whole call: psi, q and gamma are read once, the steps loop on chip
         const int64_t chunks = (p->N + 7) / 8;
@@ -1169,7 +1232,7 @@ extern "C" cn_status cn_step_td(cn_plan *p, void *psi_, int64_t nsteps, const do
     if (!p || !psi_ || nsteps < 0 || (nsteps > 0 && !field)) return CN_EINVAL;
     if (((uintptr_t)psi_ & 15) != 0) return CN_EINVAL;
     if (!p->factorized) return CN_ENOTFACTORIZED;
-    if (p->ooc || !p->tdG) return CN_EINVAL;
+    if (p->ooc || !p->tdG || p->sysMode || p->nshards > 1) return CN_EINVAL;
     if (nsteps == 0) return CN_OK;
     for (int64_t k = 0; k < nsteps; ++k)
         if (!std::isfinite(field[k])) return CN_EINVAL; // nothing has been enqueued yet
@@ -1225,8 +1288,31 @@ extern "C" cn_status cn_tridiag_destroy(cn_tridiag *t)
     return CN_OK;
 }
 
+static cn_status tridiag_create_impl(cn_tridiag **out, int64_t N, const void *b, const void *a, const void *c,
+                                     int64_t P, const int64_t *joints, void *stream_);
+
 extern "C" cn_status cn_tridiag_create(cn_tridiag **out, int64_t N, const void *b, const void *a, const void *c,
                                        void *stream_)
+{
+    return tridiag_create_impl(out, N, b, a, c, 0, nullptr, stream_);
+}
+
+// caller-placed joint lines ("the blocks may differ in size"): block w = rows (joints[w-1], joints[w]],
+// its last row joints[w] is its joint line; joints = P strictly increasing HOST values, joints[P-1] = N - 1
+extern "C" cn_status cn_tridiag_create_blocks(cn_tridiag **out, int64_t N, const void *b, const void *a, const void *c,
+                                              int64_t P, const int64_t *joints, void *stream_)
+{
+    if (!out) return CN_EINVAL;
+    *out = nullptr;
+    if (P < 1 || P > N || !joints) return CN_EINVAL;
+    for (int64_t w = 0; w < P; ++w)
+        if (joints[w] < 0 || joints[w] >= N || (w > 0 && joints[w] <= joints[w - 1])) return CN_EINVAL;
+    if (joints[P - 1] != N - 1) return CN_EINVAL;
+    return tridiag_create_impl(out, N, b, a, c, P, joints, stream_);
+}
+
+static cn_status tridiag_create_impl(cn_tridiag **out, int64_t N, const void *b, const void *a, const void *c,
+                                     int64_t P, const int64_t *joints, void *stream_)
 {
     if (!out) return CN_EINVAL;
     *out = nullptr;
@@ -1245,13 +1331,25 @@ extern "C" cn_status cn_tridiag_create(cn_tridiag **out, int64_t N, const void *
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
             return fail(CN_ECUDA);
     }
-    // levels: n_0 = N, n_{i+1} = ceil(n_i / 256) while n_i > 4096
+    // levels: n_0 = N, n_{i+1} = ceil(n_i / 256) while n_i > 4096; with caller-placed joint lines n_1 = P
     for (int64_t n = N;;) {
         cn_plan::rs_level L;
         L.n = n;
         p->lv.push_back(L);
-        if (n <= p->opt_rs_topmax || n <= 2) break;
-        n = (n + CN_RS_G - 1) / CN_RS_G;
+        const bool ragged0 = joints && p->lv.size() == 1;
+        if (!ragged0 && (n <= p->opt_rs_topmax || n <= 2)) break;
+        n = ragged0 ? P : (n + CN_RS_G - 1) / CN_RS_G;
+    }
+    if (joints) {
+        std::vector<int64_t> off((size_t)P + 1);
+        off[0] = 0;
+        for (int64_t w = 0; w < P; ++w) off[(size_t)w + 1] = joints[w] + 1;
+        if ((st = dev_alloc(p, &p->off0, (size_t)P + 1)) != CN_OK) { cn_tridiag_destroy(t); return st; }
+        if (cudaMemcpy(p->off0, off.data(), sizeof(int64_t) * ((size_t)P + 1), cudaMemcpyHostToDevice) != cudaSuccess) {
+            cn_tridiag_destroy(t);
+            return CN_ECUDA;
+        }
+        p->noff0 = P;
     }
     const int nlv = (int)p->lv.size();
     for (int i = 0; i < nlv; ++i) {
@@ -1272,12 +1370,14 @@ extern "C" cn_status cn_tridiag_create(cn_tridiag **out, int64_t N, const void *
         }
     }
     const size_t ntop = (size_t)p->lv.back().n;
-    cplx *tmpB = nullptr;
+    cplx *tmpB = nullptr, *tmpA = nullptr;
+    const size_t n1 = joints ? (size_t)P : (size_t)((N + CN_RS_G - 1) / CN_RS_G);
     if ((st = dev_alloc(p, &p->lw, ntop)) != CN_OK || (st = dev_alloc(p, &p->rq, ntop)) != CN_OK ||
         (st = dev_alloc(p, &p->uw, ntop)) != CN_OK || (st = dev_alloc(p, &p->derr, 1)) != CN_OK ||
-        (st = dev_alloc(p, &t->zero, (size_t)N)) != CN_OK ||
-        (st = dev_alloc(p, &tmpB, (size_t)((N + CN_RS_G - 1) / CN_RS_G))) != CN_OK)
+        (st = dev_alloc(p, &t->zero, (size_t)N)) != CN_OK || (st = dev_alloc(p, &tmpB, n1)) != CN_OK)
         return fail(st);
+    if (joints && (st = dev_alloc(p, &tmpA, (size_t)N)) != CN_OK) return fail(st); // scratch of the thread-per-block kernels
+    p->scratch0 = tmpA;
     cn_plan::rs_level &L0 = p->lv[0];
     const size_t nb = sizeof(cplx) * (size_t)N;
     if (cudaMemsetAsync(t->zero, 0, nb, stream) != cudaSuccess || cudaMemsetAsync(p->derr, 0, sizeof(int), stream) != cudaSuccess ||
@@ -1290,9 +1390,14 @@ extern "C" cn_status cn_tridiag_create(cn_tridiag **out, int64_t N, const void *
     const int T = 128;
     for (int i = 0; i + 1 < nlv; ++i) {
         cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        k_rs_factor_level_smem<<<(unsigned)((U.n + CN_RS_FL_WARPS - 1) / CN_RS_FL_WARPS), 32 * CN_RS_FL_WARPS, 0, stream>>>(
-            L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr);
-        k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB);
+        if (i == 0 && joints)
+            k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, (int64_t)CN_RS_G, L.sub, L.diag, L.sup, L.l,
+                                                                             L.rp, L.u, tmpA, U.sub, U.diag, tmpB, U.sup,
+                                                                             p->derr, p->off0, p->noff0);
+        else
+            k_rs_factor_level_smem<<<(unsigned)((U.n + CN_RS_FL_WARPS - 1) / CN_RS_FL_WARPS), 32 * CN_RS_FL_WARPS, 0, stream>>>(
+                L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr, 0);
+        k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB, nullptr);
     }
     k_rs_factor_top_scan<<<1, 32, 0, stream>>>(p->lv.back().n, p->lv.back().sub, p->lv.back().diag, p->lv.back().sup, p->lw,
                                                p->rq, p->uw, p->derr);
@@ -1534,6 +1639,30 @@ extern "C" cn_status cn_batched_sweep(cn_plan *p, void *psi_, int64_t nsys, int6
     }
     if (e != cudaSuccess) return cuda_fail(p, e);
     return CN_OK;
+}
+
+// ---- many systems with a potential of their own each ---------------------------------
+extern "C" cn_status cn_plan_set_systems(cn_plan *p, int64_t nsys, int64_t elem_stride, int64_t sys_stride)
+{
+    if (!p || nsys < 1 || p->N % nsys != 0 || p->nshards > 1) return CN_EINVAL;
+    const int64_t n = p->N / nsys;
+    if (n < 2) return CN_EINVAL;
+    const bool contiguous = elem_stride == 1 && (sys_stride == n || nsys == 1);
+    const bool interleaved = sys_stride == 1 && elem_stride == nsys && !contiguous;
+    if (!contiguous && !interleaved) return CN_EINVAL; // dense layouts only: V, psi and the factors share one indexing
+    p->sysWant = contiguous ? 1 : 2;
+    p->sysN = n;
+    p->sysCount = nsys;
+    p->sysEs = elem_stride;
+    p->sysSs = contiguous ? n : 1;
+    p->factorized = false;
+    return CN_OK;
+}
+
+extern "C" cn_status cn_batched_sweep_v(cn_plan *p, void *psi, int64_t nsteps, void *stream)
+{
+    if (!p || !p->sysWant) return CN_EINVAL;
+    return cn_step(p, psi, nsteps, stream);
 }
 
 // ---- sharded mode (kernels and record layout in cn_shard.cuh) ------

@@ -624,6 +624,59 @@ __global__ void k_batched_generic(int64_t N, int64_t nsys, int64_t es, int64_t s
     }
 }
 
+// ---- systems with a potential of their own each (cn_plan_set_systems), any dense layout: one thread per system ------
+// Row i of system k lives at [k ss + i es] in V, q, gamma and psi alike.  Factor side: gamma and the
+// inverse pivots of the downward elimination of every system (one block per system); d side: Eq. 3
+// fused into the downward sweep, then the upward sweep + substitution, in place.  With interleaved systems (ss == 1)
+// the threads of a warp touch consecutive addresses in every row.  The correctness path of the general layouts;
+// contiguous systems of 8 * 2^k rows run on the tiled kernels instead (cn_pass_tiled.cuh, cutMask).
+__global__ void k_batched_v_factor(int64_t N, int64_t nsys, int64_t es, int64_t ss, double two_dx2, double rho,
+                                   const double *__restrict__ V, cplx *__restrict__ q, double *__restrict__ gam,
+                                   int *__restrict__ err)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nsys) return;
+    const int64_t o = k * ss;
+    cplx qprev = cmake(0.0, 0.0);
+    bool bad = false;
+    for (int64_t i = 0; i < N; ++i) {
+        const double g = fma(two_dx2, V[o + i * es], 2.0);
+        gam[o + i * es] = g;
+        const cplx p = cmake(-g - qprev.x, rho - qprev.y);
+        if (!cfinite_nonzero(p)) bad = true;
+        qprev = crecip(p);
+        q[o + i * es] = qprev;
+    }
+    if (bad) atomicExch(err, 1);
+}
+
+__global__ void k_batched_v_sweep(int64_t N, int64_t nsys, int64_t es, int64_t ss, double rho, cplx *__restrict__ psi,
+                                  const cplx *__restrict__ q, const double *__restrict__ gam)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nsys) return;
+    const int64_t o = k * ss;
+    cplx *p = psi + o;
+    const cplx *qk = q + o;
+    const double *gk = gam + o;
+    const cplx zero = cmake(0.0, 0.0);
+    cplx lo = zero, cur = p[0], D = zero, qprev = zero;
+    for (int64_t i = 0; i < N; ++i) {
+        cplx hi = (i + 1 < N) ? p[(i + 1) * es] : zero;
+        cplx E = rhs_E(gk[i * es], rho, cur, lo, hi);
+        D = cfnma(qprev, D, E);
+        p[i * es] = D;
+        qprev = qk[i * es];
+        lo = cur;
+        cur = hi;
+    }
+    cplx x = zero;
+    for (int64_t i = N - 1; i >= 0; --i) {
+        x = cmul(qk[i * es], csub(p[i * es], x));
+        p[i * es] = x;
+    }
+}
+
 // whole-system inverse pivots (one block per system): p_0 = mu_0, p_i = mu_i - q_{i-1}, q_i = 1 / p_i
 __global__ void k_factor_whole(int64_t N, double rho, const double *__restrict__ gam, cplx *__restrict__ qB,
                                int *__restrict__ err)

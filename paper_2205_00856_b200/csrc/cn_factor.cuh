@@ -140,8 +140,9 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
                         const double *__restrict__ tdG, double tdF, // potential = V + tdF * tdG when tdG != NULL (cn_step_td)
                         cplx *__restrict__ q, double *__restrict__ gam, cplx *__restrict__ redSubD,
                         cplx *__restrict__ redDiagD, cplx *__restrict__ redSupU, cplx *__restrict__ redDiagU,
-                        int *__restrict__ err, int above = 0) // above: a shard precedes this one (cn_shard.cuh): the first
+                        int *__restrict__ err, int above = 0, // above: a shard precedes this one (cn_shard.cuh): the first
                                                               // block's JU matrix side goes to the guard element [-1]
+                        int64_t cutMask = ~(int64_t)0)        // independent systems of cutMask + 1 blocks (cn_pass_tiled.cuh)
 {
     constexpr int CPB = 1 << LOGC;
     const int lane = threadIdx.x & 31;
@@ -222,9 +223,9 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
         const cplx Zn1 = cmul(qlast, pp);
         redSubD[w] = cneg(Zn1);
         redDiagD[w] = cneg(qlast);
-        if (w > 0 || above) redSupU[w - 1] = cneg(Zn1);
+        if ((w & cutMask) != 0 || above) redSupU[w - 1] = cneg(Zn1);
     }
-    if (isFirst && (w > 0 || above)) {
+    if (isFirst && ((w & cutMask) != 0 || above)) {
         const cplx quf = cmul(U.b, crecip_fast(U.d)); // with LOGC == 0 isFirst == isLast and U is already the constant map
         if (!cfinite_nonzero(U.d)) bad = true;
         redDiagU[w - 1] = cneg(quf);

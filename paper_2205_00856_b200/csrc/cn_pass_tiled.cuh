@@ -30,6 +30,9 @@ struct cn_tiled_params {
     int64_t nchunks; // chunks (8 points) in the array the tensor maps describe: N / 8, or one streamed part of it
     int64_t chunk0;  // global index of its first chunk (0 unless psi is streamed part by part, ooc_* in cn_api.cu)
     int64_t P;
+    int64_t cutMask; // ~0: one system.  k - 1 (k a power of two): the array holds independent systems of k blocks each
+                     // (cn_plan_set_systems): a block whose index is a multiple of k has the virtual joint line "psi = 0"
+                     // above it, exactly like block 0 of a single system (reading R8)
     double rho;
     const cplx *psi_raw; // prologue only: old psi for the tile's left halo (same array as tmPsi)
     const cplx *supOld;  // psi^k   at the joint lines (RS output of the previous step)
@@ -145,17 +148,19 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
         const bool isFirst = (c & (CPB - 1)) == 0;
         const bool isLast = (c & (CPB - 1)) == CPB - 1;
         const int64_t w = cg >> LOGC;
+        const bool top = (w & prm.cutMask) == 0;                 // first block of a system
+        const bool bottom = ((w + 1) & prm.cutMask) == 0 || w == prm.P - 1; // last block of a system
 
         // the few values that live on the joint lines (issued before waiting for the tile)
         cplx supN = zero;       // new value of the own joint line (last chunk of a block)
         cplx jointAbove = zero; // new value of the joint line above the block of this thread
         if (P1 && active) {
             if (isLast) supN = prm.supNew[w];
-            if (w > 0) jointAbove = prm.supNew[w - 1];
+            if (!top) jointAbove = prm.supNew[w - 1];
         }
         cplx oldAbove = zero; // OLD psi just above the tile (needed by thread 0 only)
         // (prologue of a streamed part: the row above it is a joint line whose psi^0 the previous part recorded)
-        if (t == 0 && cg > 0) oldAbove = P1 ? prm.supOld[w - 1] : (c > 0 ? prm.psi_raw[8 * c - 1] : prm.supInit[w - 1]);
+        if (t == 0 && !top) oldAbove = P1 ? prm.supOld[w - 1] : (c > 0 ? prm.psi_raw[8 * c - 1] : prm.supInit[w - 1]);
 
         mbar_wait(bar, phase);
         phase ^= 1;
@@ -182,6 +187,7 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
             qm1 = s_q[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
         }
         if (t < TPB - 1) vhi = s_psi[(t + 1) * 8 + ((t + 1) & 7)];
+        if (isFirst && top) vlo = zero;       // nothing above the first row of a system
         if (!P1 && isFirst) jointAbove = vlo; // prologue: psi^0 of the joint above
 
         // everybody has its copy: refill the input buffers with the next tile while this one is computed.
@@ -388,10 +394,10 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
             if (active) {
                 if (isLast) {
                     prm.slotD[w] = csub(EJ, yn);
-                    if (w == prm.P - 1) prm.slotU[w] = zero;
+                    if (bottom) prm.slotU[w] = zero;
                     if (!P1) prm.supInit[w] = v[7];
                 }
-                if (isFirst && w > 0) {
+                if (isFirst && !top) {
                     cplx y0 = cfma(bwdA, yin, Y); // isLast && isFirst: bwdA = 0 and Y is already exact
                     prm.slotU[w - 1] = cneg(cadd(v[0], y0));
                 }

@@ -259,6 +259,36 @@ def run_tridiag(torch, peak, N=1 << 24):
             "bytes_per_row": 176, "GBps": gbs, "hbm_frac_measured_peak": gbs / peak, "create_ms": fms}
 
 
+def run_systems(torch, peak, n=8192, nsys=8192, nsteps=20):
+    """Many systems with a potential of their own each (cn_plan_set_systems, row f-3) at C4's shape: a non-separable
+    V(x, y) gives every line its own matrix.  Contiguous systems (the x sweep) run on the fused tiled pass: 56 B per
+    point and step; interleaved systems (the y sweep) on one thread per system (correctness path)."""
+    cfg = W.CONFIGS["C4"]
+    x = W.grid(cfg)
+    rng = np.random.default_rng(cfg.seed)
+    V2 = 0.5 * (x[None, :n] ** 2 + x[:nsys, None] ** 2) + 0.1 * np.cos(x[None, :n] * x[:nsys, None])
+    psi = rng.standard_normal((nsys, n)) + 1j * rng.standard_normal((nsys, n))
+    d = torch.from_numpy(psi.reshape(-1)).cuda()
+    out = {"config": "C4 shape, per-system potentials", "n": n, "nsys": nsys}
+    for key, lay in (("contiguous", (1, n)), ("interleaved", (nsys, 1))):
+        Vl = np.ascontiguousarray(V2 if key == "contiguous" else V2.T).reshape(-1)
+        with B.Plan(n * nsys, nsys, cfg.dx, cfg.dt, Vl) as plan:
+            plan.set_systems(nsys, *lay).factorize()
+            k = nsteps if key == "contiguous" else 2
+            plan.batched_sweep_v(d, 2)
+            torch.cuda.synchronize()
+            e0, e1 = _events(torch)
+            e0.record()
+            plan.batched_sweep_v(d, k)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / k
+            gbs = 56.0 * n * nsys / (ms * 1e-3) / 1e9
+            out[key] = {"ms_per_sweep": ms, "Gpoint_sweeps_per_s": n * nsys / ms / 1e6, "path": plan.info()["path"],
+                        "bytes_per_point": 56, "GBps": gbs, "hbm_frac_measured_peak": gbs / peak}
+    return out
+
+
 def run_shards(torch, peak, name="C2dense", S=8, nsteps=50, **opts):
     """Sharded mode (cn_shard_*, row f-4) on ONE device: the S shards of one system stepped in-process, their records
     "gathered" by concatenation (sharded.LocalShards).  The shards' kernels run one after the other on the one GPU,
@@ -366,6 +396,8 @@ def main(argv=None):
             emit(run_td(torch, peak))
         elif name == "TRI":
             emit(run_tridiag(torch, peak))
+        elif name == "SYSV":
+            emit(run_systems(torch, peak))
         elif name == "SHARD":
             for S, opts in ((1, {}), (2, {}), (8, {}), (8, {"rs_topmax": 1})):
                 emit(dict(run_shards(torch, peak, S=S, **opts), options=opts))

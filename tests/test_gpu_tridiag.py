@@ -83,3 +83,64 @@ def test_tridiag_breakdown_and_errors():
     assert e.value.status == B.CN_EBREAKDOWN
     assert B.lib().cn_tridiag_solve(None, None, None, None) == B.CN_EINVAL
     assert B.lib().cn_tridiag_destroy(None) == B.CN_EINVAL
+
+
+def ragged_joints(n, kind, seed):
+    """caller-placed joint lines (blocks may differ in size); always end at row n - 1"""
+    rng = np.random.default_rng(seed)
+    if kind == "single":            # one block: the whole system is the interior of the last row's block
+        return [n - 1]
+    if kind == "every_row":         # every row is a joint line (blocks of one row, no interior anywhere)
+        return list(range(n))
+    if kind == "pairs":             # blocks of two rows: one interior row each (+ a one-row block if n is odd)
+        return sorted(set(list(range(1, n, 2)) + [n - 1]))
+    if kind == "paper":             # the paper's literal placement J_w = round(w (n - 1) / P), P ~ sqrt(n)
+        P = max(1, int(round(n ** 0.5)))
+        return sorted(set(int(round(w * (n - 1) / P)) for w in range(1, P + 1)))
+    # random unequal blocks of 1 .. ~3 sqrt(n) rows, with some runs of adjacent joint lines
+    out, j = [], -1
+    top = max(2, int(3 * n ** 0.5))
+    while True:
+        j += int(rng.integers(1, top)) if rng.random() > 0.2 else 1
+        if j >= n - 1:
+            break
+        out.append(j)
+    return out + [n - 1]
+
+
+@pytest.mark.parametrize("n,kind", [(1, "single"), (2, "every_row"), (2, "single"), (9, "random"), (10, "pairs"),
+                                    (40, "random"), (257, "paper"), (1000, "every_row"), (4096, "random"),
+                                    (4097, "pairs"), (70001, "random"), (300000, "paper"), (300000, "single"),
+                                    ((1 << 20) + 3, "random"), ((1 << 21), "pairs")])
+def test_tridiag_caller_placed_joints(n, kind):
+    """The same solve with the joint lines where the CALLER puts them: x does not depend on the partition."""
+    import torch
+    if kind == "single" and n > 100000:
+        n = 50000  # one thread sweeps the whole system: keep it short
+    b, a, c, d = system(n, seed=300 + n % 89)
+    ref = O.thomas(b, a, c, d)
+    J = ragged_joints(n, kind, seed=n)
+    assert J[-1] == n - 1 and all(J[i] < J[i + 1] for i in range(len(J) - 1))
+    dd = torch.from_numpy(d).cuda()
+    xx = torch.empty_like(dd)
+    with B.Tridiag(b, a, c, joints=J) as t:
+        t.solve(dd, xx)
+        torch.cuda.synchronize()
+        x = xx.cpu().numpy()
+        assert np.max(np.abs(x - ref)) <= 1e-10 * max(1.0, np.max(np.abs(ref)))
+        assert residual(b, a, c, d, x) <= 1e-12
+        buf = torch.from_numpy(d).cuda()   # in place (x aliases d)
+        t.solve(buf)
+        t.solve(dd, xx)                    # and again: the factors are not consumed
+        torch.cuda.synchronize()
+        assert np.array_equal(buf.cpu().numpy(), x) and np.array_equal(xx.cpu().numpy(), x)
+
+
+def test_tridiag_joints_rejected():
+    n = 100
+    b, a, c, d = system(n, 5)
+    for J in ([10, 5, 99], [10, 10, 99], [10, 50], [-1, 99], [10, 100], []):
+        with pytest.raises((B.CnError, ValueError)) as e:
+            B.Tridiag(b, a, c, joints=J)
+        if isinstance(e.value, B.CnError):
+            assert e.value.status == B.CN_EINVAL
