@@ -561,63 +561,134 @@ __global__ void k_rs_factor_level(int64_t n, int64_t G, const cplx *__restrict__
     if (bad) atomicExch(err, 1);
 }
 
-// The same for groups of CN_RS_G = 256 rows with the group's rows staged in shared memory: one WARP per group loads
-// and stores its rows coalesced, lane 0 runs the (inherently serial) recurrences on shared memory.  The thread-per-
-// group kernel above pays a full global-memory latency per row (268 us for 512 groups at C2); this one 35 us.
-#define CN_RS_FL_WARPS 2
+// The same for groups of CN_RS_G = 256 rows by ONE WARP per group, 8 rows per lane in registers (rows moved coalesced
+// through the swizzled buffer of rs_load_rows_n).  Every serial recurrence of the thread-per-group kernel above becomes
+// a warp scan over the lanes:
+//   * pivots: rp_i = 1 / (diag_i - sub_i sup_{i-1} rp_{i-1}) is a Moebius map of rp_{i-1} (cn_factor.cuh); the lanes'
+//     2x2 matrices are composed by a Kogge-Stone scan, then every lane recomputes its 8 rows from its true inflow;
+//   * Dal_i = prod_{k <= i} (-l_k) (forward response to a unit support value above the group): multiplicative scan;
+//   * al_i = rp_i Dal_i - u_i al_{i+1} and be_i = prod_{k >= i} (-u_k): ONE backward affine scan gives both (be is its A).
+// The thread-per-group kernel pays a global-memory latency per row (268 us for 512 groups at C2), its shared-memory
+// variant with one serial lane took 45 us, this one takes a few us -- it runs once per step under cn_step_td.
+#define CN_RS_FL_WARPS 4
 __global__ void __launch_bounds__(32 * CN_RS_FL_WARPS)
 k_rs_factor_level_smem(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
                        const cplx *__restrict__ sup, cplx *__restrict__ l, cplx *__restrict__ rp, cplx *__restrict__ u,
                        cplx *__restrict__ sub2, cplx *__restrict__ diag2, cplx *__restrict__ diag2U,
                        cplx *__restrict__ sup2, int *__restrict__ err, int above = 0)
 {   // above (cn_shard.cuh): group 0 is treated like any later group; its JU matrix side goes to the guards [-1]
-    __shared__ cplx sm[CN_RS_FL_WARPS][4][CN_RS_G]; // sub -> l, diag -> rp, sup -> u, tmp
+    constexpr int K = CN_RS_K;
+    __shared__ cplx sbuf_all[CN_RS_FL_WARPS][3 * CN_RS_G];
     const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    cplx *const sbuf = sbuf_all[wp];
     const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
     const int64_t g = (int64_t)blockIdx.x * CN_RS_FL_WARPS + wp;
     if (g >= ngroups) return; // whole warps
     const int64_t g0 = g * CN_RS_G;
     const int ng = (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G);
     const int nj = ng - 1; // interior rows; row nj is the joint line
-    cplx *sS = sm[wp][0], *sD = sm[wp][1], *sU = sm[wp][2], *sT = sm[wp][3];
-    for (int i = lane; i < ng; i += 32) {
-        sS[i] = sub[g0 + i];
-        sD[i] = diag[g0 + i];
-        sU[i] = sup[g0 + i];
-    }
-    __syncwarp();
+    const int r0 = lane * K;
     const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
-    if (lane == 0) {
-        const cplx subJ = sS[nj], diagJ = sD[nj];
-        bool bad = false;
-        cplx prp = one, psup = zero, Dal = one;
-        for (int i = 0; i < nj; ++i) {
-            const cplx supi = sU[i];
-            cplx li = cmul(sS[i], prp);
-            cplx piv = cfnma(li, psup, sD[i]);
-            if (!cfinite_nonzero(piv)) bad = true;
-            cplx r = crecip_fast(piv);
-            sS[i] = li;
-            sD[i] = r;
-            sU[i] = cmul(supi, r);
-            Dal = cneg(cmul(li, Dal));
-            sT[i] = Dal;
-            prp = r;
-            psup = supi;
+    cplx F[3][K];
+    {
+        const cplx *const src[3] = {sub + g0, diag + g0, sup + g0};
+        const int lim[3] = {ng, ng, ng};
+        rs_load_rows_n<false, 3>(src, lim, sbuf, lane, F);
+    }
+    cplx (&sb)[K] = F[0], (&dg)[K] = F[1], (&sp)[K] = F[2];
+    // the joint line's own entries, for lane 0
+    cplx subJ = zero, diagJ = zero;
+#pragma unroll
+    for (int k = 0; k < K; ++k)
+        if (r0 + k == nj) {
+            subJ = sb[k];
+            diagJ = dg[k];
         }
-        sS[nj] = zero;
-        sD[nj] = zero;
-        sU[nj] = zero;
-        const bool has = nj > 0;
-        cplx al = zero, be = one, alLast = zero, beLast = zero;
-        for (int i = nj - 1; i >= 0; --i) {
-            al = cfnma(sU[i], al, cmul(sD[i], sT[i]));
-            be = cneg(cmul(sU[i], be));
-            if (i == nj - 1) {
-                alLast = al;
-                beLast = be;
+    subJ = shfl_c(subJ, nj / K);
+    diagJ = shfl_c(diagJ, nj / K);
+    // sup of the row before each own row (0 before the group's first row: nothing is eliminated against the joint above)
+    cplx spPrev0 = shfl_up_c(sp[K - 1], 1);
+    if (lane == 0) spPrev0 = zero;
+    // ---- pivots: Moebius maps of the own rows, scan, recompute ----------------------------------------------------
+    cn_mob M{one, zero, zero, one};
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        if (r0 + k < nj) {
+            const cplx ci = cmul(sb[k], (k == 0) ? spPrev0 : sp[k - 1]); // (row 0 of the group: spPrev0 = 0, a constant map)
+            cn_mob Rm; // [[0, 1], [-c_i, d_i]] * M
+            Rm.a = M.c;
+            Rm.b = M.d;
+            Rm.c = csub(cmul(dg[k], M.c), cmul(ci, M.a));
+            Rm.d = csub(cmul(dg[k], M.d), cmul(ci, M.b));
+            M = mob_scale(Rm);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const int dd = 1 << k;
+        cn_mob S = mob_shfl(M, lane - dd < 0 ? 0 : lane - dd);
+        if (lane >= dd) M = mob_scale(mob_mul(M, S));
+    }
+    cn_mob Pm = mob_shfl(M, lane == 0 ? 0 : lane - 1);
+    cplx rprev = (lane == 0) ? one : cmul(Pm.b, crecip_fast(Pm.d)); // rp := 1 above the first interior row
+    bool bad = false;
+    cplx lk[K], rpk[K], uk[K];
+    cplx pl = one; // product of (-l) over the own interior rows
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        lk[k] = rpk[k] = uk[k] = zero;
+        if (r0 + k < nj) {
+            const cplx li = cmul(sb[k], rprev);
+            const cplx piv = cfnma(li, (k == 0) ? spPrev0 : sp[k - 1], dg[k]);
+            if (!cfinite_nonzero(piv)) bad = true;
+            const cplx r = crecip_fast(piv);
+            lk[k] = li;
+            rpk[k] = r;
+            uk[k] = cmul(sp[k], r);
+            pl = cmul(pl, cneg(li));
+            rprev = r;
+        }
+    }
+    // ---- Dal_i = prod_{k <= i} (-l_k): multiplicative scan over the lanes, then the own rows -----------------------
+    cplx pin = pl;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const int dd = 1 << k;
+        const cplx s = shfl_up_c(pin, dd);
+        if (lane >= dd) pin = cmul(pin, s);
+    }
+    cplx Dal = shfl_up_c(pin, 1);
+    if (lane == 0) Dal = one;
+    // ---- backward affine scan: al_i = rp_i Dal_i - u_i al_{i+1}, be_i = -u_i be_{i+1} ---------------------------------
+    cplx Rk[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        Rk[k] = zero;
+        if (r0 + k < nj) {
+            Dal = cneg(cmul(lk[k], Dal));
+            Rk[k] = cmul(rpk[k], Dal);
+        }
+    }
+    cplx A = one, B = zero;
+    cplx alLast = zero, beLast = zero;
+#pragma unroll
+    for (int k = K - 1; k >= 0; --k) {
+        if (r0 + k < nj) {
+            B = cfnma(uk[k], B, Rk[k]);
+            A = cmul(cneg(uk[k]), A);
+            if (r0 + k == nj - 1) {
+                alLast = Rk[k];
+                beLast = cneg(uk[k]);
             }
         }
+    }
+    warp_scan_affine<-1, 5>(A, B, lane); // lane 0: the composite of all interior rows, applied to (al, be) = (0, 1) below
+    const int lastLane = nj > 0 ? (nj - 1) / K : 0;
+    alLast = shfl_c(alLast, lastLane);
+    beLast = shfl_c(beLast, lastLane);
+    if (lane == 0) {
+        const bool has = nj > 0;
+        const cplx al = B, be = A;
         sub2[g] = (g == 0 && !above) ? zero : (has ? cmul(subJ, alLast) : subJ);
         diag2[g] = has ? cfma(subJ, beLast, diagJ) : diagJ;
         if (g > 0 || above) {
@@ -629,14 +700,11 @@ k_rs_factor_level_smem(int64_t n, const cplx *__restrict__ sub, const cplx *__re
             diag2U[g] = zero;
             sup2[g] = zero;
         }
-        if (bad) atomicExch(err, 1);
     }
-    __syncwarp();
-    for (int i = lane; i < ng; i += 32) {
-        l[g0 + i] = sS[i];
-        rp[g0 + i] = sD[i];
-        u[g0 + i] = sU[i];
-    }
+    if (__any_sync(0xffffffffu, bad) && lane == 0) atomicExch(err, 1);
+    rs_store_rows(l + g0, ng, sbuf, lane, lk);
+    rs_store_rows(rp + g0, ng, sbuf, lane, rpk);
+    rs_store_rows(u + g0, ng, sbuf, lane, uk);
 }
 
 // LU of the last level's matrix by ONE WARP: rq_i = 1 / (diag_i - sub_i sup_{i-1} rq_{i-1}) is a Moebius map of
