@@ -32,6 +32,11 @@ CN_DEVINL cplx cfnma(cplx a, cplx b, cplx c)
 {
     return make_double2(fma(a.y, b.y, fma(-a.x, b.x, c.x)), fma(-a.y, b.x, fma(-a.x, b.y, c.y)));
 }
+// a*b - c
+CN_DEVINL cplx cmsub(cplx a, cplx b, cplx c)
+{
+    return make_double2(fma(-a.y, b.y, fma(a.x, b.x, -c.x)), fma(a.y, b.x, fma(a.x, b.y, -c.y)));
+}
 CN_DEVINL cplx crecip(cplx a)
 {
     // scaled by the larger component so that |a|^2 can neither overflow nor underflow early

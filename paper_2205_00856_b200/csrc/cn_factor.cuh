@@ -83,8 +83,11 @@ __global__ void k_factor_blocks(cn_geom g, double two_dx2, double rho, const dou
 // [[a, b], [c, d]] : q -> (a q + b) / (c q + d), row i contributing [[0, 1], [-1, mu_i]].  Every thread multiplies the
 // matrices of its 8 rows, a segmented Kogge-Stone scan over the lanes of the block composes them (a block's first
 // chunk is entered by q = 0, so its map is the CONSTANT b / d and everything downstream of it is constant too), and
-// each thread then recomputes its own 8 pivots serially from its true inflow.  The upward pivots (only Z_{1,1} is
-// needed) are the same scan in the other direction.  The matrix of a chunk is rescaled by a power of two (a Moebius
+// each thread then recomputes its own 8 pivots serially from its true inflow.  Of the upward elimination only
+// Z_{1,1} = (block matrix)^-1_{1,1} is needed; solving A x = e_1 with the downward factors (y_i = prod_{k<i} (-q_k),
+// x_i = q_i (y_i - x_{i+1})) gives the closed form  Z_{1,1} = sum_i q_i prod_{k<i} q_k^2  over the block's interior rows:
+// a running product in the same serial loop and one segmented SUM over the lanes of the block -- no second Moebius
+// scan (it cost a third of this kernel's FP64 work).  The matrix of a chunk is rescaled by a power of two (a Moebius
 // map does not change when its matrix is scaled), so |mu|^8 never overflows; the scan then multiplies at most 2^LOGC
 // matrices with components below 2, which needs no further rescaling.
 // Memory: a thread reads 64 contiguous bytes of V and writes 128 of q and 64 of gamma -- whole sectors, against one
@@ -97,8 +100,8 @@ CN_DEVINL cn_mob mob_row(cn_mob M, cplx mu) // [[0, 1], [-1, mu]] * M
     cn_mob R;
     R.a = M.c;
     R.b = M.d;
-    R.c = csub(cmul(mu, M.c), M.a);
-    R.d = csub(cmul(mu, M.d), M.b);
+    R.c = cmsub(mu, M.c, M.a);
+    R.d = cmsub(mu, M.d, M.b);
     return R;
 }
 CN_DEVINL cn_mob mob_mul(cn_mob H, cn_mob L) // H * L : first L, then H
@@ -188,15 +191,19 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
     cplx qin = isFirst ? zero : cmul(Pm.b, crecip_fast(Pm.d));
     bool bad = false;
     cplx pp = one, qlast = zero; // product of (-q) over this chunk's rows except the block's last interior row
+    cplx tq = zero, zacc = zero;  // q_j prod_{k<j} q_k^2 over the rows of this chunk (k from the chunk's first row), its sum
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
         if (j < nrow) {
             cplx p = cmake(-g[j] - qin.x, rho - qin.y);
             if (!cfinite_nonzero(p)) bad = true;
-            qin = crecip_fast(p);
-            q[8 * c + j] = qin;
-            if (!(isLast && j == 6)) pp = cmul(pp, cneg(qin));
-            qlast = qin;
+            const cplx qnew = crecip_fast(p);
+            q[8 * c + j] = qnew;
+            if (!(isLast && j == 6)) pp = cmul(pp, cneg(qnew));
+            tq = (j == 0) ? qnew : cmul(cmul(tq, qlast), qnew);
+            zacc = cadd(zacc, tq);
+            qlast = qnew;
+            qin = qnew;
         }
     }
     if (isLast) q[8 * c + 7] = one;
@@ -206,18 +213,15 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
         cplx sp = shfl_c(pp, lane - dd < 0 ? 0 : lane - dd);
         if (pos >= dd) pp = cmul(pp, sp);
     }
-    // ---- upward: only Z_{1,1} = qu of the block's first row ---------------------------------------------------
-    cn_mob U{one, zero, zero, one};
-#pragma unroll
-    for (int j = 7; j >= 0; --j)
-        if (j < nrow) U = mob_row(U, cmake(-g[j], rho));
-    if (isLast) { U.a = zero; U.c = zero; } // nothing enters from the joint line below
-    U = mob_scale(U);
+    // ---- Z_{1,1} = sum over the block of (prod of (-q) over the chunks before)^2 * (this chunk's sum) ----------------
+    cplx yin = shfl_up_c(pp, 1); // inclusive product of the chunks before this one (all of them whole chunks)
+    if (isFirst) yin = one;
+    cplx zs = cmul(cmul(yin, yin), zacc);
 #pragma unroll
     for (int k = 0; k < LOGC; ++k) {
         const int dd = 1 << k;
-        cn_mob S = mob_shfl(U, lane + dd > 31 ? 31 : lane + dd);
-        if (pos + dd < CPB) U = mob_mul(U, S);
+        const cplx s = shfl_down_c(zs, dd);
+        if (pos + dd < CPB) zs = cadd(zs, s);
     }
     if (isLast) {
         const cplx Zn1 = cmul(qlast, pp);
@@ -225,11 +229,7 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
         redDiagD[w] = cneg(qlast);
         if ((w & cutMask) != 0 || above) redSupU[w - 1] = cneg(Zn1);
     }
-    if (isFirst && ((w & cutMask) != 0 || above)) {
-        const cplx quf = cmul(U.b, crecip_fast(U.d)); // with LOGC == 0 isFirst == isLast and U is already the constant map
-        if (!cfinite_nonzero(U.d)) bad = true;
-        redDiagU[w - 1] = cneg(quf);
-    }
+    if (isFirst && ((w & cutMask) != 0 || above)) redDiagU[w - 1] = cneg(zs);
     if (bad) atomicExch(err, 1);
 }
 
