@@ -116,6 +116,35 @@ def run_c4(torch, peak):
     return out
 
 
+def run_c4_sizes(torch, peak, total=8192 * 8192):
+    """The shared-matrix sweeps at C4's total size (2^26 points) cut into systems of 512 ... 8192 rows: where the
+    kernels lose their bandwidth (cross-warp scan from 512 rows, one CTA per system at 2048, clusters of 2 / 4 CTAs at
+    4096 / 8192 rows for x; clusters from 2048 rows for y)."""
+    cfg = W.CONFIGS["C4"]
+    d = torch.randn(total, dtype=torch.complex128, device="cuda")
+    rows = []
+    for n in (512, 1024, 2048, 4096, 8192):
+        nsys = total // n
+        c = W.scaled(cfg, N=n)
+        with B.Plan(n, 8, c.dx, c.dt, W.potential(c)) as p:
+            p.factorize()
+            for key, args in (("x", (nsys, 1, n)), ("y", (nsys, nsys, 1))):
+                for _ in range(3):
+                    p.batched_sweep(d, *args, 1)
+                torch.cuda.synchronize()
+                e0, e1 = _events(torch)
+                e0.record()
+                for _ in range(20):
+                    p.batched_sweep(d, *args, 1)
+                e1.record()
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1) / 20
+                gbs = 32.0 * total / (ms * 1e-3) / 1e9
+                rows.append({"rows_per_system": n, "systems": nsys, "sweep": key, "ms": ms, "GBps": gbs,
+                             "hbm_frac_measured_peak": gbs / peak})
+    return {"config": "C4 total size, systems of 512..8192 rows (shared matrix)", "rows": rows}
+
+
 def link_rate(torch, nbytes=1 << 30):
     """pinned host <-> device copy rates of this box (GB/s): H2D alone, D2H alone, both at once."""
     h0 = torch.empty(nbytes, dtype=torch.uint8).pin_memory()
@@ -396,6 +425,8 @@ def main(argv=None):
             emit(run_td(torch, peak))
         elif name == "TRI":
             emit(run_tridiag(torch, peak))
+        elif name == "C4SIZES":
+            emit(run_c4_sizes(torch, peak))
         elif name == "SYSV":
             emit(run_systems(torch, peak))
         elif name == "SHARD":
