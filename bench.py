@@ -293,6 +293,75 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_sharded(args, torch, dist, B, rank, world, local):
+    """ONE C2 system over `world` GPUs (row f-4): rank r owns rows [r N / world, (r + 1) N / world) and never sees the
+    rest; per step one all-gather of `step_count` complex values per rank (paper_2205_00856_b200/sharded.py).  Same
+    timing contract as the replica mode (barrier + synchronize on both sides, CUDA events, max over ranks); value = the
+    WHOLE system's point-steps per second, so the scaling is strong."""
+    from paper_2205_00856_b200 import sharded as SH
+    cfg = W.CONFIGS["C2dense"]
+    n = cfg.N // world
+    assert n * world == cfg.N and n % 256 == 0, "the shards must be equal and multiples of 256 rows"
+    cn_per = args.cn_per_step
+    V = W.potential(cfg, rank * n, (rank + 1) * n)
+    norm = W.psi0_norm2(cfg)
+    d_psi = torch.from_numpy(W.psi0(cfg, rank * n, (rank + 1) * n, norm=norm)).cuda()
+    plan = B.ShardPlan(n, max(1, n // 256), cfg.dx, cfg.dt, V, rank, world)
+    if world == 1:
+        class _One:  # a single process: the gather is the record itself
+            def get_world_size(self, group=None):
+                return 1
+
+            def all_gather_into_tensor(self, out, inp, group=None):
+                out.copy_(inp)
+        dist = _One()
+    st = SH.DistributedStepper(plan, device=torch.device("cuda", local), dist=dist)
+    st.factorize()
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+    for _ in range(args.warmup):
+        st.step(d_psi, cn_per)
+    launches0 = plan.info()["launches"]
+    sampler = ClockSampler(local, args.clock_interval_ms)
+    sampler.start()
+    time.sleep(0.1)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    w0 = time.time()
+    e0.record(stream)
+    for _ in range(args.steps):
+        st.step(d_psi, cn_per)
+    e1.record(stream)
+    barrier()
+    w1 = time.time()
+    ms = R.max_over_ranks(e0.elapsed_time(e1), world, device="cuda")
+    clocks = sampler.stop(w0, w1)
+    mcount, scount = plan.counts()
+    nrm = d_psi.real.square().sum() + d_psi.imag.square().sum()
+    if world > 1:
+        dist.all_reduce(nrm)
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": cfg.N * cn_per * args.steps / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": dict(bench_config(cfg, cfg.P, world), parallelism="one system over %d shards (cn_shard_*)" % world),
+            "launch": {"cn_steps_per_bench_step": cn_per, "rows_per_shard": n, "record_values_per_step": scount,
+                       "record_values_matrix": mcount, "exchange": "all_gather_into_tensor per step, %d B per rank" % (16 * scount)},
+            "clocks": clocks, "gpu_launches": int(plan.info()["launches"] - launches0),
+            "norm_minus_1": float(nrm.item()) * cfg.dx - 1.0,
+        }
+        print(json.dumps(line), flush=True)
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -308,6 +377,10 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="also time the P sweep 2^8..2^16 (extra JSON key)")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config object (C1, C4, TD, TRI)")
     ap.add_argument("--full", action="store_true", help="per_config also runs C3 (2^30, 85 GB host) and C5 (2^29, streamed)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: ONE C2 system spread over the N GPUs (cn_shard_*, one all-gather of a small record per step "
+                         "over NCCL) instead of N replicas; \"scaling\": \"strong\".  Not what the driver runs; unmeasured on "
+                         "hardware in this build (DESIGN.md section 9)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -324,6 +397,9 @@ def main():
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    if args.sharded:
+        return run_sharded(args, torch, dist, B, rank, world, local)
 
     cfg = W.CONFIGS["C2dense"]
     P = args.P or cfg.P

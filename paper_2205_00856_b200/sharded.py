@@ -82,9 +82,11 @@ class DistributedStepper:
     it is in flight the next pass kernel is already resident and prefetching its first psi / q / gamma tiles
     (programmatic dependent launch), which depend on nothing that is exchanged."""
 
-    def __init__(self, plan, group=None, device=None):
+    def __init__(self, plan, group=None, device=None, dist=None):
+        """dist: anything with get_world_size / all_gather_into_tensor (default: torch.distributed, initialised)."""
         import torch
-        import torch.distributed as dist
+        if dist is None:
+            import torch.distributed as dist
         self.torch, self.dist, self.plan, self.group = torch, dist, plan, group
         self.world = dist.get_world_size(group)
         self.device = device if device is not None else (torch.device("cuda", torch.cuda.current_device())
