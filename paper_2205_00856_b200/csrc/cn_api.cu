@@ -1150,7 +1150,7 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
     if (p->nshards > 1) return CN_EINVAL; // a sharded plan is stepped by cn_shard_prologue / _advance / _epilogue
     if (p->ooc) return ooc_step(p, psi, nsteps, stream);
     if (p->sysMode == 2) {
-        const int T = 64;
+        const int T = 32; // few systems: small CTAs spread the warps over the SMs
         for (int64_t k = 0; k < nsteps; ++k) {
             cudaError_t e = launch_k(k_batched_v_sweep, (unsigned)((p->sysCount + T - 1) / T), (unsigned)T, 0, stream, false,
                                      p->sysN, p->sysCount, p->sysEs, p->sysSs, p->rho, psi, (const cplx *)p->q,

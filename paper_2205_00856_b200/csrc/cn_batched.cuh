@@ -650,9 +650,16 @@ __global__ void k_batched_v_factor(int64_t N, int64_t nsys, int64_t es, int64_t 
     if (bad) atomicExch(err, 1);
 }
 
-__global__ void k_batched_v_sweep(int64_t N, int64_t nsys, int64_t es, int64_t ss, double rho, cplx *__restrict__ psi,
-                                  const cplx *__restrict__ q, const double *__restrict__ gam)
+// Rows are handled in batches of CN_BV_U: all loads of a batch are issued before its serial arithmetic and its stores (the
+// in-place update keeps the compiler from hoisting loads over stores by itself), so a thread has CN_BV_U rows of three
+// arrays in flight instead of one -- the difference between a latency-bound and a bandwidth-bound sweep when there are
+// only a few thousand systems.
+#define CN_BV_U 16
+__global__ void __launch_bounds__(32)
+k_batched_v_sweep(int64_t N, int64_t nsys, int64_t es, int64_t ss, double rho, cplx *__restrict__ psi,
+                  const cplx *__restrict__ q, const double *__restrict__ gam)
 {
+    constexpr int U = CN_BV_U;
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nsys) return;
     const int64_t o = k * ss;
@@ -660,20 +667,49 @@ __global__ void k_batched_v_sweep(int64_t N, int64_t nsys, int64_t es, int64_t s
     const cplx *qk = q + o;
     const double *gk = gam + o;
     const cplx zero = cmake(0.0, 0.0);
+    // Eq. 3 fused into the downward sweep: D_i = E_i - q_{i-1} D_{i-1}, D overwrites psi
     cplx lo = zero, cur = p[0], D = zero, qprev = zero;
-    for (int64_t i = 0; i < N; ++i) {
-        cplx hi = (i + 1 < N) ? p[(i + 1) * es] : zero;
-        cplx E = rhs_E(gk[i * es], rho, cur, lo, hi);
-        D = cfnma(qprev, D, E);
-        p[i * es] = D;
-        qprev = qk[i * es];
-        lo = cur;
-        cur = hi;
+    for (int64_t i0 = 0; i0 < N; i0 += U) {
+        cplx hv[U], qv[U];
+        double gv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t r = i0 + u;
+            hv[u] = (r + 1 < N) ? p[(r + 1) * es] : zero;
+            qv[u] = (r < N) ? qk[r * es] : zero;
+            gv[u] = (r < N) ? gk[r * es] : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t r = i0 + u;
+            if (r < N) {
+                const cplx E = rhs_E(gv[u], rho, cur, lo, hv[u]);
+                D = cfnma(qprev, D, E);
+                p[r * es] = D;
+                qprev = qv[u];
+                lo = cur;
+                cur = hv[u];
+            }
+        }
     }
+    // upward sweep + substitution: x_i = q_i (D_i - x_{i+1})
     cplx x = zero;
-    for (int64_t i = N - 1; i >= 0; --i) {
-        x = cmul(qk[i * es], csub(p[i * es], x));
-        p[i * es] = x;
+    for (int64_t i1 = N; i1 > 0; i1 -= U) {
+        cplx dv[U], qv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t r = i1 - 1 - u;
+            dv[u] = (r >= 0) ? p[r * es] : zero;
+            qv[u] = (r >= 0) ? qk[r * es] : zero;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int64_t r = i1 - 1 - u;
+            if (r >= 0) {
+                x = cmul(qv[u], csub(dv[u], x));
+                p[r * es] = x;
+            }
+        }
     }
 }
 
