@@ -64,6 +64,7 @@ struct cn_plan {
     int64_t *off0 = nullptr; // caller-placed joint lines of level 0 (cn_tridiag_create_blocks): group g = rows [off0[g], off0[g+1])
     int64_t noff0 = 0;       // number of such groups
     cplx *scratch0 = nullptr; // their reduction's scratch (the solution vector may alias the right-hand side)
+    bool off0_warp = false;   // every such group has at most CN_RS_G rows: the warp-per-group kernels take the offsets
     // configuration
     int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
     int opt_pdl = 1, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0, opt_rs_top_in_subst = 1, opt_keep_p = 0;
@@ -165,6 +166,7 @@ static void free_factors(cn_plan *p)
     p->gamJ = nullptr;
     p->off0 = nullptr;
     p->scratch0 = nullptr;
+    p->off0_warp = false;
     p->topX[0] = p->topX[1] = nullptr; p->gsub = p->gdiag = p->gsup = nullptr; p->diagAcc = nullptr;
     p->sh_local_done = false;
     for (int b = 0; b < cn_plan::NB; ++b) { p->bPsi[b] = nullptr; p->bQ[b] = nullptr; p->bV[b] = nullptr; }
@@ -975,19 +977,20 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase =
     const bool tg = p->opt_rs_group != CN_RS_G; // one thread per group of any size (paper-shaped, cn_reduced.cuh)
     // the last level is solved inside the substitution kernel of the level below it (one launch less per step)
     const bool tis = !tg && !sharded && p->opt_rs_top_in_subst && p->opt_rs_levels >= 0 && !p->opt_rs_serial_top &&
-                     nlv >= 2 && p->lv.back().n <= p->opt_rs_top_in_subst_max && !(p->off0 && nlv == 2);
+                     nlv >= 2 && p->lv.back().n <= p->opt_rs_top_in_subst_max && !(p->off0 && !p->off0_warp && nlv == 2);
     const int64_t G = p->opt_rs_group;
     for (int i = 0; i < nsep && e == cudaSuccess && phase != 2; ++i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        const int64_t *off = (i == 0) ? p->off0 : nullptr; // caller-placed joint lines: one thread per (ragged) block
-        if (tg || off)
+        const int64_t *off = (i == 0) ? p->off0 : nullptr; // caller-placed joint lines: ragged blocks
+        const bool offw = off && p->off0_warp;              // ... of at most 256 rows: one warp per block, else one thread
+        if (tg || (off && !offw))
             e = launch_k(k_rs_reduce_thread, (unsigned)((U.n + 63) / 64), 64u, 0, stream, pdl, L.n, G, (const cplx *)L.rD,
                          (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
                          (const cplx *)L.sup, (off && p->scratch0) ? p->scratch0 : L.X, U.rD, U.rU, off, p->noff0);
         else
         e = launch_k(k_rs_reduce, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
                      (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
-                     (const cplx *)L.sup, U.rD, U.rU, above);
+                     (const cplx *)L.sup, U.rD, U.rU, above, offw ? off : (const int64_t *)nullptr, p->noff0);
         p->launches += 1;
     }
     if (sharded && phase == 1 && e == cudaSuccess) { // the record of this step: JU guards of all levels + last-level rhs
@@ -1036,7 +1039,8 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase =
     for (int i = nsep - 1; i >= 0 && e == cudaSuccess; --i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
         const int64_t *off = (i == 0) ? p->off0 : nullptr;
-        if (tg || off)
+        const bool offw = off && p->off0_warp;
+        if (tg || (off && !offw))
             e = launch_k(k_rs_subst_thread, (unsigned)((U.n + 63) / 64), 64u, 0, stream, pdl, L.n, G, (const cplx *)L.rD,
                          (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X,
                          off, p->noff0);
@@ -1047,7 +1051,7 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase =
 #define CN_SUBST(KT) launch_k(k_rs_subst<KT>, gr, 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU, \
                               (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X, U.n,                 \
                               (const cplx *)U.rD, (const cplx *)U.rU, (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw, \
-                              Xabove)
+                              Xabove, offw ? off : (const int64_t *)nullptr, p->noff0)
             e = kt == 0 ? CN_SUBST(0) : (kt == 1 ? CN_SUBST(1) : (kt == 2 ? CN_SUBST(2) : (kt == 4 ? CN_SUBST(4) : CN_SUBST(8))));
 #undef CN_SUBST
         }
@@ -1343,7 +1347,12 @@ static cn_status tridiag_create_impl(cn_tridiag **out, int64_t N, const void *b,
     if (joints) {
         std::vector<int64_t> off((size_t)P + 1);
         off[0] = 0;
-        for (int64_t w = 0; w < P; ++w) off[(size_t)w + 1] = joints[w] + 1;
+        int64_t widest = 0;
+        for (int64_t w = 0; w < P; ++w) {
+            off[(size_t)w + 1] = joints[w] + 1;
+            if (off[(size_t)w + 1] - off[(size_t)w] > widest) widest = off[(size_t)w + 1] - off[(size_t)w];
+        }
+        p->off0_warp = widest <= CN_RS_G; // blocks of at most 256 rows: one warp per block; wider ones: one thread
         if ((st = dev_alloc(p, &p->off0, (size_t)P + 1)) != CN_OK) { cn_tridiag_destroy(t); return st; }
         if (cudaMemcpy(p->off0, off.data(), sizeof(int64_t) * ((size_t)P + 1), cudaMemcpyHostToDevice) != cudaSuccess) {
             cn_tridiag_destroy(t);
@@ -1390,13 +1399,16 @@ static cn_status tridiag_create_impl(cn_tridiag **out, int64_t N, const void *b,
     const int T = 128;
     for (int i = 0; i + 1 < nlv; ++i) {
         cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        if (i == 0 && joints)
+        if (i == 0 && joints && p->off0_warp)
+            k_rs_factor_level_smem<<<(unsigned)((U.n + CN_RS_FL_WARPS - 1) / CN_RS_FL_WARPS), 32 * CN_RS_FL_WARPS, 0, stream>>>(
+                L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr, 0, p->off0, p->noff0);
+        else if (i == 0 && joints)
             k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, (int64_t)CN_RS_G, L.sub, L.diag, L.sup, L.l,
                                                                              L.rp, L.u, tmpA, U.sub, U.diag, tmpB, U.sup,
                                                                              p->derr, p->off0, p->noff0);
         else
             k_rs_factor_level_smem<<<(unsigned)((U.n + CN_RS_FL_WARPS - 1) / CN_RS_FL_WARPS), 32 * CN_RS_FL_WARPS, 0, stream>>>(
-                L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr, 0);
+                L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr, 0, nullptr, 0);
         k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB, nullptr);
     }
     k_rs_factor_top_scan<<<1, 32, 0, stream>>>(p->lv.back().n, p->lv.back().sub, p->lv.back().diag, p->lv.back().sup, p->lw,

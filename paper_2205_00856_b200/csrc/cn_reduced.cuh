@@ -199,16 +199,18 @@ CN_DEVINL void rs_load_rows_n(const cplx *const (&src)[NA], const int (&lim)[NA]
 __global__ void __launch_bounds__(32 * CN_RS_WARPS)
 k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
             const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ sub,
-            const cplx *__restrict__ sup, cplx *__restrict__ outD, cplx *__restrict__ outU, int above = 0)
+            const cplx *__restrict__ sup, cplx *__restrict__ outD, cplx *__restrict__ outU, int above = 0,
+            const int64_t *__restrict__ off = nullptr, int64_t noff = 0)
 {   // above: the rows of a shard that another shard precedes (cn_shard.cuh): group 0 has a real joint line above it,
     // whose coupling sup[-1] and slot outU[-1] are the guard elements of the arrays
+    // off != NULL: caller-placed joint lines with blocks of at most CN_RS_G rows: group g = rows [off[g], off[g+1])
     constexpr int K = CN_RS_K;
     const int lane = threadIdx.x & 31;
-    const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
+    const int64_t ngroups = off ? noff : (n + CN_RS_G - 1) / CN_RS_G;
     const int64_t g = (int64_t)blockIdx.x * CN_RS_WARPS + (threadIdx.x >> 5);
     const bool live = g < ngroups; // whole warps only: the shuffles below stay convergent
-    const int64_t g0 = g * CN_RS_G;
-    const int ng = live ? (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G) : 0;
+    const int64_t g0 = !live ? 0 : (off ? off[g] : g * CN_RS_G);
+    const int ng = live ? (off ? (int)(off[g + 1] - g0) : (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G)) : 0;
     const int r0 = lane * K; // first row of this lane inside the group
     const cplx zero = cmake(0.0, 0.0);
     __shared__ cplx sbuf_all[CN_RS_WARPS][3 * CN_RS_G];
@@ -291,15 +293,17 @@ __global__ void __launch_bounds__(32 * CN_RS_WARPS)
 k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, const cplx *__restrict__ l,
            const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ Xup,
            cplx *__restrict__ X, int64_t ntop, const cplx *topD, const cplx *topU, const cplx *__restrict__ lw,
-           const cplx *__restrict__ rq, const cplx *__restrict__ uw, const cplx *Xabove = nullptr)
+           const cplx *__restrict__ rq, const cplx *__restrict__ uw, const cplx *Xabove = nullptr,
+           const int64_t *__restrict__ off = nullptr, int64_t noff = 0)
 {   // Xabove (KT == 0 only): support value of the joint line above group 0 when a shard precedes this one (cn_shard.cuh)
+    // off: caller-placed joint lines (see k_rs_reduce)
     constexpr int K = CN_RS_K;
     const int lane = threadIdx.x & 31;
-    const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
+    const int64_t ngroups = off ? noff : (n + CN_RS_G - 1) / CN_RS_G;
     const int64_t g = (int64_t)blockIdx.x * CN_RS_WARPS + (threadIdx.x >> 5);
     const bool live = g < ngroups;
-    const int64_t g0 = g * CN_RS_G;
-    const int ng = live ? (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G) : 0;
+    const int64_t g0 = !live ? 0 : (off ? off[g] : g * CN_RS_G);
+    const int ng = live ? (off ? (int)(off[g + 1] - g0) : (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G)) : 0;
     const int r0 = lane * K;
     const cplx zero = cmake(0.0, 0.0);
     __shared__ cplx sbuf_all[CN_RS_WARPS][3 * CN_RS_G];
@@ -575,17 +579,19 @@ __global__ void __launch_bounds__(32 * CN_RS_FL_WARPS)
 k_rs_factor_level_smem(int64_t n, const cplx *__restrict__ sub, const cplx *__restrict__ diag,
                        const cplx *__restrict__ sup, cplx *__restrict__ l, cplx *__restrict__ rp, cplx *__restrict__ u,
                        cplx *__restrict__ sub2, cplx *__restrict__ diag2, cplx *__restrict__ diag2U,
-                       cplx *__restrict__ sup2, int *__restrict__ err, int above = 0)
+                       cplx *__restrict__ sup2, int *__restrict__ err, int above = 0,
+                       const int64_t *__restrict__ off = nullptr, int64_t noff = 0)
 {   // above (cn_shard.cuh): group 0 is treated like any later group; its JU matrix side goes to the guards [-1]
+    // off: caller-placed joint lines with blocks of at most CN_RS_G rows (see k_rs_reduce)
     constexpr int K = CN_RS_K;
     __shared__ cplx sbuf_all[CN_RS_FL_WARPS][3 * CN_RS_G];
     const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
     cplx *const sbuf = sbuf_all[wp];
-    const int64_t ngroups = (n + CN_RS_G - 1) / CN_RS_G;
+    const int64_t ngroups = off ? noff : (n + CN_RS_G - 1) / CN_RS_G;
     const int64_t g = (int64_t)blockIdx.x * CN_RS_FL_WARPS + wp;
     if (g >= ngroups) return; // whole warps
-    const int64_t g0 = g * CN_RS_G;
-    const int ng = (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G);
+    const int64_t g0 = off ? off[g] : g * CN_RS_G;
+    const int ng = off ? (int)(off[g + 1] - g0) : (int)((n - g0 < CN_RS_G) ? (n - g0) : CN_RS_G);
     const int nj = ng - 1; // interior rows; row nj is the joint line
     const int r0 = lane * K;
     const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
