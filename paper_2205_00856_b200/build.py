@@ -10,7 +10,7 @@ CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libcn_nshape.so")
 SOURCES = ["cn_api.cu"]
 HEADERS = ["cn_common.cuh", "cn_factor.cuh", "cn_pass_generic.cuh", "cn_pass_tiled.cuh", "cn_reduced.cuh",
-           "cn_batched.cuh", "cn_onchip.cuh", os.path.join("..", "..", "include", "cn_nshape.h")]
+           "cn_batched.cuh", "cn_onchip.cuh", "cn_shard.cuh", os.path.join("..", "..", "include", "cn_nshape.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--threads", "4", "-diag-suppress", "550"]
 
