@@ -261,6 +261,20 @@ cn_status cn_shard_prologue(cn_plan *plan, void *psi, const void *edges_all, voi
 cn_status cn_shard_advance(cn_plan *plan, void *psi, const void *step_all, void *step_send, void *stream);
 cn_status cn_shard_epilogue(cn_plan *plan, void *psi, const void *step_all, void *stream);
 
+/*
+ * The same protocol driven by the library, one shard per process (or thread): the plan owns the records and calls
+ * `exchange` wherever a gather is due.  exchange(ctx, send, recv, count, stream) must ENQUEUE on `stream` an all-gather
+ * of `count` complex128 values per shard -- send: this shard's record, recv: nshards records in rank order, both DEVICE
+ * pointers owned by the plan -- and return CN_OK (e.g. one ncclAllGather of 2 * count doubles); any other status aborts
+ * the call and is returned.  It is not called when nshards = 1.
+ *   cn_shard_factorize : cn_shard_factorize_local -> exchange -> cn_shard_factorize_finish (synchronises twice).
+ *   cn_shard_run       : nsteps steps of this shard's rows: nsteps + 1 exchanges, no synchronisation,
+ *                        no allocation after the first call.
+ */
+typedef cn_status (*cn_exchange_fn)(void *ctx, const void *send, void *recv, int64_t count, void *stream);
+cn_status cn_shard_factorize(cn_plan *plan, cn_exchange_fn exchange, void *ctx, void *stream);
+cn_status cn_shard_run(cn_plan *plan, void *psi, int64_t nsteps, cn_exchange_fn exchange, void *ctx, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

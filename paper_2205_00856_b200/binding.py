@@ -24,7 +24,12 @@ EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", 
            "cn_tridiag_create", "cn_tridiag_solve", "cn_tridiag_destroy",
            "cn_tridiag_create_blocks", "cn_plan_set_systems", "cn_batched_sweep_v",
            "cn_shard_plan_create", "cn_shard_counts", "cn_shard_factorize_local", "cn_shard_factorize_finish",
-           "cn_shard_edge", "cn_shard_prologue", "cn_shard_advance", "cn_shard_epilogue"]
+           "cn_shard_edge", "cn_shard_prologue", "cn_shard_advance", "cn_shard_epilogue",
+           "cn_shard_factorize", "cn_shard_run"]
+
+# cn_exchange_fn: cn_status (*)(void *ctx, const void *send, void *recv, int64_t count, void *stream)
+EXCHANGE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
+                               ctypes.c_void_p)
 
 
 class CnError(RuntimeError):
@@ -90,6 +95,10 @@ def lib():
                         ("cn_shard_prologue", 5), ("cn_shard_advance", 5), ("cn_shard_epilogue", 4)):
             getattr(L, name).restype = i32
             getattr(L, name).argtypes = [vp] * n
+        L.cn_shard_factorize.restype = i32
+        L.cn_shard_factorize.argtypes = [vp, EXCHANGE_FN, vp, vp]
+        L.cn_shard_run.restype = i32
+        L.cn_shard_run.argtypes = [vp, vp, i64, EXCHANGE_FN, vp, vp]
         L.cn_destroy.restype = i32
         L.cn_destroy.argtypes = [vp]
         L.cn_plan_get_info.restype = i32
@@ -287,6 +296,26 @@ class ShardPlan:
 
     def epilogue(self, psi, step_all, stream=None):
         _check(self.h, lib().cn_shard_epilogue(self.h, _ptr(psi), _ptr(step_all), _stream(stream)), "cn_shard_epilogue")
+
+    # the same protocol driven by the library: `exchange` is a Python callable (send_ptr, recv_ptr, count, stream_ptr)
+    # that enqueues the all-gather of `count` complex128 values per shard and returns CN_OK
+    def _wrap(self, exchange):
+        def cb(ctx, send, recv, count, stream):
+            try:
+                return int(exchange(send, recv, count, stream) or CN_OK)
+            except Exception:  # an exception must not unwind through the C frames
+                import traceback
+                traceback.print_exc()
+                return CN_ECUDA
+        return EXCHANGE_FN(cb)
+
+    def factorize(self, exchange, stream=None):
+        fn = self._wrap(exchange)
+        _check(self.h, lib().cn_shard_factorize(self.h, fn, None, _stream(stream)), "cn_shard_factorize")
+
+    def run(self, psi, nsteps, exchange, stream=None):
+        fn = self._wrap(exchange)
+        _check(self.h, lib().cn_shard_run(self.h, _ptr(psi), nsteps, fn, None, _stream(stream)), "cn_shard_run")
 
     def info(self):
         return cn_plan_get_info(self.h)

@@ -87,6 +87,7 @@ struct cn_plan {
     cplx *diagAcc = nullptr;           // what this shard adds to the diagonal of the row above it, summed over the levels
     int sh_out = 1;                    // sup[] / topX[] buffer the pending RS writes
     bool sh_local_done = false;        // cn_shard_factorize_local has run, cn_shard_factorize_finish is due
+    cplx *xbuf = nullptr;              // send / receive records of cn_shard_factorize / cn_shard_run
     // profiling (CN_OPT_PROFILE): event pairs around fused-pass (kind 0) and RS (kind 1) launches
     struct ev_pair { cudaEvent_t a, b; int kind; };
     std::vector<ev_pair> ev_pool;
@@ -226,6 +227,7 @@ extern "C" cn_status cn_destroy(cn_plan *plan)
     if (plan->tdG) cudaFree(plan->tdG);
     if (plan->tdV) cudaFree(plan->tdV);
     if (plan->tdRed) cudaFree(plan->tdRed);
+    if (plan->xbuf) cudaFree(plan->xbuf);
     if (plan->hV) cudaFreeHost(plan->hV);
     if (plan->sIn) cudaStreamDestroy(plan->sIn);
     if (plan->sCmp) cudaStreamDestroy(plan->sCmp);
@@ -1811,4 +1813,71 @@ extern "C" cn_status cn_shard_epilogue(cn_plan *p, void *psi_, const void *step_
         if ((st = launch_rs(p, p->sh_out, stream, 2, (cplx *)step_all)) != CN_OK) return st;
     }
     return launch_pass(p, (cplx *)psi_, 2, p->sh_out, stream);
+}
+
+// ---- the same protocol driven by the library, the exchange left to a callback (one shard per process / thread) ------------
+// send / recv records are device buffers the plan owns (allocated once, here); the callback enqueues an all-gather of
+// `count` complex128 values per shard, in rank order, on `stream` and returns CN_OK.
+struct cn_shard_bufs {
+    cplx *msend = nullptr, *mrecv = nullptr, *esend = nullptr, *erecv = nullptr, *ssend[2] = {nullptr, nullptr}, *srecv = nullptr;
+};
+
+static cn_status shard_buffers(cn_plan *p, cn_shard_bufs *b)
+{
+    int64_t mc = 0, sc = 0;
+    cn_status st = cn_shard_counts(p, &mc, &sc);
+    if (st != CN_OK) return st;
+    const size_t S = (size_t)p->nshards;
+    if (!p->xbuf) {
+        const size_t total = (size_t)mc * (1 + S) + (1 + S) + (size_t)sc * (2 + S);
+        CN_CUDA(p, cudaMalloc((void **)&p->xbuf, sizeof(cplx) * total));
+        CN_CUDA(p, cudaMemset(p->xbuf, 0, sizeof(cplx) * total));
+    }
+    cplx *q = p->xbuf;
+    b->msend = q; q += mc;
+    b->mrecv = q; q += (size_t)mc * S;
+    b->esend = q; q += 1;
+    b->erecv = q; q += S;
+    b->ssend[0] = q; q += sc;
+    b->ssend[1] = q; q += sc;
+    b->srecv = q;
+    return CN_OK;
+}
+
+extern "C" cn_status cn_shard_factorize(cn_plan *p, cn_exchange_fn exchange, void *ctx, void *stream)
+{
+    if (!p || (p->nshards > 1 && !exchange)) return CN_EINVAL;
+    if (p->xbuf) { cudaFree(p->xbuf); p->xbuf = nullptr; } // options may have changed the record sizes
+    cn_shard_bufs b;
+    cn_status st = shard_buffers(p, &b);
+    if (st != CN_OK) return st;
+    int64_t mc = 0, sc = 0;
+    cn_shard_counts(p, &mc, &sc);
+    if ((st = cn_shard_factorize_local(p, b.msend, stream)) != CN_OK) return st;
+    if (p->nshards > 1 && (st = exchange(ctx, b.msend, b.mrecv, mc, stream)) != CN_OK) return st;
+    return cn_shard_factorize_finish(p, b.mrecv, stream);
+}
+
+extern "C" cn_status cn_shard_run(cn_plan *p, void *psi, int64_t nsteps, cn_exchange_fn exchange, void *ctx, void *stream)
+{
+    if (!p || !psi || nsteps < 0 || (p->nshards > 1 && !exchange)) return CN_EINVAL;
+    if (!p->factorized) return CN_ENOTFACTORIZED;
+    if (nsteps == 0) return CN_OK;
+    cn_shard_bufs b;
+    cn_status st = shard_buffers(p, &b);
+    if (st != CN_OK) return st;
+    int64_t mc = 0, sc = 0;
+    cn_shard_counts(p, &mc, &sc);
+    const bool many = p->nshards > 1;
+    if (many) {
+        if ((st = cn_shard_edge(p, psi, b.esend, stream)) != CN_OK) return st;
+        if ((st = exchange(ctx, b.esend, b.erecv, 1, stream)) != CN_OK) return st;
+    }
+    if ((st = cn_shard_prologue(p, psi, b.erecv, b.ssend[0], stream)) != CN_OK) return st;
+    for (int64_t k = 1; k <= nsteps; ++k) {
+        if (many && (st = exchange(ctx, b.ssend[(k - 1) & 1], b.srecv, sc, stream)) != CN_OK) return st;
+        st = (k < nsteps) ? cn_shard_advance(p, psi, b.srecv, b.ssend[k & 1], stream) : cn_shard_epilogue(p, psi, b.srecv, stream);
+        if (st != CN_OK) return st;
+    }
+    return CN_OK;
 }

@@ -145,3 +145,66 @@ def test_rejects_unequal_shards_and_wrong_calls():
     with pytest.raises(B.CnError) as e:
         B.ShardPlan(1000, 4, cfg.dx, cfg.dt, V[:1000], 0, 2)  # N_local must be a multiple of 256
     assert e.value.status == B.CN_EINVAL
+
+
+def test_callback_driven_run_threads():
+    """cn_shard_factorize / cn_shard_run: the library drives the protocol and calls back for every exchange.  Four
+    shards of one system, ONE HOST THREAD AND ONE STREAM PER SHARD on the single device (as four ranks would run); the
+    callback emulates the all-gather with device copies into a shared buffer, events and a host barrier.  Against the
+    oracle on the whole system."""
+    import threading
+    torch = torch_()
+    from cuda.bindings import runtime as rt
+    S, nsteps = 4, 9
+    cfg = W.scaled(W.CONFIGS["C2dense"], N=1 << 19)
+    V, psi = W.potential(cfg), W.psi0(cfg)
+    ref = O.step(cfg.dx, cfg.dt, V, psi, nsteps)
+    n = cfg.N // S
+    maxc = 8192
+    G = [torch.zeros(S * maxc, dtype=torch.complex128, device="cuda") for _ in range(2)]  # shared gather buffers (ping-pong)
+    ev = [[torch.cuda.Event() for _ in range(2)] for _ in range(S)]
+    bar = threading.Barrier(S)
+    parts, errors = [None] * S, []
+
+    def worker(r):
+        try:
+            torch.cuda.set_device(0)
+            stream = torch.cuda.Stream()
+            calls = [0]
+
+            def exchange(send, recv, count, stream_ptr):
+                idx = calls[0] & 1
+                calls[0] += 1
+                nb = 16 * count
+                assert count <= maxc and stream_ptr == stream.cuda_stream
+                e, = rt.cudaMemcpyAsync(G[idx].data_ptr() + r * nb, send, nb, rt.cudaMemcpyKind.cudaMemcpyDeviceToDevice, stream_ptr)
+                assert e == rt.cudaError_t.cudaSuccess
+                ev[r][idx].record(stream)
+                bar.wait()                      # every shard has enqueued its contribution and recorded its event
+                for k in range(S):
+                    stream.wait_event(ev[k][idx])
+                e, = rt.cudaMemcpyAsync(recv, G[idx].data_ptr(), S * nb, rt.cudaMemcpyKind.cudaMemcpyDeviceToDevice, stream_ptr)
+                assert e == rt.cudaError_t.cudaSuccess
+                bar.wait()                      # every shard has enqueued its waits: the events may be recorded again
+                return B.CN_OK
+
+            with torch.cuda.stream(stream):
+                d = torch.from_numpy(psi[r * n:(r + 1) * n].copy()).cuda()
+                with B.ShardPlan(n, n // 256, cfg.dx, cfg.dt, V[r * n:(r + 1) * n], r, S, rs_topmax=16) as plan:
+                    plan.factorize(exchange, stream)
+                    plan.run(d, 4, exchange, stream)
+                    plan.run(d, nsteps - 4, exchange, stream)
+                    stream.synchronize()
+                parts[r] = d.cpu().numpy()
+        except Exception as ex:  # pragma: no cover
+            errors.append((r, repr(ex)))
+            bar.abort()
+
+    threads = [threading.Thread(target=worker, args=(r,)) for r in range(S)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join(timeout=300)
+    assert not errors, errors
+    out = np.concatenate(parts)
+    assert np.max(np.abs(out - ref)) <= TOL_PSI
