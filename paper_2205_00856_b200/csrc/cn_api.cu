@@ -1160,7 +1160,7 @@ extern "C" cn_status cn_step(cn_plan *p, void *psi_, int64_t nsteps, void *strea
         for (int64_t k = 0; k < nsteps; ++k) {
             cudaError_t e = launch_k(k_batched_v_sweep, (unsigned)((p->sysCount + T - 1) / T), (unsigned)T, 0, stream, false,
                                      p->sysN, p->sysCount, p->sysEs, p->sysSs, p->rho, psi, (const cplx *)p->q,
-                                     (const double *)p->gam);
+                                     (const double *)p->gam, p->sysEs, p->sysSs);
             p->launches += 1;
             if (e != cudaSuccess) return cuda_fail(p, e);
         }
@@ -1638,10 +1638,10 @@ extern "C" cn_status cn_batched_sweep(cn_plan *p, void *psi_, int64_t nsys, int6
             p->launches += 1;
         }
     } else {
-        const int T = 64;
+        const int T = 32;
         for (int64_t s = 0; s < nsteps && e == cudaSuccess; ++s) {
-            e = launch_k(k_batched_generic, (unsigned)((nsys + T - 1) / T), T, 0, stream, pdl, N, nsys, es, ss, p->rho, psi,
-                         (const cplx *)p->qB, (const double *)p->gam);
+            e = launch_k(k_batched_v_sweep, (unsigned)((nsys + T - 1) / T), (unsigned)T, 0, stream, pdl, N, nsys, es, ss, p->rho,
+                         psi, (const cplx *)p->qB, (const double *)p->gam, (int64_t)1, (int64_t)0);
             p->launches += 1;
         }
     }

@@ -21,7 +21,8 @@
 //                systems is 128 B wide; thread (g, c) owns 16 rows of column c, so global accesses are
 //                whole lines without any transposition.  The strip arrives by TMA (prefetched one strip
 //                ahead), the new psi leaves by 128-bit stores straight from registers.
-//   k_batched_generic  any N, any strides: one thread per system, in-place serial sweeps (correctness path).
+//   k_batched_v_sweep  any N, any strides: one thread per system, in-place serial sweeps (correctness path; also the
+//                sweep of systems with a matrix of their own each, cn_plan_set_systems).
 #pragma once
 #include <cuda.h>
 #include "cn_common.cuh"
@@ -597,33 +598,6 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
     }
 }
 
-// ---- correctness path: one thread per system, in place, any N and any strides -------------------------
-__global__ void k_batched_generic(int64_t N, int64_t nsys, int64_t es, int64_t ss, double rho, cplx *__restrict__ psi,
-                                  const cplx *__restrict__ qB, const double *__restrict__ gam)
-{
-    pdl_wait();
-    pdl_launch_dependents();
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= nsys) return;
-    cplx *p = psi + k * ss;
-    const cplx zero = cmake(0.0, 0.0);
-    cplx lo = zero, cur = p[0], D = zero, qprev = zero;
-    for (int64_t i = 0; i < N; ++i) {
-        cplx hi = (i + 1 < N) ? p[(i + 1) * es] : zero;
-        cplx E = rhs_E(gam[i], rho, cur, lo, hi);
-        D = cfnma(qprev, D, E); // RD on d (Eq. 11); D overwrites psi_i, no longer needed
-        p[i * es] = D;
-        qprev = qB[i];
-        lo = cur;
-        cur = hi;
-    }
-    cplx x = zero;
-    for (int64_t i = N - 1; i >= 0; --i) {
-        x = cmul(qB[i], csub(p[i * es], x));
-        p[i * es] = x;
-    }
-}
-
 // ---- systems with a potential of their own each (cn_plan_set_systems), any dense layout: one thread per system ------
 // Row i of system k lives at [k ss + i es] in V, q, gamma and psi alike.  Factor side: gamma and the
 // inverse pivots of the downward elimination of every system (one block per system); d side: Eq. 3
@@ -655,17 +629,19 @@ __global__ void k_batched_v_factor(int64_t N, int64_t nsys, int64_t es, int64_t 
 // arrays in flight instead of one -- the difference between a latency-bound and a bandwidth-bound sweep when there are
 // only a few thousand systems.
 #define CN_BV_U 16
+// qes / qss: strides of q and gamma (es / ss for systems with a matrix of their own; 1 / 0 for a shared matrix).
 __global__ void __launch_bounds__(32)
 k_batched_v_sweep(int64_t N, int64_t nsys, int64_t es, int64_t ss, double rho, cplx *__restrict__ psi,
-                  const cplx *__restrict__ q, const double *__restrict__ gam)
+                  const cplx *__restrict__ q, const double *__restrict__ gam, int64_t qes, int64_t qss)
 {
     constexpr int U = CN_BV_U;
+    pdl_wait();
+    pdl_launch_dependents();
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nsys) return;
-    const int64_t o = k * ss;
-    cplx *p = psi + o;
-    const cplx *qk = q + o;
-    const double *gk = gam + o;
+    cplx *p = psi + k * ss;
+    const cplx *qk = q + k * qss;
+    const double *gk = gam + k * qss;
     const cplx zero = cmake(0.0, 0.0);
     // Eq. 3 fused into the downward sweep: D_i = E_i - q_{i-1} D_{i-1}, D overwrites psi
     cplx lo = zero, cur = p[0], D = zero, qprev = zero;
@@ -676,8 +652,8 @@ k_batched_v_sweep(int64_t N, int64_t nsys, int64_t es, int64_t ss, double rho, c
         for (int u = 0; u < U; ++u) {
             const int64_t r = i0 + u;
             hv[u] = (r + 1 < N) ? p[(r + 1) * es] : zero;
-            qv[u] = (r < N) ? qk[r * es] : zero;
-            gv[u] = (r < N) ? gk[r * es] : 0.0;
+            qv[u] = (r < N) ? qk[r * qes] : zero;
+            gv[u] = (r < N) ? gk[r * qes] : 0.0;
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
@@ -700,7 +676,7 @@ k_batched_v_sweep(int64_t N, int64_t nsys, int64_t es, int64_t ss, double rho, c
         for (int u = 0; u < U; ++u) {
             const int64_t r = i1 - 1 - u;
             dv[u] = (r >= 0) ? p[r * es] : zero;
-            qv[u] = (r >= 0) ? qk[r * es] : zero;
+            qv[u] = (r >= 0) ? qk[r * qes] : zero;
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
