@@ -202,18 +202,22 @@ def p_sweep(torch, peak, name="C2dense"):
     V, psi = _inputs(cfg)
     d = torch.from_numpy(psi).cuda()
     rows = []
-    arms = (("tiled", dict(keep_p=1)), ("paper_shape", dict(path=B.PATH_GENERIC, rs_levels=-1)),
+    arms = (("tiled_default", dict()),          # the library partitions the system itself (P is a hint): flat in P by construction
+            ("tiled_keep_p", dict(keep_p=1)),   # the caller's blocks on the tiled kernels (blocks of at most 4096 rows fit a CTA tile)
+            ("paper_shape", dict(path=B.PATH_GENERIC, rs_levels=-1)),
             ("generic_nested_rs", dict(path=B.PATH_GENERIC)))
     for arm, opts in arms:
         for Pk in cfg.P_sweep:
+            if arm == "tiled_keep_p" and cfg.N // Pk > 4096:
+                continue  # such blocks do not fit a tile: CN_OPT_KEEP_P would run them on the thread-per-block kernels (= generic_nested_rs)
             with B.Plan(cfg.N, Pk, cfg.dx, cfg.dt, V, **opts) as plan:
                 plan.factorize()
                 info = plan.info()
-                best, med = time_plan(torch, plan, d, 20 if arm == "tiled" else 3, reps=3)
+                best, med = time_plan(torch, plan, d, 20 if arm.startswith("tiled") else 3, reps=3)
             rows.append({"arm": arm, "P": Pk, "P_effective": info["P_effective"], "rs_levels": info["rs_levels"],
-                         "us_per_cn_step": 1e3 * best})
+                         "path": info["path"], "us_per_cn_step": 1e3 * best})
     fits = {}
-    for arm, _ in arms:
+    for arm in ("paper_shape", "generic_nested_rs"):  # (the tiled arms are flat / not of the model's shape: not fitted)
         Ps = np.array([r["P"] for r in rows if r["arm"] == arm], float)
         ts = np.array([r["us_per_cn_step"] for r in rows if r["arm"] == arm], float)
         A = np.stack([cfg.N / Ps, Ps, np.ones_like(Ps)], 1)
