@@ -234,9 +234,10 @@ cn_status cn_tridiag_destroy(cn_tridiag *t);
  *   - once per (H, dt), the matrix side:  cn_shard_factorize_local writes this shard's record of
  *     `matrix_count` values, cn_shard_factorize_finish reads the nshards records and factors the last RS level of the
  *     whole system, replicated on every shard (no root process; PAPER.md:207 names the alternative);
- *   - per step, the d side: a record of `step_count` = nt + 1 values -- the JU contribution to the last row of the
- *     preceding shard and the right-hand sides of this shard's nt last-level rows; with nt = 1 these are the two
- *     values per process of PAPER.md:175 for a pre-factored matrix.  The two support values a process gets back
+ *   - per step, the d side: a record of `step_count` = 2 nt values -- the two right-hand-side slots of this shard's
+ *     nt last-level rows, written in place by the kernels (nothing is packed), one of them the JU
+ *     contribution to the last row of the preceding shard; with nt = 1 these are the two values per process of
+ *     PAPER.md:175 for a pre-factored matrix.  The two support values a process gets back
  *      are computed locally from the gathered records;
  *   - once per run, psi^0 on the last row of every shard (1 value; cn_shard_edge), which the first explicit half-step
  *     of the next shard needs (Eq. 3).

@@ -933,7 +933,8 @@ static cn_status launch_pass(cn_plan *p, cplx *psi, int mode, int cur, cudaStrea
             prm.supOld -= 1; prm.supNew -= 1; prm.slotD -= 1; prm.slotU -= 1; prm.supInit -= 1;
             prm.P += 1;
         }
-        if (p->below) prm.P = 0; // the last block of this shard is not the last block of the system
+        if (p->nshards > 1) prm.P = 0; // no block of a shard clears slotU of "the last joint line": that slot belongs to the
+                                       // next shard (or, on the last shard, stays at the 0 of the factorization)
         tiled_kernel_t k = tiled_kernel(p->tpb, p->logc, mode);
         e = launch_k(k, (unsigned)p->grid_tiled, (unsigned)p->tpb, tiled_smem(p->tpb), stream, pdl, p->tmPsi, p->tmQ,
                      p->tmGam, prm);
@@ -995,23 +996,18 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase =
                      (const cplx *)L.sup, U.rD, U.rU, above, offw ? off : (const int64_t *)nullptr, p->noff0);
         p->launches += 1;
     }
-    if (sharded && phase == 1 && e == cudaSuccess) { // the record of this step: JU guards of all levels + last-level rhs
-        cn_shard_guards gs;
-        gs.n = nlv;
-        for (int i = 0; i < nlv; ++i) gs.g[i] = p->lv[i].rU - 1;
-        const cn_plan::rs_level &L = p->lv.back();
-        e = launch_k(k_shard_pack_step, (unsigned)((p->nt + 127) / 128), 128u, 0, stream, pdl, p->nt, (const cplx *)L.rD,
-                     (const cplx *)L.rU, gs, above, rec);
-        p->launches += 1;
-    }
+    // (sharded, phase 1: the last level's right-hand-side slots ARE the record to send, shard_bind_record; nothing to pack)
     if (phase == 1) {
         prof_end(p, pi, stream);
         return e == cudaSuccess ? CN_OK : cuda_fail(p, e);
     }
-    if (sharded && e == cudaSuccess) {
-        // RS of the whole last level, replicated; launched WITHOUT programmatic serialization: the kernel before it on
-        // the stream is the caller's exchange, which must be complete
-        const int64_t n = (int64_t)p->nshards * p->nt;
+    // sharded: RS of the whole last level (nshards * nt rows), replicated, from the gathered records `rec`; inside the
+    // substitution kernel of the level below when it is small enough, else by k_shard_top.  Whichever kernel comes first
+    // is launched WITHOUT programmatic serialization: the work before it on the stream is the caller's exchange.
+    const int64_t ntopS = (int64_t)p->nshards * p->nt;
+    const bool stis = sharded && nlv >= 2 && p->opt_rs_top_in_subst && ntopS <= 1024;
+    if (sharded && !stis && e == cudaSuccess) {
+        const int64_t n = ntopS;
         cplx *guard0 = (above && nlv >= 2) ? p->sup[out] - 1 : nullptr;
         int T = CN_RS_TOP_THREADS;
 #define CN_STOP(K)                                                                                                     \
@@ -1049,11 +1045,18 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase =
         else {
             const unsigned gr = (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS);
             const int64_t T = 32 * CN_RS_WARPS;
-            const int kt = (tis && i == nlv - 2) ? (U.n <= T ? 1 : (U.n <= 2 * T ? 2 : (U.n <= 4 * T ? 4 : 8))) : 0;
-#define CN_SUBST(KT) launch_k(k_rs_subst<KT>, gr, 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD, (const cplx *)L.rU, \
-                              (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X, U.n,                 \
+            const bool top_here = (tis || stis) && i == nlv - 2;        // the last level is solved inside this launch
+            const int64_t ntop = stis ? ntopS : U.n;
+            const int kt = top_here ? (ntop <= T ? 1 : (ntop <= 2 * T ? 2 : (ntop <= 4 * T ? 4 : 8))) : 0;
+            cplx *guardOut = (sharded && above && i == 0) ? p->sup[out] - 1 : nullptr; // level 0 leaves X of the row above
+            const cplx *gath = (stis && top_here) ? (const cplx *)rec : nullptr;
+            cplx *xaboveOut = (stis && top_here && above) ? p->topX[out] + toff - 1 : nullptr;
+            const bool pdl_here = pdl && !(stis && top_here);         // (first kernel after the caller's exchange)
+#define CN_SUBST(KT) launch_k(k_rs_subst<KT>, gr, 32u * CN_RS_WARPS, 0, stream, pdl_here, L.n, (const cplx *)L.rD, (const cplx *)L.rU, \
+                              (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X, ntop,                \
                               (const cplx *)U.rD, (const cplx *)U.rU, (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw, \
-                              Xabove, offw ? off : (const int64_t *)nullptr, p->noff0)
+                              Xabove, offw ? off : (const int64_t *)nullptr, p->noff0, guardOut, gath, (int64_t)p->nshards,          \
+                              stis ? toff : (int64_t)0, xaboveOut)
             e = kt == 0 ? CN_SUBST(0) : (kt == 1 ? CN_SUBST(1) : (kt == 2 ? CN_SUBST(2) : (kt == 4 ? CN_SUBST(4) : CN_SUBST(8))));
 #undef CN_SUBST
         }
@@ -1703,7 +1706,7 @@ extern "C" cn_status cn_shard_counts(const cn_plan *p, int64_t *matrix_count, in
     int64_t Peff = 0, nt = 0;
     choose_partition(p, &Peff, &nt);
     *matrix_count = CN_SHARD_MREC(nt);
-    *step_count = nt + 1;
+    *step_count = 2 * nt;
     return CN_OK;
 }
 
@@ -1756,6 +1759,18 @@ static cn_status shard_map_psi(cn_plan *p, void *psi_)
     return st;
 }
 
+// The right-hand-side slots of the shard's last RS level live in the record to send (layout: shard_rhs, cn_shard.cuh)
+static void shard_bind_record(cn_plan *p, cplx *rec)
+{
+    cn_plan::rs_level &T = p->lv.back();
+    T.rD = rec;
+    T.rU = rec + p->nt + 1; // rU[-1] = rec[nt]: the guard
+    if (p->lv.size() == 1) { // level 0 is the last level: the pass kernel writes the record
+        p->slotD = T.rD;
+        p->slotU = T.rU;
+    }
+}
+
 extern "C" cn_status cn_shard_prologue(cn_plan *p, void *psi_, const void *edges_all, void *step_send, void *stream_)
 {
     if (!p || !psi_ || (((uintptr_t)psi_) & 15) != 0) return CN_EINVAL;
@@ -1773,6 +1788,7 @@ extern "C" cn_status cn_shard_prologue(cn_plan *p, void *psi_, const void *edges
     if (p->above) // psi^0 on the last row of the preceding shard: the old value of "the joint line above" for block 0
         CN_CUDA(p, cudaMemcpyAsync(p->sup[0] - 1, (const cplx *)edges_all + (p->shard - 1), sizeof(cplx),
                                    cudaMemcpyDeviceToDevice, stream));
+    shard_bind_record(p, (cplx *)step_send);
     if ((st = launch_pass(p, (cplx *)psi_, 0, /*cur=*/1, stream)) != CN_OK) return st;
     p->sh_out = 1;
     return launch_rs(p, p->sh_out, stream, 1, (cplx *)step_send);
@@ -1794,6 +1810,7 @@ extern "C" cn_status cn_shard_advance(cn_plan *p, void *psi_, const void *step_a
     if (!step_all || !step_send) return CN_EINVAL;
     if ((st = launch_rs(p, p->sh_out, stream, 2, (cplx *)step_all)) != CN_OK) return st;
     const int cur = p->sh_out;
+    shard_bind_record(p, (cplx *)step_send);
     if ((st = launch_pass(p, (cplx *)psi_, 1, cur, stream)) != CN_OK) return st;
     p->sh_out = cur ^ 1;
     return launch_rs(p, p->sh_out, stream, 1, (cplx *)step_send);

@@ -24,6 +24,8 @@
 #include "cn_common.cuh"
 #include "cn_factor.cuh" // cn_mob
 
+CN_DEVINL cplx shard_rhs(const cplx *gathered, int64_t S, int64_t nt, int64_t w); // cn_shard.cuh (sharded last level)
+
 #define CN_RS_G 256          // joint lines per group
 #define CN_RS_TOP_THREADS 1024
 
@@ -280,7 +282,11 @@ k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
     yN = shfl_c(yN, ng > 1 ? (ng - 2) / K : 0);
     if (live && lane == 0) {
         outD[g] = (ng >= 2) ? cfnma(subJ, yN, Rj) : Rj;                        // JD
-        if (g > 0 || above) outU[g - 1] = (ng >= 2) ? cneg(cmul(supAbove, y0)) : zero; // JU
+        if (g > 0 || above) {
+            cplx ju = (ng >= 2) ? cneg(cmul(supAbove, y0)) : zero; // JU
+            if (g == 0) ju = cadd(ju, ld_dep(rU - 1)); // (a shard's first group) the guard of this level rides along
+            outU[g - 1] = ju;
+        }
     }
 }
 
@@ -294,9 +300,14 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
            const cplx *__restrict__ rp, const cplx *__restrict__ u, const cplx *__restrict__ Xup,
            cplx *__restrict__ X, int64_t ntop, const cplx *topD, const cplx *topU, const cplx *__restrict__ lw,
            const cplx *__restrict__ rq, const cplx *__restrict__ uw, const cplx *Xabove = nullptr,
-           const int64_t *__restrict__ off = nullptr, int64_t noff = 0)
+           const int64_t *__restrict__ off = nullptr, int64_t noff = 0, cplx *guardOut = nullptr,
+           const cplx *gathered = nullptr, int64_t nshards = 1, int64_t toff = 0, cplx *xaboveOut = nullptr)
 {   // Xabove (KT == 0 only): support value of the joint line above group 0 when a shard precedes this one (cn_shard.cuh)
     // off: caller-placed joint lines (see k_rs_reduce)
+    // guardOut: a shard's level-0 substitution also leaves the support value of the row above the shard in the guard
+    //           element of the level-0 array, where the pass kernel expects it
+    // gathered (KT > 0): the last level is the WHOLE system's (nshards records, shard_rhs), this shard's rows start at
+    //           toff; xaboveOut receives the support value of the row above the shard for the levels below
     constexpr int K = CN_RS_K;
     const int lane = threadIdx.x & 31;
     const int64_t ngroups = off ? noff : (n + CN_RS_G - 1) / CN_RS_G;
@@ -340,7 +351,12 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
         }
         pdl_wait();
 #pragma unroll
-        for (int k = 0; k < KK; ++k) tR[k] = (w0 + k < ntop) ? cadd(ld_dep(topD + w0 + k), ld_dep(topU + w0 + k)) : zero;
+        for (int k = 0; k < KK; ++k) {
+            tR[k] = zero;
+            if (w0 + k < ntop)
+                tR[k] = gathered ? shard_rhs(gathered, nshards, ntop / nshards, w0 + k)
+                                 : cadd(ld_dep(topD + w0 + k), ld_dep(topU + w0 + k));
+        }
         pdl_launch_dependents();
         __syncthreads(); // every warp is done with its transfer buffer: the buffers become the scratch of the solve
         cplx *const sX = &sbuf_all[0][0];                    // [32 * CN_RS_WARPS * 8] <= 1024 values
@@ -372,15 +388,22 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
         }
         __syncthreads();
         if (live) {
-            if (g > 0) XL = sX[g - 1];
-            XJ = sX[g];
+            if (toff + g > 0) XL = sX[toff + g - 1];
+            XJ = sX[toff + g];
+            if (g == 0 && lane == 0 && toff > 0) {
+                if (xaboveOut) *xaboveOut = XL;
+                if (guardOut) *guardOut = XL;
+            }
         }
         __syncthreads(); // sX is read: the warps may use their transfer buffers again (rs_store_rows below)
     } else {
         pdl_wait();
         if (live) {
             if (g > 0) XL = ld_dep(Xup + g - 1);
-            else if (Xabove) XL = ld_dep(Xabove);
+            else if (Xabove) {
+                XL = ld_dep(Xabove);
+                if (lane == 0 && guardOut) *guardOut = XL;
+            }
             XJ = ld_dep(Xup + g);
         }
         pdl_launch_dependents();

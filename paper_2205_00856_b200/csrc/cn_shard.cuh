@@ -13,38 +13,32 @@
 //     last level, then sub / diag / sup of the shard's nt last-level rows].  Every shard assembles and factors the whole
 //     last-level matrix (S nt rows) from the gathered records: RS replicated, no root process.
 //   * per step: the JU contribution of the first block / first groups to the row above the shard is one value per level
-//     (guard [-1] of every rU array); they all add into that row's last-level right-hand side.  Record sent:
-//     [their sum, then rD + rU of the nt last-level rows] = nt + 1 values -- with nt = 1 exactly the two values per
-//     process of PAPER.md:175 for a pre-factored matrix.  k_shard_top solves the replicated last level from the gathered
-//     records and hands every shard the support values of its own rows and of the row above it.
+//     (guard [-1] of every rU array); they all add into that row's last-level right-hand side, so every reduction
+//     carries the guard of its level into the guard of the next.  Record sent: the two right-hand-side slots of the nt
+//     last-level rows with that guard = 2 nt values (shard_rhs below) -- with nt = 1 exactly the two values per process
+//     of PAPER.md:175 for a pre-factored matrix.  The replicated last level is solved from the gathered records
+//     (k_shard_top, or inside the substitution kernel of the level below when it is small) and hands every shard the
+//     support values of its own rows and of the row above it.
 #pragma once
 #include "cn_reduced.cuh"
 
-#define CN_SHARD_MAXLV 8
-
-struct cn_shard_guards {
-    const cplx *g[CN_SHARD_MAXLV]; // &rU_i[-1] of every level
-    int n;
-};
-
-// per-step record of this shard: rec[0] = sum over the levels of the JU guard, rec[1 + j] = rD[j] + rU[j] (last level)
-__global__ void k_shard_pack_step(int64_t nt, const cplx *__restrict__ rD, const cplx *__restrict__ rU, cn_shard_guards gs,
-                                  int above, cplx *__restrict__ rec)
+// Per-step record of a shard, 2 nt values: [rD[0..nt), guard, rU[0..nt-1)] -- the two right-hand-side slots of its nt
+// last-level rows exactly as its kernels write them (the record IS the storage of those arrays: nothing is packed),
+// with the guard element of rU -- the JU contributions of all levels to the row above the shard, carried up level by
+// level by k_rs_reduce -- in the middle, where rU[-1] lives.  rU of a shard's last row comes from the next shard (its
+// guard) and has no slot.  Right-hand side of last-level row w of the whole system:
+CN_DEVINL cplx shard_rhs(const cplx *gathered, int64_t S, int64_t nt, int64_t w)
 {
-    pdl_wait();
-    pdl_launch_dependents();
-    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j < nt) rec[1 + j] = cadd(ld_dep(rD + j), ld_dep(rU + j));
-    if (j == 0) {
-        cplx s = cmake(0.0, 0.0);
-        if (above)
-            for (int i = 0; i < gs.n; ++i) s = cadd(s, ld_dep(gs.g[i]));
-        rec[0] = s;
-    }
+    const int64_t rr = w / nt, j = w - rr * nt;
+    const cplx *rec = gathered + rr * (2 * nt);
+    cplx R = ld_dep(rec + j);
+    if (j < nt - 1) R = cadd(R, ld_dep(rec + nt + 1 + j));
+    else if (rr + 1 < S) R = cadd(R, ld_dep(gathered + (rr + 1) * (2 * nt) + nt)); // JU of the next shard
+    return R;
 }
 
 // RS[M_last] of the sharded system, replicated on every shard: right-hand side of row
-// w = r nt + j from the gathered records (S records of nt + 1 values), pre-factored matrix (lw, rq, uw), ONE CTA,
+// w = r nt + j from the gathered records (shard_rhs), pre-factored matrix (lw, rq, uw), ONE CTA,
 // K rows per thread (the structure of k_rs_top).  X: all S nt support values; guard0 (may be NULL): receives the
 // support value of the row above this shard, X[toff - 1], where the level-0 array of the pass kernels expects it.
 template <int K>
@@ -69,12 +63,7 @@ k_shard_top(int64_t S, int64_t nt, const cplx *__restrict__ gathered, const cplx
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const int64_t w = w0 + k;
-        R[k] = zero;
-        if (w < n) {
-            const int64_t rr = w / nt, j = w - rr * nt;
-            R[k] = ld_dep(gathered + rr * (nt + 1) + 1 + j);
-            if (j == nt - 1 && rr + 1 < S) R[k] = cadd(R[k], ld_dep(gathered + (rr + 1) * (nt + 1))); // JU of the next shard
-        }
+        R[k] = (w < n) ? shard_rhs(gathered, S, nt, w) : zero;
     }
     pdl_launch_dependents();
     cplx A = one, B = zero;

@@ -2,7 +2,7 @@
 
 One system is spread over `nshards` processes; the wave function is never gathered.  Per step
 every shard all-gathers ONE small record around the RS stage ("collecting four values per process
-... after the RS stage, two support values must be made available to each process"; here nt + 1 values per shard with
+... after the RS stage, two support values must be made available to each process"; here 2 nt values per shard with
 the matrix pre-factored, and the support values are computed locally from the gathered records because the last RS
 level is replicated).  This module holds no arithmetic of the method: it moves opaque records.
 
