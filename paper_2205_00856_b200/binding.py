@@ -270,7 +270,8 @@ class ShardPlan:
         self.h, self.N, self.shard, self.nshards = h, N_local, shard, nshards
         for k, v in opts.items():
             cn_plan_set_option(self.h, {"rs_topmax": CN_OPT_RS_TOPMAX, "pdl": CN_OPT_PDL, "keep_p": CN_OPT_KEEP_P,
-                                        "tile_threads": CN_OPT_TILE_THREADS}[k], v)
+                                        "tile_threads": CN_OPT_TILE_THREADS,
+                                        "rs_top_in_subst": CN_OPT_RS_TOP_IN_SUBST}[k], v)
 
     def counts(self):
         m, s = ctypes.c_int64(0), ctypes.c_int64(0)

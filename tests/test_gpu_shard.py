@@ -79,6 +79,8 @@ def test_c1_shape(S):
     (4, {}, None),
     (2, {"rs_topmax": 64}, None),    # two levels per shard (2048 -> 8 rows)
     (4, {"rs_topmax": 64}, None),
+    (4, {"rs_topmax": 64, "rs_top_in_subst": 0}, None),  # the replicated last level by its own kernel under two-level shards
+    (8, {"rs_topmax": 4, "pdl": 0}, None),               # three levels, plain launches
     (4, {"rs_topmax": 1}, None),     # levels down to ONE row per shard: 2 values per shard and step
     (8, {"rs_topmax": 1}, None),
     (2, {"rs_topmax": 1}, 1 << 16),  # blocks of 8 rows: 65536 -> 256 -> 1
