@@ -206,12 +206,12 @@ const char *cn_version(void);
  *   cn_tridiag_create_blocks : the same with CALLER-PLACED joint lines ("the blocks may differ in
  *                       size"): joints = P strictly increasing HOST row indices (0-based), joints[P-1] = N - 1; block w =
  *                       rows (joints[w-1], joints[w]], its last row is its joint line, blocks of one row (joint line
- *                       only) and two rows allowed.  Blocks of at most 256 rows run on one warp per block (as fast as
- *                       the library's own partition when they have 256 rows); if any block is wider, the ragged first
- *                       level runs on one thread per block straight in global memory -- the shape of the paper's own
- *                       kernels, an order of magnitude slower.  The reduced system on the P joint
- *                       lines runs on the nested warp-per-group levels.  CN_EINVAL for joints that are not increasing or
- *                       do not end at N - 1.  The solution does not depend on the joints.
+ *                       only) and two rows allowed.  Every caller joint line is a joint line of the first level; a
+ *                       block of more than 256 rows is partitioned again by the library (further joint lines inside it,
+ *                       the same method one level down), so that every block runs on one warp.  The
+ *                       reduced system on the joint lines runs on the nested warp-per-group levels.  CN_EINVAL for
+ *                       joints that are not increasing or do not end at N - 1.  The solution does not depend on the
+ *                       joints.
  */
 typedef struct cn_tridiag cn_tridiag;
 cn_status cn_tridiag_create(cn_tridiag **out, int64_t N, const void *b, const void *a, const void *c, void *stream);

@@ -63,8 +63,6 @@ struct cn_plan {
     std::vector<rs_level> lv;
     int64_t *off0 = nullptr; // caller-placed joint lines of level 0 (cn_tridiag_create_blocks): group g = rows [off0[g], off0[g+1])
     int64_t noff0 = 0;       // number of such groups
-    cplx *scratch0 = nullptr; // their reduction's scratch (the solution vector may alias the right-hand side)
-    bool off0_warp = false;   // every such group has at most CN_RS_G rows: the warp-per-group kernels take the offsets
     // configuration
     int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
     int opt_pdl = 1, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0, opt_rs_top_in_subst = 1, opt_keep_p = 0;
@@ -166,8 +164,6 @@ static void free_factors(cn_plan *p)
     p->qB = nullptr;
     p->gamJ = nullptr;
     p->off0 = nullptr;
-    p->scratch0 = nullptr;
-    p->off0_warp = false;
     p->topX[0] = p->topX[1] = nullptr; p->gsub = p->gdiag = p->gsup = nullptr; p->diagAcc = nullptr;
     p->sh_local_done = false;
     for (int b = 0; b < cn_plan::NB; ++b) { p->bPsi[b] = nullptr; p->bQ[b] = nullptr; p->bV[b] = nullptr; }
@@ -980,20 +976,19 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase =
     const bool tg = p->opt_rs_group != CN_RS_G; // one thread per group of any size (paper-shaped, cn_reduced.cuh)
     // the last level is solved inside the substitution kernel of the level below it (one launch less per step)
     const bool tis = !tg && !sharded && p->opt_rs_top_in_subst && p->opt_rs_levels >= 0 && !p->opt_rs_serial_top &&
-                     nlv >= 2 && p->lv.back().n <= p->opt_rs_top_in_subst_max && !(p->off0 && !p->off0_warp && nlv == 2);
+                     nlv >= 2 && p->lv.back().n <= p->opt_rs_top_in_subst_max;
     const int64_t G = p->opt_rs_group;
     for (int i = 0; i < nsep && e == cudaSuccess && phase != 2; ++i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        const int64_t *off = (i == 0) ? p->off0 : nullptr; // caller-placed joint lines: ragged blocks
-        const bool offw = off && p->off0_warp;              // ... of at most 256 rows: one warp per block, else one thread
-        if (tg || (off && !offw))
+        const int64_t *off = (i == 0) ? p->off0 : nullptr; // caller-placed joint lines: ragged blocks of at most 256 rows
+        if (tg)
             e = launch_k(k_rs_reduce_thread, (unsigned)((U.n + 63) / 64), 64u, 0, stream, pdl, L.n, G, (const cplx *)L.rD,
                          (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
-                         (const cplx *)L.sup, (off && p->scratch0) ? p->scratch0 : L.X, U.rD, U.rU, off, p->noff0);
+                         (const cplx *)L.sup, L.X, U.rD, U.rU);
         else
         e = launch_k(k_rs_reduce, (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS), 32u * CN_RS_WARPS, 0, stream, pdl, L.n, (const cplx *)L.rD,
                      (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)L.sub,
-                     (const cplx *)L.sup, U.rD, U.rU, above, offw ? off : (const int64_t *)nullptr, p->noff0);
+                     (const cplx *)L.sup, U.rD, U.rU, above, off, p->noff0);
         p->launches += 1;
     }
     // (sharded, phase 1: the last level's right-hand-side slots ARE the record to send, shard_bind_record; nothing to pack)
@@ -1037,11 +1032,9 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase =
     for (int i = nsep - 1; i >= 0 && e == cudaSuccess; --i) {
         const cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
         const int64_t *off = (i == 0) ? p->off0 : nullptr;
-        const bool offw = off && p->off0_warp;
-        if (tg || (off && !offw))
+        if (tg)
             e = launch_k(k_rs_subst_thread, (unsigned)((U.n + 63) / 64), 64u, 0, stream, pdl, L.n, G, (const cplx *)L.rD,
-                         (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X,
-                         off, p->noff0);
+                         (const cplx *)L.rU, (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X);
         else {
             const unsigned gr = (unsigned)((U.n + CN_RS_WARPS - 1) / CN_RS_WARPS);
             const int64_t T = 32 * CN_RS_WARPS;
@@ -1055,7 +1048,7 @@ static cn_status launch_rs(cn_plan *p, int out, cudaStream_t stream, int phase =
 #define CN_SUBST(KT) launch_k(k_rs_subst<KT>, gr, 32u * CN_RS_WARPS, 0, stream, pdl_here, L.n, (const cplx *)L.rD, (const cplx *)L.rU, \
                               (const cplx *)L.l, (const cplx *)L.rp, (const cplx *)L.u, (const cplx *)U.X, L.X, ntop,                \
                               (const cplx *)U.rD, (const cplx *)U.rU, (const cplx *)p->lw, (const cplx *)p->rq, (const cplx *)p->uw, \
-                              Xabove, offw ? off : (const int64_t *)nullptr, p->noff0, guardOut, gath, (int64_t)p->nshards,          \
+                              Xabove, off, p->noff0, guardOut, gath, (int64_t)p->nshards,          \
                               stis ? toff : (int64_t)0, xaboveOut)
             e = kt == 0 ? CN_SUBST(0) : (kt == 1 ? CN_SUBST(1) : (kt == 2 ? CN_SUBST(2) : (kt == 4 ? CN_SUBST(4) : CN_SUBST(8))));
 #undef CN_SUBST
@@ -1340,30 +1333,36 @@ static cn_status tridiag_create_impl(cn_tridiag **out, int64_t N, const void *b,
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
             return fail(CN_ECUDA);
     }
-    // levels: n_0 = N, n_{i+1} = ceil(n_i / 256) while n_i > 4096; with caller-placed joint lines n_1 = P
+    // Caller-placed joint lines: every one of them is a joint line of the first level.  A block of more than 256 rows is
+    // partitioned again by the library (more joint lines inside it, every 256 rows from its first row: the same method
+    // one level down; x does not depend on the partition), so that every block of the first level fits
+    // the warp-per-group kernels.
+    std::vector<int64_t> off;
+    if (joints) {
+        off.push_back(0);
+        for (int64_t w = 0; w < P; ++w) {
+            const int64_t end = joints[w] + 1;
+            while (end - off.back() > CN_RS_G) off.push_back(off.back() + CN_RS_G);
+            off.push_back(end);
+        }
+    }
+    const int64_t P1 = joints ? (int64_t)off.size() - 1 : 0; // blocks of the first level
+    // levels: n_0 = N, n_{i+1} = ceil(n_i / 256) while n_i > 4096; with caller-placed joint lines n_1 = P1
     for (int64_t n = N;;) {
         cn_plan::rs_level L;
         L.n = n;
         p->lv.push_back(L);
         const bool ragged0 = joints && p->lv.size() == 1;
         if (!ragged0 && (n <= p->opt_rs_topmax || n <= 2)) break;
-        n = ragged0 ? P : (n + CN_RS_G - 1) / CN_RS_G;
+        n = ragged0 ? P1 : (n + CN_RS_G - 1) / CN_RS_G;
     }
     if (joints) {
-        std::vector<int64_t> off((size_t)P + 1);
-        off[0] = 0;
-        int64_t widest = 0;
-        for (int64_t w = 0; w < P; ++w) {
-            off[(size_t)w + 1] = joints[w] + 1;
-            if (off[(size_t)w + 1] - off[(size_t)w] > widest) widest = off[(size_t)w + 1] - off[(size_t)w];
-        }
-        p->off0_warp = widest <= CN_RS_G; // blocks of at most 256 rows: one warp per block; wider ones: one thread
-        if ((st = dev_alloc(p, &p->off0, (size_t)P + 1)) != CN_OK) { cn_tridiag_destroy(t); return st; }
-        if (cudaMemcpy(p->off0, off.data(), sizeof(int64_t) * ((size_t)P + 1), cudaMemcpyHostToDevice) != cudaSuccess) {
+        if ((st = dev_alloc(p, &p->off0, (size_t)P1 + 1)) != CN_OK) { cn_tridiag_destroy(t); return st; }
+        if (cudaMemcpy(p->off0, off.data(), sizeof(int64_t) * ((size_t)P1 + 1), cudaMemcpyHostToDevice) != cudaSuccess) {
             cn_tridiag_destroy(t);
             return CN_ECUDA;
         }
-        p->noff0 = P;
+        p->noff0 = P1;
     }
     const int nlv = (int)p->lv.size();
     for (int i = 0; i < nlv; ++i) {
@@ -1384,14 +1383,12 @@ static cn_status tridiag_create_impl(cn_tridiag **out, int64_t N, const void *b,
         }
     }
     const size_t ntop = (size_t)p->lv.back().n;
-    cplx *tmpB = nullptr, *tmpA = nullptr;
-    const size_t n1 = joints ? (size_t)P : (size_t)((N + CN_RS_G - 1) / CN_RS_G);
+    cplx *tmpB = nullptr;
+    const size_t n1 = joints ? (size_t)P1 : (size_t)((N + CN_RS_G - 1) / CN_RS_G);
     if ((st = dev_alloc(p, &p->lw, ntop)) != CN_OK || (st = dev_alloc(p, &p->rq, ntop)) != CN_OK ||
         (st = dev_alloc(p, &p->uw, ntop)) != CN_OK || (st = dev_alloc(p, &p->derr, 1)) != CN_OK ||
         (st = dev_alloc(p, &t->zero, (size_t)N)) != CN_OK || (st = dev_alloc(p, &tmpB, n1)) != CN_OK)
         return fail(st);
-    if (joints && (st = dev_alloc(p, &tmpA, (size_t)N)) != CN_OK) return fail(st); // scratch of the thread-per-block kernels
-    p->scratch0 = tmpA;
     cn_plan::rs_level &L0 = p->lv[0];
     const size_t nb = sizeof(cplx) * (size_t)N;
     if (cudaMemsetAsync(t->zero, 0, nb, stream) != cudaSuccess || cudaMemsetAsync(p->derr, 0, sizeof(int), stream) != cudaSuccess ||
@@ -1404,16 +1401,9 @@ static cn_status tridiag_create_impl(cn_tridiag **out, int64_t N, const void *b,
     const int T = 128;
     for (int i = 0; i + 1 < nlv; ++i) {
         cn_plan::rs_level &L = p->lv[i], &U = p->lv[i + 1];
-        if (i == 0 && joints && p->off0_warp)
-            k_rs_factor_level_smem<<<(unsigned)((U.n + CN_RS_FL_WARPS - 1) / CN_RS_FL_WARPS), 32 * CN_RS_FL_WARPS, 0, stream>>>(
-                L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr, 0, p->off0, p->noff0);
-        else if (i == 0 && joints)
-            k_rs_factor_level<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(L.n, (int64_t)CN_RS_G, L.sub, L.diag, L.sup, L.l,
-                                                                             L.rp, L.u, tmpA, U.sub, U.diag, tmpB, U.sup,
-                                                                             p->derr, p->off0, p->noff0);
-        else
-            k_rs_factor_level_smem<<<(unsigned)((U.n + CN_RS_FL_WARPS - 1) / CN_RS_FL_WARPS), 32 * CN_RS_FL_WARPS, 0, stream>>>(
-                L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr, 0, nullptr, 0);
+        k_rs_factor_level_smem<<<(unsigned)((U.n + CN_RS_FL_WARPS - 1) / CN_RS_FL_WARPS), 32 * CN_RS_FL_WARPS, 0, stream>>>(
+            L.n, L.sub, L.diag, L.sup, L.l, L.rp, L.u, U.sub, U.diag, tmpB, U.sup, p->derr, 0, (i == 0) ? p->off0 : nullptr,
+            (i == 0) ? p->noff0 : 0);
         k_rs_add<<<(unsigned)((U.n + T - 1) / T), T, 0, stream>>>(U.n, U.diag, tmpB, nullptr);
     }
     k_rs_factor_top_scan<<<1, 32, 0, stream>>>(p->lv.back().n, p->lv.back().sub, p->lv.back().diag, p->lv.back().sup, p->lw,

@@ -205,7 +205,8 @@ k_rs_reduce(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
             const int64_t *__restrict__ off = nullptr, int64_t noff = 0)
 {   // above: the rows of a shard that another shard precedes (cn_shard.cuh): group 0 has a real joint line above it,
     // whose coupling sup[-1] and slot outU[-1] are the guard elements of the arrays
-    // off != NULL: caller-placed joint lines with blocks of at most CN_RS_G rows: group g = rows [off[g], off[g+1])
+    // off != NULL: caller-placed joint lines ("blocks may differ in size"), blocks of at most CN_RS_G rows:
+    // group g = rows [off[g], off[g+1])
     constexpr int K = CN_RS_K;
     const int lane = threadIdx.x & 31;
     const int64_t ngroups = off ? noff : (n + CN_RS_G - 1) / CN_RS_G;
@@ -450,15 +451,14 @@ k_rs_subst(int64_t n, const cplx *__restrict__ rD, const cplx *__restrict__ rU, 
 __global__ void k_rs_reduce_thread(int64_t n, int64_t G, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
                                    const cplx *__restrict__ l, const cplx *__restrict__ rp, const cplx *__restrict__ u,
                                    const cplx *__restrict__ sub, const cplx *__restrict__ sup, cplx *scratch,
-                                   cplx *__restrict__ outD, cplx *__restrict__ outU,
-                                   const int64_t *__restrict__ off = nullptr, int64_t noff = 0)
-{   // off != NULL: caller-placed joint lines ("blocks may differ in size"): group g = rows [off[g], off[g+1])
+                                   cplx *__restrict__ outD, cplx *__restrict__ outU)
+{
     pdl_wait();
     pdl_launch_dependents();
-    const int64_t ngroups = off ? noff : (n + G - 1) / G;
+    const int64_t ngroups = (n + G - 1) / G;
     const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= ngroups) return;
-    const int64_t g0 = off ? off[g] : g * G, J = (off ? off[g + 1] : ((g0 + G < n) ? (g0 + G) : n)) - 1;
+    const int64_t g0 = g * G, J = ((g0 + G < n) ? (g0 + G) : n) - 1;
     const cplx zero = cmake(0.0, 0.0);
     cplx D = zero;
     for (int64_t i = g0; i < J; ++i) {
@@ -477,15 +477,14 @@ __global__ void k_rs_reduce_thread(int64_t n, int64_t G, const cplx *__restrict_
 
 __global__ void k_rs_subst_thread(int64_t n, int64_t G, const cplx *__restrict__ rD, const cplx *__restrict__ rU,
                                   const cplx *__restrict__ l, const cplx *__restrict__ rp, const cplx *__restrict__ u,
-                                  const cplx *__restrict__ Xup, cplx *X,
-                                  const int64_t *__restrict__ off = nullptr, int64_t noff = 0)
+                                  const cplx *__restrict__ Xup, cplx *X)
 {
     pdl_wait();
     pdl_launch_dependents();
-    const int64_t ngroups = off ? noff : (n + G - 1) / G;
+    const int64_t ngroups = (n + G - 1) / G;
     const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= ngroups) return;
-    const int64_t g0 = off ? off[g] : g * G, J = (off ? off[g + 1] : ((g0 + G < n) ? (g0 + G) : n)) - 1;
+    const int64_t g0 = g * G, J = ((g0 + G < n) ? (g0 + G) : n) - 1;
     cplx D = (g > 0) ? ld_dep(Xup + g - 1) : cmake(0.0, 0.0);
     for (int64_t i = g0; i < J; ++i) {
         D = cfnma(l[i], D, cadd(ld_dep(rD + i), ld_dep(rU + i)));
@@ -536,13 +535,13 @@ __global__ void k_rs_factor_level(int64_t n, int64_t G, const cplx *__restrict__
                                   const cplx *__restrict__ sup, cplx *__restrict__ l, cplx *__restrict__ rp,
                                   cplx *__restrict__ u, cplx *__restrict__ tmp, cplx *__restrict__ sub2,
                                   cplx *__restrict__ diag2, cplx *__restrict__ diag2U, cplx *__restrict__ sup2,
-                                  int *__restrict__ err, const int64_t *__restrict__ off = nullptr, int64_t noff = 0)
-{   // off != NULL: caller-placed joint lines, group g = rows [off[g], off[g+1]) (see k_rs_reduce_thread)
-    const int64_t ngroups = off ? noff : (n + G - 1) / G;
+                                  int *__restrict__ err)
+{
+    const int64_t ngroups = (n + G - 1) / G;
     const int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= ngroups) return;
-    const int64_t g0 = off ? off[g] : g * G;
-    const int64_t J = (off ? off[g + 1] : ((g0 + G < n) ? (g0 + G) : n)) - 1;
+    const int64_t g0 = g * G;
+    const int64_t J = ((g0 + G < n) ? (g0 + G) : n) - 1;
     const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
     bool bad = false;
     cplx prp = one, psup = zero, Dal = one; // Dal: forward sweep of the response to X_{g-1} = 1
