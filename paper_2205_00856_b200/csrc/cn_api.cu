@@ -172,7 +172,7 @@ static void free_factors(cn_plan *p)
     p->tmBatchFor = nullptr;
 }
 
-extern "C" const char *cn_version(void) { return "cn_nshape 0.1 (sm_100a)"; }
+extern "C" const char *cn_version(void) { return "cn_nshape 0.2 (sm_100a)"; }
 
 extern "C" const char *cn_status_string(cn_status s)
 {
