@@ -37,7 +37,10 @@ from paper_2205_00856_b200 import replicas as R  # noqa: E402
 from paper_2205_00856_b200 import workloads as W  # noqa: E402
 
 CN_PER_STEP = 100            # CN steps per bench step (one cn_step call)
-BYTES_PER_POINT_STEP = 56.0  # algorithmic: psi in 16 + q 16 + gamma 8 + psi out 16
+BYTES_PER_POINT_STEP = 56.0  # algorithmic bytes per point-step as SURVEY 8d declares them: psi in 16 + one stored complex factor
+                             # 16 + real V / gamma 8 + psi out 16 -- the figure `roofline.achieved` is computed from
+BYTES_MOVED_PER_POINT = 48.0  # what the fused pass of this build moves: it recovers gamma from the stored pivots (DESIGN.md
+                              # section 5), so it reads psi 16 + q 16 and writes psi 16; reported beside the declared figure
 METRIC = "cn_grid_point_steps_per_sec_complex128"
 UNIT = "Gpoint-steps/s"
 WORKLOAD = ("C2 (N=2^24 complex128, dx=0.05, dt=0.005, soft-Coulomb V, Gaussian x random phase + 1e-3 dense noise, "
@@ -477,6 +480,10 @@ def main():
                           "(events between launches disable the PDL overlap that `value` has)",
                 "ms_per_step_profiled": ms_prof / args.steps,
                 "algorithmic_bytes_per_launch": BYTES_PER_POINT_STEP * cfg.N, "peak_source": peak_src,
+                "bytes_per_point": {"declared_minimum_SURVEY_8d": BYTES_PER_POINT_STEP,
+                                    "moved_by_this_formulation": BYTES_MOVED_PER_POINT},
+                "achieved_on_bytes_moved": (BYTES_MOVED_PER_POINT * cfg.N / (pass_ms * 1e-3) / 1e9) if prof["pass_count"] else None,
+                "frac_on_bytes_moved": (BYTES_MOVED_PER_POINT * cfg.N / (pass_ms * 1e-3) / 1e9 / peak) if prof["pass_count"] else None,
                 "whole_step_GBps": BYTES_PER_POINT_STEP * cfg.N * cn_per * args.steps / (ms * 1e-3) / 1e9}
 
     # ---- e2e: every bench step takes its wave function from PINNED HOST memory (H2D), advances it by cn_per CN steps

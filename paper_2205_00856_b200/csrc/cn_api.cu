@@ -533,7 +533,10 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
         }
         const int64_t nch = N / 8;
         const unsigned gridc = (unsigned)((nch + 127) / 128);
-#define CN_FB(L) k_factor_blocks_chunked<L><<<gridc, 128, 0, stream>>>(nch, p->two_dx2, p->rho, Vsrc, tdG, tdF, p->q, p->gam, redSubD, redDiagD, redSupU, redDiagU, p->derr, above, cutMask)
+        // (a driven step does not store gamma: the tiled pass recovers it from q and reads only gamJ; the factorization of
+        // the static H at the end of cn_step_td and cn_factorize write it for the kernels that want it)
+        double *const gamOut = (tdG && p->path == 2) ? nullptr : p->gam;
+#define CN_FB(L) k_factor_blocks_chunked<L><<<gridc, 128, 0, stream>>>(nch, p->two_dx2, p->rho, Vsrc, tdG, tdF, p->q, gamOut, redSubD, redDiagD, redSupU, redDiagU, p->derr, above, cutMask, p->gamJ)
         switch (logc) {
         case 0: CN_FB(0); break;
         case 1: CN_FB(1); break;
@@ -549,7 +552,7 @@ static cn_status factor_compute(cn_plan *p, const double *Vsrc, cplx *red, int64
                 p->launches += 1;
             }
             k_factor_blocks<<<(unsigned)((P + T - 1) / T), T, 0, stream>>>(g, p->two_dx2, p->rho, Vsrc, p->q, p->gam, redSubD,
-                                                                          redDiagD, redSupU, redDiagU, p->derr);
+                                                                          redDiagD, redSupU, redDiagU, p->derr, p->gamJ);
         }
 #undef CN_FB
     } else {
@@ -713,9 +716,10 @@ static cn_status factorize_impl(cn_plan *p, cudaStream_t stream, cplx *msend)
     if (!p->ooc) {
         if ((st = dev_alloc(p, &p->q, (size_t)N)) != CN_OK) return st;
         if ((st = dev_alloc(p, &p->gam, (size_t)N)) != CN_OK) return st;
-    } else {
-        if ((st = dev_alloc(p, &p->gamJ, (size_t)P)) != CN_OK) return st;
     }
+    // gamma on the joint lines: all the tiled pass reads of gamma (the rest it recovers from q); all there is out of core
+    if (p->ooc || p->path == 2)
+        if ((st = dev_alloc_g(p, &p->gamJ, (size_t)P, sharded)) != CN_OK) return st;
     if ((st = dev_alloc_g(p, &p->slotD, (size_t)P, sharded)) != CN_OK) return st;
     if ((st = dev_alloc_g(p, &p->slotU, (size_t)P, sharded)) != CN_OK) return st;
     if ((st = dev_alloc(p, &p->derr, 1)) != CN_OK) return st;
@@ -921,12 +925,13 @@ static cn_status launch_pass(cn_plan *p, cplx *psi, int mode, int cur, cudaStrea
         prm.slotD = p->slotD;
         prm.slotU = p->slotU;
         prm.supInit = p->sup[0];
+        prm.gamJ = p->gamJ;
         if (p->above) {
             // a shard with a predecessor: its blocks are numbered from 1, so that "the joint line above block w" is
             // index w - 1 >= 0 for every block -- for the first one the guard element in front of the arrays, which
             // holds what belongs to the last row of the preceding shard (the same mechanism as a streamed part)
             prm.chunk0 = (int64_t)1 << p->logc;
-            prm.supOld -= 1; prm.supNew -= 1; prm.slotD -= 1; prm.slotU -= 1; prm.supInit -= 1;
+            prm.supOld -= 1; prm.supNew -= 1; prm.slotD -= 1; prm.slotU -= 1; prm.supInit -= 1; prm.gamJ -= 1;
             prm.P += 1;
         }
         if (p->nshards > 1) prm.P = 0; // no block of a shard clears slotU of "the last joint line": that slot belongs to the
@@ -1092,6 +1097,7 @@ static cn_status ooc_pass(cn_plan *p, cplx *hpsi, int mode, int cur, bool first)
         prm.slotD = p->slotD;
         prm.slotU = p->slotU;
         prm.supInit = p->sup[0];
+        prm.gamJ = p->gamJ;
         const int64_t tiles = (n / 8 + p->tpb - 1) / p->tpb;
         const unsigned grid = (unsigned)(tiles < p->grid_tiled ? tiles : p->grid_tiled);
         cudaError_t e = launch_k(k, grid, (unsigned)p->tpb, tiled_smem(p->tpb), p->sCmp, false, p->tmPsiB[b], p->tmQB[b],

@@ -30,7 +30,8 @@ struct cn_geom {
 __global__ void k_factor_blocks(cn_geom g, double two_dx2, double rho, const double *__restrict__ V,
                                 cplx *__restrict__ q, double *__restrict__ gam,
                                 cplx *__restrict__ redSubD, cplx *__restrict__ redDiagD,
-                                cplx *__restrict__ redSupU, cplx *__restrict__ redDiagU, int *__restrict__ err)
+                                cplx *__restrict__ redSupU, cplx *__restrict__ redDiagU, int *__restrict__ err,
+                                double *__restrict__ gamJ = nullptr) // gamJ: also gamma of the joint lines, per block
 {
     int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= g.P) return;
@@ -50,6 +51,7 @@ __global__ void k_factor_blocks(cn_geom g, double two_dx2, double rho, const dou
         qprev = qi;
     }
     gam[J] = fma(two_dx2, V[J], 2.0);
+    if (gamJ) gamJ[w] = gam[J];
     q[J] = cmake(1.0, 0.0);
     if (n >= 1) {
         cplx Znn = qprev;
@@ -145,7 +147,8 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
                         cplx *__restrict__ redDiagD, cplx *__restrict__ redSupU, cplx *__restrict__ redDiagU,
                         int *__restrict__ err, int above = 0, // above: a shard precedes this one (cn_shard.cuh): the first
                                                               // block's JU matrix side goes to the guard element [-1]
-                        int64_t cutMask = ~(int64_t)0)        // independent systems of cutMask + 1 blocks (cn_pass_tiled.cuh)
+                        int64_t cutMask = ~(int64_t)0,        // independent systems of cutMask + 1 blocks (cn_pass_tiled.cuh)
+                        double *__restrict__ gamJ = nullptr)  // also gamma of the joint lines, per block
 {
     constexpr int CPB = 1 << LOGC;
     const int lane = threadIdx.x & 31;
@@ -169,9 +172,11 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
             g[2 * jj] = fma(two_dx2, vv.x, 2.0);
             g[2 * jj + 1] = fma(two_dx2, vv.y, 2.0);
         }
-        double2 *g2 = reinterpret_cast<double2 *>(gam + 8 * c);
+        if (gam) { // (NULL under cn_step_td: the tiled pass recovers gamma from q, only gamJ is needed)
+            double2 *g2 = reinterpret_cast<double2 *>(gam + 8 * c);
 #pragma unroll
-        for (int jj = 0; jj < 4; ++jj) g2[jj] = make_double2(g[2 * jj], g[2 * jj + 1]);
+            for (int jj = 0; jj < 4; ++jj) g2[jj] = make_double2(g[2 * jj], g[2 * jj + 1]);
+        }
     }
     const int nrow = isLast ? 7 : 8; // the joint line (row 7 of a block's last chunk) is not part of the recurrence
     // ---- downward: inflow of every chunk -----------------------------------------------------------------
@@ -206,7 +211,10 @@ k_factor_blocks_chunked(int64_t nchunks, double two_dx2, double rho, const doubl
             qin = qnew;
         }
     }
-    if (isLast) q[8 * c + 7] = one;
+    if (isLast) {
+        q[8 * c + 7] = one;
+        if (gamJ) gamJ[w] = g[7];
+    }
 #pragma unroll
     for (int k = 0; k < LOGC; ++k) { // product over the block, wanted at its last chunk
         const int dd = 1 << k;

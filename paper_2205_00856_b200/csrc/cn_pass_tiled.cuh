@@ -18,7 +18,10 @@
 //   P2 (start step k+1): E of the new psi -> RD, RU with zero support values -> JD / JU contributions
 //                        slotD[w], slotU[w-1] (two slots per joint line instead of atomics).
 //
-// Algorithmic HBM bytes per point of a fused pass: psi in 16 + q 16 + gamma 8 + psi out 16 = 56.
+// gamma is NOT read: mu_i = p_i + q_{i-1} with p_i = 1 / q_i (the block-local pivot recurrence, cn_factor.cuh), so
+// gamma_i = -Re(1 / q_i + q_{i-1}) costs one real reciprocal per point (at a block's first row mu_f = 1 / q_f; on a
+// joint line, where q := 1 is stored, gamma comes from the O(P) array gamJ).  HBM bytes moved per point of a fused pass:
+// psi in 16 + q 16 + psi out 16 = 48, against the 56 of the formulation that also stores gamma (SURVEY 8d's minimum).
 #pragma once
 #include <cuda.h>
 #include "cn_common.cuh"
@@ -39,6 +42,7 @@ struct cn_tiled_params {
     const cplx *supNew;  // psi^k+1 at the joint lines (RS output of this step)
     cplx *slotD, *slotU;
     cplx *supInit; // prologue only: receives psi^0 at the joint lines
+    const double *gamJ; // gamma on the joint lines (gamma of every other row is recovered from the stored pivots)
 };
 
 CN_DEVINL uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -86,7 +90,7 @@ CN_DEVINL void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta
 template <int TPB>
 constexpr size_t tiled_smem_bytes()
 {
-    return (size_t)TPB * (128 + 128 + 64 + 128) + (size_t)(TPB / 32) * (2 * 2 + 2) * sizeof(cplx) + 16;
+    return (size_t)TPB * (128 + 128 + 128) + (size_t)(TPB / 32) * (2 * 2 + 2) * sizeof(cplx) + 16;
 }
 
 // TPB threads, 8 points per thread, 2^LOGC chunks (threads) per block.  PERSISTENT: CTA b handles tiles
@@ -107,9 +111,8 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
     extern __shared__ __align__(1024) uint8_t smem[];
     cplx *const s_psi = (cplx *)smem;
     cplx *const s_q = (cplx *)(smem + (size_t)TPB * 128);
-    double2 *const s_g = (double2 *)(smem + (size_t)TPB * 256);
-    cplx *const s_out = (cplx *)(smem + (size_t)TPB * 320);
-    cplx *const s_scan = (cplx *)(smem + (size_t)TPB * 448); // [2 buffers][A,B][NW]
+    cplx *const s_out = (cplx *)(smem + (size_t)TPB * 256);
+    cplx *const s_scan = (cplx *)(smem + (size_t)TPB * 384); // [2 buffers][A,B][NW]
     cplx *const s_edge = s_scan + 2 * 2 * NW;                // [2][NW] edge exchange between warps
     uint64_t *const bar = (uint64_t *)(s_edge + 2 * NW);
 
@@ -120,12 +123,11 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
 
     auto issue_loads = [&](int64_t tile) {
         const int64_t r0 = tile * TPB;
-        mbar_expect_tx(bar, (uint32_t)(TPB * 320));
+        mbar_expect_tx(bar, (uint32_t)(TPB * 256));
 #pragma unroll
         for (int r = 0; r < TPB; r += 256) {
             tma_load_2d((uint8_t *)s_psi + (size_t)r * 128, &tmPsi, bar, 0, (int)(r0 + r));
             tma_load_2d((uint8_t *)s_q + (size_t)r * 128, &tmQ, bar, 0, (int)(r0 + r));
-            tma_load_2d((uint8_t *)s_g + (size_t)r * 64, &tmGam, bar, 0, (int)(r0 + r));
         }
     };
 
@@ -158,6 +160,8 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
             if (isLast) supN = prm.supNew[w];
             if (!top) jointAbove = prm.supNew[w - 1];
         }
+        double gJ = 2.0; // gamma of the own joint line (last chunk of a block)
+        if (active && isLast) gJ = prm.gamJ[w];
         cplx oldAbove = zero; // OLD psi just above the tile (needed by thread 0 only)
         // (prologue of a streamed part: the row above it is a joint line whose psi^0 the previous part recorded)
         if (t == 0 && !top) oldAbove = P1 ? prm.supOld[w - 1] : (c > 0 ? prm.psi_raw[8 * c - 1] : prm.supInit[w - 1]);
@@ -174,18 +178,22 @@ k_pass_tiled(const __grid_constant__ CUtensorMap tmPsi, const __grid_constant__ 
             v[j] = s_psi[t * 8 + (j ^ sw)];
             qv[j] = s_q[t * 8 + (j ^ sw)];
         }
-        const int sg = (t >> 1) & 3;
-#pragma unroll
-        for (int jj = 0; jj < 4; ++jj) {
-            double2 gg = s_g[t * 4 + (jj ^ sg)];
-            g[2 * jj] = gg.x;
-            g[2 * jj + 1] = gg.y;
-        }
         cplx vlo = oldAbove, vhi = zero, qm1 = cmake(1.0, 0.0); // the row above a tile is a joint line
         if (t > 0) {
             vlo = s_psi[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
             qm1 = s_q[(t - 1) * 8 + (7 ^ ((t - 1) & 7))];
         }
+        // gamma_j = -Re(mu_j), mu_j = 1 / q_j + q_{j-1}; nothing is subtracted at a block's first row (its pivot is mu_f)
+        // (the lanes beyond the end of the array hold q = 0: `pad` keeps their reciprocal finite, the unpredicated scans
+        // multiply what those lanes hold by A = 0)
+        const double pad = active ? 0.0 : 1.0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const double qpx = (j == 0) ? (isFirst ? 0.0 : qm1.x) : qv[j - 1].x;
+            const double r = rcp_pos(fma(qv[j].x, qv[j].x, fma(qv[j].y, qv[j].y, pad)));
+            g[j] = -fma(qv[j].x, r, qpx);
+        }
+        if (isLast) g[7] = gJ;
         if (t < TPB - 1) vhi = s_psi[(t + 1) * 8 + ((t + 1) & 7)];
         if (isFirst && top) vlo = zero;       // nothing above the first row of a system
         if (!P1 && isFirst) jointAbove = vlo; // prologue: psi^0 of the joint above

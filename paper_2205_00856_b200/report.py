@@ -231,9 +231,9 @@ def p_sweep(torch, peak, name="C2dense"):
     return {"config": name + " P sweep", "N": cfg.N, "sqrtN": math.isqrt(cfg.N), "rows": rows, "fit": fits}
 
 
-# algorithmic HBM bytes per point of one driven step: factor kernel V 8 + g 8 in, q 16 + gamma 8
-# out; prologue pass psi 16 + q 16 + gamma 8 in; epilogue pass the same in + psi 16 out
-TD_BYTES_PER_POINT = 136
+# HBM bytes per point of one driven step: factor kernel V 8 + g 8 in, q 16 out; prologue pass
+# psi 16 + q 16 in; epilogue pass the same in + psi 16 out (gamma is recovered from q by the passes: 136 before that)
+TD_BYTES_PER_POINT = 112
 
 
 def run_td(torch, peak, name="C2dense", nsteps=20):
