@@ -92,7 +92,8 @@ typedef struct {
     int32_t out_of_core;     /* 1 if a device budget forces host streaming */
     size_t device_bytes;     /* device memory owned by the plan */
     int64_t launches;        /* kernels launched by this plan so far (all entry points) */
-    double bytes_per_point_step; /* algorithmic HBM bytes per point per fused step of the chosen path */
+    double bytes_per_point_step; /* HBM bytes per point a fused step of the tiled path moves (48: psi 16 + q 16 in, psi 16
+                                    out; the formulation that also reads gamma, SURVEY 8d's declared minimum, moves 56) */
     int64_t P_effective;     /* blocks the kernels work with: P, or N / (8 * 2^k) when the tiled path chooses the
                                 partition itself (see cn_plan_create, CN_OPT_KEEP_P) */
 } cn_plan_info;

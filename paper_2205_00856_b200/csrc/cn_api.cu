@@ -347,7 +347,7 @@ extern "C" cn_status cn_plan_get_info(const cn_plan *plan, cn_plan_info *info)
     info->out_of_core = plan->ooc ? 1 : 0;
     info->device_bytes = plan->device_bytes;
     info->launches = plan->launches;
-    info->bytes_per_point_step = 56.0;
+    info->bytes_per_point_step = (plan->path == 2) ? 48.0 : 56.0; // the tiled pass recovers gamma from q: psi 16 + q 16 in, psi 16 out
     return CN_OK;
 }
 
