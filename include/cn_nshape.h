@@ -52,7 +52,8 @@ typedef enum {
 typedef enum {
     CN_OPT_PATH = 1,        /* 0 = auto (default), 1 = force the generic thread-per-block kernels,
                                2 = force the tiled TMA kernels (CN_EINVAL at factorize if the shape does not fit) */
-    CN_OPT_TILE_THREADS = 2,/* threads per CTA of the tiled kernels: 0 = auto, else 128/256/512 (8 points per thread) */
+    CN_OPT_TILE_THREADS = 2,/* threads per CTA of the tiled kernels: 0 = auto (64), else 32/64/128/256/512 (8 points per
+                               thread; at least one block per tile) */
     CN_OPT_RS_TOPMAX = 3,   /* largest reduced system solved by the single-CTA RS kernel (1..8192, default 4096);
                                a larger one is partitioned again into groups of 256 joint lines (next RS level) */
                             /* 4: not used (CN_EINVAL) */

@@ -283,7 +283,7 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
         plan->factorized = false;
         return CN_OK;
     case CN_OPT_TILE_THREADS:
-        if (value != 0 && value != 128 && value != 256 && value != 512) return CN_EINVAL;
+        if (value != 0 && value != 32 && value != 64 && value != 128 && value != 256 && value != 512) return CN_EINVAL;
         plan->opt_tile_threads = (int)value;
         plan->factorized = false;
         return CN_OK;
@@ -387,7 +387,7 @@ typedef void (*tiled_kernel_t)(const CUtensorMap, const CUtensorMap, const CUten
 template <int TPB, int LOGC, int MODE>
 static tiled_kernel_t tiled_kernel_inst()
 {
-    constexpr int MINB = (TPB == 128) ? 4 : (TPB == 256 ? 2 : 1);
+    constexpr int MINB = (TPB == 32) ? 16 : (TPB == 64) ? 8 : ((TPB == 128) ? 4 : (TPB == 256 ? 2 : 1));
     if (MODE == 0) return k_pass_tiled<TPB, LOGC, false, true, MINB>;
     if (MODE == 1) return k_pass_tiled<TPB, LOGC, true, true, MINB>;
     return k_pass_tiled<TPB, LOGC, true, false, MINB>;
@@ -403,8 +403,8 @@ static tiled_kernel_t tiled_kernel_for_logc(int logc)
     case 3: return tiled_kernel_inst<TPB, 3, MODE>();
     case 4: return tiled_kernel_inst<TPB, 4, MODE>();
     case 5: return tiled_kernel_inst<TPB, 5, MODE>();
-    case 6: return tiled_kernel_inst<TPB, 6, MODE>();
-    case 7: return tiled_kernel_inst<TPB, 7, MODE>();
+    case 6: if (TPB >= 64) return tiled_kernel_inst<(TPB >= 64 ? TPB : 64), 6, MODE>(); break;
+    case 7: if (TPB >= 128) return tiled_kernel_inst<(TPB >= 128 ? TPB : 128), 7, MODE>(); break;
     case 8: if (TPB >= 256) return tiled_kernel_inst<(TPB >= 256 ? TPB : 256), 8, MODE>(); break;
     case 9: if (TPB >= 512) return tiled_kernel_inst<(TPB >= 512 ? TPB : 512), 9, MODE>(); break;
     }
@@ -419,6 +419,8 @@ static tiled_kernel_t tiled_kernel(int tpb, int logc, int mode)
         if (mode == 1) return tiled_kernel_for_logc<T, 1>(logc); \
         return tiled_kernel_for_logc<T, 2>(logc);                \
     }
+    CN_PICK(32)
+    CN_PICK(64)
     CN_PICK(128)
     CN_PICK(256)
     CN_PICK(512)
@@ -428,7 +430,8 @@ static tiled_kernel_t tiled_kernel(int tpb, int logc, int mode)
 
 static size_t tiled_smem(int tpb)
 {
-    return tpb == 128 ? tiled_smem_bytes<128>() : (tpb == 256 ? tiled_smem_bytes<256>() : tiled_smem_bytes<512>());
+    return tpb == 32 ? tiled_smem_bytes<32>() : tpb == 64 ? tiled_smem_bytes<64>()
+                     : (tpb == 128 ? tiled_smem_bytes<128>() : (tpb == 256 ? tiled_smem_bytes<256>() : tiled_smem_bytes<512>()));
 }
 
 
@@ -696,9 +699,11 @@ static cn_status factorize_impl(cn_plan *p, cudaStream_t stream, cplx *msend)
     int tpb = 0;
     if (tiled_ok) {
         const int cpb = 1 << logc;
-        // tiles of 128 threads (four CTAs per SM) since the pass stopped staging gamma: 147 against 153 us per C2 step
-        tpb = p->opt_tile_threads ? p->opt_tile_threads : 128;
-        if (tpb < cpb) tpb = (cpb <= 128) ? 128 : (cpb <= 256 ? 256 : 512);
+        // small tiles since the pass stopped staging gamma (25 KB of shared memory per 64 threads): eight CTAs of two
+        // warps per SM interleave their load and compute phases more finely than two of eight -- 144 against 153 us per
+        // C2 step in a 100-step call (32 threads: the same; the two-pass step of cn_step_td prefers 128: 391 / 394 / 400 us)
+        tpb = p->opt_tile_threads ? p->opt_tile_threads : 64;
+        if (tpb < cpb) tpb = (cpb <= 64) ? 64 : ((cpb <= 128) ? 128 : (cpb <= 256 ? 256 : 512));
         if (p->opt_tile_threads && p->opt_tile_threads < cpb) tiled_ok = false;
     }
     if (p->opt_path == 2 && !tiled_ok) return CN_EINVAL;

@@ -71,7 +71,8 @@ TILED_SHAPES = [
     (4096, 64, 512), (1 << 16, 1 << 13, 0), (1 << 16, 1 << 12, 0), (1 << 16, 1 << 11, 128), (1 << 16, 1 << 10, 0),
     (1 << 16, 1 << 9, 0), (1 << 16, 1 << 8, 0), (1 << 16, 1 << 7, 512), (1 << 16, 1 << 6, 0), (1 << 16, 1 << 5, 0),
     (1 << 16, 1 << 4, 512), (6656, 26, 0), (6656, 26, 128), (8 * 1000, 1000, 0), (2048 * 3 + 512, 13, 0),
-    (2048 * 5 + 1024, 11, 0),
+    (2048 * 5 + 1024, 11, 0), (4096, 64, 32), (4096, 64, 64), (1 << 16, 1 << 13, 32), (1 << 16, 1 << 8, 32), (1 << 16, 1 << 9, 64),
+    (6656, 26, 64), (6656 + 256, 27, 32), (1 << 16, 1 << 7, 64),
 ]
 
 
@@ -268,11 +269,11 @@ def test_errors_on_device():
         B.cn_step(plan.h, psi.data_ptr() + 8, 1)
     assert ei.value.status == B.CN_EINVAL
     # every option value the header documents is accepted, everything else is CN_EINVAL (include/cn_nshape.h)
-    good = {B.CN_OPT_PATH: (0, 1, 2), B.CN_OPT_TILE_THREADS: (0, 128, 256, 512), B.CN_OPT_RS_TOPMAX: (1, 4096, 8192),
+    good = {B.CN_OPT_PATH: (0, 1, 2), B.CN_OPT_TILE_THREADS: (0, 32, 64, 128, 256, 512), B.CN_OPT_RS_TOPMAX: (1, 4096, 8192),
             B.CN_OPT_RS_LEVELS: (-1, 0, 1, 8), B.CN_OPT_PROFILE: (0, 1), B.CN_OPT_PDL: (0, 1), B.CN_OPT_ONCHIP: (0, 1),
             B.CN_OPT_RS_GROUP: (2, 256, 1 << 20), B.CN_OPT_RS_SERIAL_TOP: (0, 1), B.CN_OPT_RS_TOP_IN_SUBST: (0, 1, 1024),
             B.CN_OPT_KEEP_P: (0, 1)}
-    bad = {B.CN_OPT_PATH: (-1, 3), B.CN_OPT_TILE_THREADS: (64, 1024), B.CN_OPT_RS_TOPMAX: (0, 8193),
+    bad = {B.CN_OPT_PATH: (-1, 3), B.CN_OPT_TILE_THREADS: (16, 96, 1024), B.CN_OPT_RS_TOPMAX: (0, 8193),
            B.CN_OPT_RS_LEVELS: (-2, 9), B.CN_OPT_RS_GROUP: (1, (1 << 20) + 1), 4: (0, 1), 9: (0, 1), 0: (0,), 14: (0,)}
     for key, vals in good.items():
         for v in vals:
