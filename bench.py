@@ -223,7 +223,8 @@ def per_config_report(torch, peak, full, with_cpu):
     r = RP.run_systems(torch, peak)
     out["C4V"] = {"workload": "C4 shape (8192 x 8192), non-separable V(x, y): every line of a sweep has its own matrix",
                   "bytes_per_point_sweep": 56, "contiguous": r["contiguous"], "interleaved": r["interleaved"],
-                  "frac": r["contiguous"]["hbm_frac_measured_peak"]}
+                  "frac": r["contiguous"]["hbm_frac_measured_peak"],
+                  "frac_on_bytes_moved": r["contiguous"]["hbm_frac_on_bytes_moved"]}
 
     if full:
         # ---- C3: 2^30 points resident (psi 17 GB + factors 26 GB) -----------------------------------------------------
@@ -231,7 +232,8 @@ def per_config_report(torch, peak, full, with_cpu):
         r = RP.run_1d(torch, "C3", peak)
         c3 = {"workload": "C3 (N=2^30, dx=0.01, dt=0.001, 32 seeded Gaussians, 50 CN steps)",
               "us_per_cn_step": r["us_per_cn_step_best"], "Gpoint_steps_per_s": r["Gpoint_steps_per_s"],
-              "bytes_per_point": 56, "frac": r["hbm_frac_measured_peak"], "P_effective": r["P_effective"],
+              "bytes_per_point": 56, "frac": r["hbm_frac_measured_peak"],
+              "frac_on_bytes_moved": r["hbm_frac_on_bytes_moved"], "P_effective": r["P_effective"],
               "rs_levels": r["rs_levels"]}
         if O:
             n = 1 << 26

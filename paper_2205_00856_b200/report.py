@@ -78,7 +78,8 @@ def run_1d(torch, name, peak, nsteps=None, P=None, **opts):
         best, med = time_plan(torch, plan, d, n)
         info = plan.info()
     gbs = 56.0 * cfg.N / (best * 1e-3) / 1e9
-    return {"config": name, "N": cfg.N, "P": P or cfg.P, "P_effective": info["P_effective"], "path": info["path"],
+    moved = info["bytes_per_point_step"]  # 48 on the tiled path (gamma recovered from the pivots), else 56
+    return {"config": name, "bytes_moved_per_point": moved, "hbm_frac_on_bytes_moved": gbs * moved / 56.0 / peak, "N": cfg.N, "P": P or cfg.P, "P_effective": info["P_effective"], "path": info["path"],
             "rs_levels": info["rs_levels"], "cn_steps_per_call": n, "us_per_cn_step_best": 1e3 * best,
             "us_per_cn_step_median": 1e3 * med, "Gpoint_steps_per_s": cfg.N / best / 1e6, "bytes_per_point": 56,
             "whole_step_GBps": gbs, "hbm_frac_measured_peak": gbs / peak, "hbm_frac_8TBps": gbs / 8000.0,
@@ -317,8 +318,11 @@ def run_systems(torch, peak, n=8192, nsys=8192, nsteps=20):
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / k
             gbs = 56.0 * n * nsys / (ms * 1e-3) / 1e9
-            out[key] = {"ms_per_sweep": ms, "Gpoint_sweeps_per_s": n * nsys / ms / 1e6, "path": plan.info()["path"],
-                        "bytes_per_point": 56, "GBps": gbs, "hbm_frac_measured_peak": gbs / peak}
+            info = plan.info()
+            moved = info["bytes_per_point_step"] if key == "contiguous" else 56
+            out[key] = {"ms_per_sweep": ms, "Gpoint_sweeps_per_s": n * nsys / ms / 1e6, "path": info["path"],
+                        "bytes_per_point": 56, "GBps": gbs, "hbm_frac_measured_peak": gbs / peak,
+                        "bytes_moved_per_point": moved, "hbm_frac_on_bytes_moved": gbs * moved / 56.0 / peak}
     return out
 
 
