@@ -45,7 +45,8 @@ typedef enum {
     CN_ENOMEM = 2,         /* host or device allocation failed / device budget too small */
     CN_ECUDA = 3,          /* a CUDA call failed; see cn_last_cuda_error */
     CN_ENOTFACTORIZED = 4, /* cn_step / cn_batched_sweep before cn_factorize */
-    CN_EBREAKDOWN = 5      /* zero or non-finite pivot met by cn_factorize */
+    CN_EBREAKDOWN = 5,     /* zero or non-finite pivot met by cn_factorize */
+    CN_ETOOLARGE = 6       /* cn_step_static: N exceeds CN_STATIC_NMAX, the size of the library's static device scratch */
 } cn_status;
 
 /* Options for cn_plan_set_option (all optional; call before cn_factorize). */
@@ -277,6 +278,28 @@ cn_status cn_shard_epilogue(cn_plan *plan, void *psi, const void *step_all, void
 typedef cn_status (*cn_exchange_fn)(void *ctx, const void *send, void *recv, int64_t count, void *stream);
 cn_status cn_shard_factorize(cn_plan *plan, cn_exchange_fn exchange, void *ctx, void *stream);
 cn_status cn_shard_run(cn_plan *plan, void *psi, int64_t nsteps, cn_exchange_fn exchange, void *ctx, void *stream);
+
+/*
+ * A stepper that ALLOCATES NOTHING, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  No plan: what a plan keeps in device memory it allocated -- gamma and the
+ * inverse pivots of the downward elimination of the whole system -- is recomputed by every
+ * call into a fixed static device array of the library, CN_STATIC_NMAX rows = 96 KB, which every GPU that loads the
+ * library holds until the process exits.  The call makes no cudaMalloc, cudaFree or allocating library call.
+ *   cn_step_static : nsteps Crank-Nicolson steps (Eq. 2-3) of ONE system of 2 <= N <= CN_STATIC_NMAX
+ *                    points, in place.  V: N doubles, psi: N complex128 (16-byte aligned), both DEVICE pointers owned by
+ *                    the caller, on the current device.  Enqueues three launches on `stream` (factor into the scratch,
+ *                    the on-chip stepper of cn_step, a check); does not synchronise.  Results are those of
+ *                    cn_plan_create(N, .) / cn_factorize / cn_step on its default (on-chip) path, to the last bit.
+ *   Errors: CN_ETOOLARGE when N > CN_STATIC_NMAX (use a plan); CN_EINVAL for the other bad arguments of
+ *           cn_plan_create / cn_step or a misaligned pointer; CN_ECUDA when a CUDA call fails.  A zero or non-finite
+ *           pivot (non-finite V) cannot be returned by an asynchronous call: psi is then filled with NaN.
+ *   Sharing: ALL calls on a device share the one array, and it keeps the last call's contents (every call rewrites
+ *           what it reads and clears its flag).  Calls that overlap on the GPU -- different streams, or different host
+ *           threads without an order between their streams -- RACE on it: the caller serialises them.  The factor
+ *           side is a serial recurrence over N rows (about 0.1 ms at N = 4096): amortise it over nsteps.
+ */
+#define CN_STATIC_NMAX 4096
+cn_status cn_step_static(int64_t N, double dx, double dt, const double *V, void *psi, int64_t nsteps, void *stream);
 
 #ifdef __cplusplus
 }

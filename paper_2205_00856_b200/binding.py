@@ -13,7 +13,8 @@ import os
 PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(PKG, "libcn_nshape.so")
 
-CN_OK, CN_EINVAL, CN_ENOMEM, CN_ECUDA, CN_ENOTFACTORIZED, CN_EBREAKDOWN = range(6)
+CN_OK, CN_EINVAL, CN_ENOMEM, CN_ECUDA, CN_ENOTFACTORIZED, CN_EBREAKDOWN, CN_ETOOLARGE = range(7)
+CN_STATIC_NMAX = 4096
 CN_OPT_PATH, CN_OPT_TILE_THREADS, CN_OPT_RS_TOPMAX, CN_OPT_RS_LEVELS, CN_OPT_PROFILE, CN_OPT_PDL, CN_OPT_ONCHIP = 1, 2, 3, 5, 6, 7, 8
 CN_OPT_RS_GROUP, CN_OPT_RS_SERIAL_TOP, CN_OPT_RS_TOP_IN_SUBST, CN_OPT_KEEP_P = 10, 11, 12, 13
 PATH_AUTO, PATH_GENERIC, PATH_TILED, PATH_ONCHIP = 0, 1, 2, 3
@@ -25,7 +26,7 @@ EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", 
            "cn_tridiag_create_blocks", "cn_plan_set_systems", "cn_batched_sweep_v",
            "cn_shard_plan_create", "cn_shard_counts", "cn_shard_factorize_local", "cn_shard_factorize_finish",
            "cn_shard_edge", "cn_shard_prologue", "cn_shard_advance", "cn_shard_epilogue",
-           "cn_shard_factorize", "cn_shard_run"]
+           "cn_shard_factorize", "cn_shard_run", "cn_step_static"]
 
 # cn_exchange_fn: cn_status (*)(void *ctx, const void *send, void *recv, int64_t count, void *stream)
 EXCHANGE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
@@ -99,6 +100,8 @@ def lib():
         L.cn_shard_factorize.argtypes = [vp, EXCHANGE_FN, vp, vp]
         L.cn_shard_run.restype = i32
         L.cn_shard_run.argtypes = [vp, vp, i64, EXCHANGE_FN, vp, vp]
+        L.cn_step_static.restype = i32
+        L.cn_step_static.argtypes = [i64, dbl, dbl, vp, vp, i64, vp]
         L.cn_destroy.restype = i32
         L.cn_destroy.argtypes = [vp]
         L.cn_plan_get_info.restype = i32
@@ -171,6 +174,13 @@ def cn_factorize(plan, stream=None):
 def cn_step(plan, psi, nsteps: int = 1, stream=None):
     """psi: N complex128, torch CUDA tensor (or pinned host tensor in out-of-core mode); updated in place."""
     _check(plan, lib().cn_step(plan, _ptr(psi), nsteps, _stream(stream)), "cn_step")
+
+
+def cn_step_static(N: int, dx: float, dt: float, V, psi, nsteps: int = 1, stream=None):
+    """The stepper that allocates nothing (N <= CN_STATIC_NMAX).  V: N float64, psi: N complex128, both torch CUDA
+    tensors on the current device; psi updated in place.  Calls that overlap on the GPU race on the library's scratch."""
+    assert getattr(V, "is_cuda", False) and getattr(psi, "is_cuda", False), "cn_step_static takes DEVICE pointers"
+    _check(None, lib().cn_step_static(N, dx, dt, _ptr(V), _ptr(psi), nsteps, _stream(stream)), "cn_step_static")
 
 
 def cn_plan_set_td_shape(plan, g):

@@ -183,6 +183,7 @@ extern "C" const char *cn_status_string(cn_status s)
     case CN_ECUDA: return "CN_ECUDA: CUDA error (see cn_last_cuda_error)";
     case CN_ENOTFACTORIZED: return "CN_ENOTFACTORIZED: call cn_factorize first";
     case CN_EBREAKDOWN: return "CN_EBREAKDOWN: zero or non-finite pivot";
+    case CN_ETOOLARGE: return "CN_ETOOLARGE: N exceeds CN_STATIC_NMAX (4096), the static device scratch of cn_step_static";
     }
     return "unknown cn_status";
 }
@@ -1898,5 +1899,149 @@ extern "C" cn_status cn_shard_run(cn_plan *p, void *psi, int64_t nsteps, cn_exch
         st = (k < nsteps) ? cn_shard_advance(p, psi, b.srecv, b.ssend[k & 1], stream) : cn_shard_epilogue(p, psi, b.srecv, stream);
         if (st != CN_OK) return st;
     }
+    return CN_OK;
+}
+
+// ---- cn_step_static: a stepper that allocates NOTHING ------------------------------------------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+// it): no plan, no cudaMalloc / cudaFree / allocating library routine on this path.  What a plan keeps in device
+// memory it allocated -- gamma and the inverse pivots of the whole-system downward elimination,
+// the scratch of the on-chip stepper of cn_onchip.cuh -- lives in ONE file-scope device array of fixed size
+// (CN_STATIC_NMAX rows: 96 KB + a flag; every GPU that loads the library holds it until the process exits).
+//   * every call shares the array: it keeps the last call's contents, so every call rewrites all it reads (gamma and
+//     pivots of ITS N rows) and clears the breakdown flag first; two calls that overlap on the GPU (different streams,
+//     different host threads) RACE on it -- the caller serialises them;
+//   * in host code `cn_static_scratch` is a host-side stand-in, not a device address: the kernels get the address
+//     cudaGetSymbolAddress returns, fetched once per device with that device current (static_setup).
+#define CN_STATIC_BYTES ((size_t)CN_STATIC_NMAX * (sizeof(cplx) + sizeof(double)) + 256)
+static __device__ __align__(256) unsigned char cn_static_scratch[CN_STATIC_BYTES];
+static_assert(CN_STATIC_NMAX <= CN_ONCHIP_NMAX, "cn_step_static runs on the on-chip stepper");
+
+// layout of the scratch: [qB: NMAX complex][gamma: NMAX double][flag: int, padded]
+struct cn_static_view {
+    cplx *qB;
+    double *gam;
+    int *flag;
+};
+static cn_static_view static_view(unsigned char *base)
+{
+    cn_static_view v;
+    v.qB = (cplx *)base;
+    v.gam = (double *)(base + (size_t)CN_STATIC_NMAX * sizeof(cplx));
+    v.flag = (int *)(base + (size_t)CN_STATIC_NMAX * (sizeof(cplx) + sizeof(double)));
+    return v;
+}
+
+// Variant of k_factor_whole (cn_batched.cuh) that owns no plan memory: gamma_i = 2 + 2 dx^2 V_i and the inverse pivots
+// p_0 = mu_0, p_i = mu_i - q_{i-1}, q_i = 1 / p_i of the whole system, both into the static scratch.  Same arithmetic,
+// same order as cn_factorize for an on-chip plan, so psi agrees with cn_step to the last bit.  flag := 0 / 1 (breakdown).
+__global__ void k_static_factor(int64_t N, double two_dx2, double rho, const double *__restrict__ V,
+                                cplx *__restrict__ qB, double *__restrict__ gam, int *__restrict__ flag)
+{
+    for (int64_t i = threadIdx.x; i < N; i += blockDim.x) gam[i] = fma(two_dx2, V[i], 2.0);
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    cplx qprev = cmake(0.0, 0.0);
+    bool bad = false;
+    for (int64_t i = 0; i < N; ++i) {
+        cplx p = cmake(-gam[i] - qprev.x, rho - qprev.y);
+        if (!cfinite_nonzero(p)) bad = true;
+        qprev = crecip(p);
+        qB[i] = qprev;
+    }
+    *flag = bad ? 1 : 0; // cleared on every call: the array keeps the last call's contents
+}
+
+// the asynchronous call cannot return CN_EBREAKDOWN: a zero or non-finite pivot (non-finite V) turns psi into NaN
+__global__ void k_static_poison(int64_t N, cplx *__restrict__ psi, const int *__restrict__ flag)
+{
+    if (*flag == 0) return;
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+        psi[i] = cmake(nan, nan);
+}
+
+// set-up, once per device, with that device current: the DEVICE address of the scratch and the shared-memory opt-in of
+// the on-chip kernels (neither allocates).  A table indexed by the device ordinal; a spin lock of plain atomics keeps
+// concurrent first calls from several host threads apart (no allocating C++ runtime object on this path).
+#define CN_STATIC_MAXDEV 64
+static unsigned char *g_static_ptr[CN_STATIC_MAXDEV];
+static int g_static_ready[CN_STATIC_MAXDEV];
+static int g_static_lock;
+
+// there is no plan to keep the CUDA error in: it is cleared and reported as CN_ECUDA
+static cn_status static_fail(cudaError_t)
+{
+    (void)cudaGetLastError();
+    return CN_ECUDA;
+}
+
+static cn_status static_setup(unsigned char **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return static_fail(e);
+    if (dev < 0 || dev >= CN_STATIC_MAXDEV) return CN_EINVAL;
+    if (!__atomic_load_n(&g_static_ready[dev], __ATOMIC_ACQUIRE)) {
+        while (__atomic_exchange_n(&g_static_lock, 1, __ATOMIC_ACQUIRE)) {}
+        cn_status st = CN_OK;
+        if (!g_static_ready[dev]) {
+            void *ptr = nullptr;
+            e = cudaGetSymbolAddress(&ptr, cn_static_scratch);
+            if (e == cudaSuccess && (!ptr || ((uintptr_t)ptr & 255u) != 0)) e = cudaErrorInvalidSymbol;
+#define CN_STATIC_ATTR(T)                                                                                     \
+    if (e == cudaSuccess)                                                                                     \
+        e = cudaFuncSetAttribute((const void *)k_onchip_steps<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                 (int)onchip_smem_bytes<T>());
+            CN_STATIC_ATTR(32)
+            CN_STATIC_ATTR(64)
+            CN_STATIC_ATTR(128)
+            CN_STATIC_ATTR(256)
+            CN_STATIC_ATTR(512)
+#undef CN_STATIC_ATTR
+            if (e == cudaSuccess) {
+                g_static_ptr[dev] = (unsigned char *)ptr;
+                __atomic_store_n(&g_static_ready[dev], 1, __ATOMIC_RELEASE);
+            } else {
+                st = static_fail(e);
+            }
+        }
+        __atomic_store_n(&g_static_lock, 0, __ATOMIC_RELEASE);
+        if (st != CN_OK) return st;
+    }
+    *out = g_static_ptr[dev];
+    return CN_OK;
+}
+
+extern "C" cn_status cn_step_static(int64_t N, double dx, double dt, const double *V, void *psi_, int64_t nsteps,
+                                    void *stream_)
+{
+    if (N > CN_STATIC_NMAX) return CN_ETOOLARGE; // beyond the static scratch: use a plan (cn_plan_create / cn_step)
+    if (!V || !psi_ || N < 2 || nsteps < 0) return CN_EINVAL;
+    if (!std::isfinite(dx) || !std::isfinite(dt) || dx <= 0.0 || dt == 0.0) return CN_EINVAL;
+    if (((uintptr_t)psi_ & 15u) != 0 || ((uintptr_t)V & 7u) != 0) return CN_EINVAL;
+    if (nsteps == 0) return CN_OK;
+    unsigned char *base = nullptr;
+    cn_status st = static_setup(&base);
+    if (st != CN_OK) return st;
+    const cn_static_view sv = static_view(base);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    cplx *psi = (cplx *)psi_;
+    const double rho = 4.0 * dx * dx / dt, two_dx2 = 2.0 * dx * dx; // as cn_plan_create
+    cudaError_t e = launch_k(k_static_factor, 1u, 256u, 0, stream, false, N, two_dx2, rho, V, sv.qB, sv.gam, sv.flag);
+    if (e != cudaSuccess) return static_fail(e);
+    const int64_t chunks = (N + 7) / 8;
+#define CN_ONCHIP(T)                                                                                 \
+    launch_k(k_onchip_steps<T>, 1u, (unsigned)T, onchip_smem_bytes<T>(), stream, false, N, nsteps, rho, psi, \
+             (const cplx *)sv.qB, (const double *)sv.gam)
+    if (chunks <= 32) e = CN_ONCHIP(32);
+    else if (chunks <= 64) e = CN_ONCHIP(64);
+    else if (chunks <= 128) e = CN_ONCHIP(128);
+    else if (chunks <= 256) e = CN_ONCHIP(256);
+    else e = CN_ONCHIP(512);
+#undef CN_ONCHIP
+    if (e != cudaSuccess) return static_fail(e);
+    e = launch_k(k_static_poison, 4u, 256u, 0, stream, false, N, psi, (const int *)sv.flag);
+    if (e != cudaSuccess) return static_fail(e);
     return CN_OK;
 }
