@@ -84,13 +84,24 @@ struct cn_bx_params {
 #define CN_BX_TPB 256
 #define CN_BATCHED_NMAX (1 << 20) // largest N for which cn_factorize also keeps whole-system pivots
 
+// shared memory of k_batched_x: two psi tiles, the per-tile B aggregates and mailboxes, and the CONSTANT multipliers of
+// every scan step (the matrix is the same for every system and every tile, so the A side of all scans is computed once)
 constexpr size_t batched_x_smem_bytes()
 {
-    return (size_t)CN_BX_TPB * 256 + (size_t)(CN_BX_TPB / 32) * 4 * sizeof(cplx) + 4 * 8 * sizeof(cplx) + 32;
+    return (size_t)CN_BX_TPB * 256                               // s_psi, s_out
+           + (size_t)2 * (CN_BX_TPB / 32) * sizeof(cplx)          // s_wB   [2 dirs][NW]
+           + (size_t)4 * 8 * sizeof(cplx) + 32                    // s_mailB, s_mailA [2 dirs][8 ranks] each; 4 mbarriers
+           + (size_t)10 * CN_BX_TPB * sizeof(cplx)                // s_M [2][4][TPB], s_Ae [2][TPB]
+           + (size_t)8 * (CN_BX_TPB / 32) * sizeof(cplx);         // s_wM [2][3][NW], s_cA [2][NW]
 }
 
 // 256 threads x 8 points.  LOGC = log2(chunks per system) when a system fits one CTA (CL == 1, several
 // systems per tile); CL > 1: one system = CL CTAs of a cluster (LOGC == 8, every CTA chains all its chunks).
+//
+// Scans: a sweep restricted to a chunk is the affine map x -> A x + B (cn_common.cuh); A depends on the matrix alone.
+// All A products of the Kogge-Stone steps -- warp level, warps of a CTA, CTAs of a cluster -- are therefore computed
+// ONCE before the tile loop and kept as multipliers (0 where a lane has no partner); per tile a scan step is one
+// shuffle of B and one complex fused multiply-add.
 template <int LOGC, int CL>
 __global__ void __launch_bounds__(CN_BX_TPB, 2)
 k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
@@ -101,6 +112,7 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
     constexpr int SPT = TPB / CPB;            // systems per tile (CL == 1)
     constexpr bool XWARP = (LOGC > 5);
     constexpr int WSTEPS = XWARP ? 5 : LOGC;
+    constexpr int XSTEPS = XWARP ? LOGC - 5 : 0;
     constexpr int NW = TPB / 32;
     constexpr int WPB = XWARP ? (CPB / 32) : 1;
     static_assert(CL == 1 || LOGC == 8, "a cluster chains whole CTAs");
@@ -108,9 +120,14 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
     extern __shared__ __align__(1024) uint8_t smem[];
     cplx *const s_psi = (cplx *)smem;
     cplx *const s_out = (cplx *)(smem + (size_t)TPB * 128);
-    cplx *const s_scan = (cplx *)(smem + (size_t)TPB * 256); // [2 dirs][A,B][NW]
-    cplx *const s_mail = s_scan + 4 * NW;                    // [2 dirs][A,B][8 ranks]
-    uint64_t *const bar = (uint64_t *)(s_mail + 4 * 8); // [0] TMA loads, [1] downward mailbox, [2] upward mailbox
+    cplx *const s_wB = (cplx *)(smem + (size_t)TPB * 256); // [2 dirs][NW]        per-tile B aggregate of every warp
+    cplx *const s_mailB = s_wB + 2 * NW;                   // [2 dirs][8 ranks]   per-tile B aggregate of every CTA
+    cplx *const s_mailA = s_mailB + 16;                    // [2 dirs][8 ranks]   constant A aggregate of every CTA
+    uint64_t *const bar = (uint64_t *)(s_mailA + 16);      // [0] TMA loads, [1] downward mailbox, [2] upward mailbox
+    cplx *const s_M = (cplx *)(bar + 4);                   // [2][4][TPB]  multiplier of warp-scan steps 1..4
+    cplx *const s_Ae = s_M + 8 * TPB;                      // [2][TPB]     inclusive A of the neighbouring lane
+    cplx *const s_wM = s_Ae + 2 * TPB;                     // [2][3][NW]   multipliers of the scan over the warp aggregates
+    cplx *const s_cA = s_wM + 6 * NW;                      // [2][NW]      A of the warps of this block before this warp
 
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const uint32_t rank = (CL > 1) ? cluster_ctarank() : 0u;
@@ -120,6 +137,7 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
     const double rho = prm.rho;
     const int pos = (CL > 1) ? (int)rank * TPB + t : (t & (CPB - 1)); // chunk position inside its system
     const bool sysFirst = pos == 0, sysLast = pos == CPS - 1;
+    const int vb = warp & ~(WPB - 1), wl = vb + (lane & (WPB - 1)); // first warp of this block; this lane's warp slot
 
     auto issue_load = [&](int64_t tile) {
         mbar_expect_tx(bar, (uint32_t)(TPB * 128));
@@ -136,11 +154,6 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
         g[j] = prm.gam[8 * pos + j];
     }
     const cplx qm1 = sysFirst ? zero : prm.qB[8 * pos - 1];
-    cplx Qp = cneg(qv[0]);
-#pragma unroll
-    for (int j = 1; j < 7; ++j) Qp = cmul(Qp, cneg(qv[j]));
-    const cplx fwdA = sysFirst ? zero : cmul(cneg(qm1), Qp); // nothing enters a system from above
-    const cplx bwdA = sysLast ? zero : cmul(Qp, cneg(qv[7])); // ... nor from below (Dirichlet)
 
     if (t == 0) {
         if ((smem_u32(smem) & 1023u) != 0) __trap();
@@ -149,80 +162,125 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
         mbar_init(bar + 2, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (CL > 1) { // every CTA of the cluster is resident before anything is stored into its shared memory
+        cluster_arrive();
+        cluster_wait();
+    }
+
+    // ---- the A side of every scan, once (the matrix side) --------------------------------------
+    cplx M0[2]; // multiplier of warp-scan step 0, in registers; steps 1..4 in s_M
+    {
+        cplx Qp = cneg(qv[0]);
+#pragma unroll
+        for (int j = 1; j < 7; ++j) Qp = cmul(Qp, cneg(qv[j]));
+        const cplx chunkA[2] = {sysFirst ? zero : cmul(cneg(qm1), Qp),  // nothing enters a system from above
+                                sysLast ? zero : cmul(Qp, cneg(qv[7]))}; // ... nor from below (Dirichlet)
+#pragma unroll
+        for (int di = 0; di < 2; ++di) { // 0: information flows to higher chunks (downward sweep), 1: to lower chunks
+            cplx A = chunkA[di];
+            M0[di] = zero;
+#pragma unroll
+            for (int k = 0; k < WSTEPS; ++k) {
+                const int d = 1 << k;
+                const bool ok = (di == 0) ? (lane >= d) : (lane + d < 32);
+                const cplx Mk = ok ? A : zero;
+                if (k == 0) M0[di] = Mk;
+                else s_M[(di * 4 + k - 1) * TPB + t] = Mk;
+                const cplx As = (di == 0) ? shfl_up_c(A, d) : shfl_down_c(A, d);
+                if (ok) A = cmul(A, As);
+            }
+            s_Ae[di * TPB + t] = (di == 0) ? shfl_up_c(A, 1) : shfl_down_c(A, 1);
+            cplx aggA = A;
+            if (XWARP) {
+                if (lane == (di == 0 ? 31 : 0)) s_cA[di * NW + warp] = A; // for now: the aggregate of this warp
+                __syncthreads();
+                cplx wA = s_cA[di * NW + wl];
+#pragma unroll
+                for (int k = 0; k < XSTEPS; ++k) {
+                    const int d = 1 << k, l = lane & (WPB - 1);
+                    const bool ok = (di == 0) ? (l >= d) : (l + d < WPB);
+                    if (lane < WPB && warp == vb) s_wM[(di * 3 + k) * NW + wl] = ok ? wA : zero;
+                    const cplx As = (di == 0) ? shfl_up_c(wA, d) : shfl_down_c(wA, d);
+                    if (ok) wA = cmul(wA, As);
+                }
+                aggA = shfl_c(wA, di == 0 ? WPB - 1 : 0);
+                const int src = (di == 0) ? warp - vb - 1 : warp - vb + 1;
+                const bool has = (di == 0) ? (src >= 0) : (src < WPB);
+                const cplx xA = shfl_c(wA, has ? src : 0);
+                __syncthreads(); // every warp has read the aggregates
+                if (lane == 0) s_cA[di * NW + warp] = has ? xA : one;
+            }
+            if (CL > 1 && warp == 0 && lane < CL) { // the aggregate of this CTA to the CTAs that chain after it
+                const bool wants = (di == 0) ? ((uint32_t)lane > rank) : ((uint32_t)lane < rank);
+                if (wants) dsmem_store(s_mailA + di * 8 + rank, (uint32_t)lane, aggA);
+            }
+        }
+    }
     pdl_wait(); // psi is the output of the preceding sweep
     pdl_launch_dependents();
     if (t == 0 && cid < ntiles) issue_load(cid);
-    if (CL > 1) {
+    if (CL > 1) { // the A aggregates have arrived everywhere
         cluster_arrive();
         cluster_wait();
     } else {
         __syncthreads();
     }
 
-    // exclusive map of the chunks of this CTA before (DIR > 0) / after (DIR < 0) this thread: (Aex, Bex);
-    // also leaves the aggregate of the whole CTA in (aggA, aggB)
-    auto scan_cta = [&](auto dirtag, cplx A, cplx B, cplx &Aex, cplx &Bex, cplx &aggA, cplx &aggB) {
+    // value entering this thread's chunk from the chunks before it in direction DIR (B: what leaves the chunk when
+    // nothing enters it); per step one shuffle and one complex fused multiply-add against the stored multipliers
+    uint32_t xphase = 0;
+    auto inflow = [&](auto dirtag, cplx B) -> cplx {
         constexpr int DIR = decltype(dirtag)::value;
-        warp_scan_affine<DIR, WSTEPS>(A, B, lane);
-        cplx cA = one, cB = zero; // composite of the warps of this block before this warp
+        constexpr int di = DIR > 0 ? 0 : 1;
+        {
+            const cplx Bs = (DIR > 0) ? shfl_up_c(B, 1) : shfl_down_c(B, 1);
+            B = cfma(M0[di], Bs, B);
+        }
+#pragma unroll
+        for (int k = 1; k < WSTEPS; ++k) {
+            const cplx Bs = (DIR > 0) ? shfl_up_c(B, 1 << k) : shfl_down_c(B, 1 << k);
+            B = cfma(s_M[(di * 4 + k - 1) * TPB + t], Bs, B);
+        }
+        cplx cB = zero; // what enters this warp
         if (XWARP) {
-            cplx *sA = s_scan + (DIR > 0 ? 0 : 2 * NW), *sB = sA + NW;
-            if (lane == (DIR > 0 ? 31 : 0)) {
-                sA[warp] = A;
-                sB[warp] = B;
-            }
+            if (lane == (DIR > 0 ? 31 : 0)) s_wB[di * NW + warp] = B;
             __syncthreads();
-            const int vb = warp & ~(WPB - 1);
-            cplx wA = one, wB = zero;
-            if (lane < WPB) {
-                wA = sA[vb + lane];
-                wB = sB[vb + lane];
+            cplx wB = s_wB[di * NW + wl];
+#pragma unroll
+            for (int k = 0; k < XSTEPS; ++k) {
+                const cplx Bs = (DIR > 0) ? shfl_up_c(wB, 1 << k) : shfl_down_c(wB, 1 << k);
+                wB = cfma(s_wM[(di * 3 + k) * NW + wl], Bs, wB);
             }
-            warp_scan_affine<DIR, (LOGC > 5 ? LOGC - 5 : 0)>(wA, wB, lane);
-            aggA = shfl_c(wA, DIR > 0 ? WPB - 1 : 0);
-            aggB = shfl_c(wB, DIR > 0 ? WPB - 1 : 0);
             const int src = (DIR > 0) ? warp - vb - 1 : warp - vb + 1;
             const bool has = (DIR > 0) ? (src >= 0) : (src < WPB);
-            cplx xA = shfl_c(wA, has ? src : 0), xB = shfl_c(wB, has ? src : 0);
-            if (has) {
-                cA = xA;
-                cB = xB;
+            const cplx xB = shfl_c(wB, has ? src : 0);
+            if (has) cB = xB;
+            if (CL > 1) {
+                // level 3: the aggregates travel by asynchronous DSMEM stores that signal the receiver's mbarrier: a
+                // CTA waits only for the CTAs it depends on, never for the whole cluster.  A sender can never be a
+                // whole tile ahead of a receiver: it needs that receiver's aggregate of the opposite direction to
+                // finish its own tile.
+                const cplx aggB = shfl_c(wB, DIR > 0 ? WPB - 1 : 0);
+                cplx *mA = s_mailA + di * 8, *mB = s_mailB + di * 8;
+                uint64_t *mb = bar + 1 + di;
+                if (warp == 0 && lane < CL) {
+                    const bool wants = (DIR > 0) ? ((uint32_t)lane > rank) : ((uint32_t)lane < rank);
+                    if (wants) dsmem_store_signal(mB + rank, mb, (uint32_t)lane, aggB);
+                }
+                const int nsend = (DIR > 0) ? (int)rank : CL - 1 - (int)rank;
+                if (nsend > 0) mbar_wait(mb, xphase);
+                cplx cin = zero;
+                if (DIR > 0) {
+                    for (int u = 0; u < (int)rank; ++u) cin = cfma(mA[u], cin, mB[u]);
+                } else {
+                    for (int u = CL - 1; u > (int)rank; --u) cin = cfma(mA[u], cin, mB[u]);
+                }
+                cB = cfma(s_cA[di * NW + warp], cin, cB);
             }
         }
-        cplx Ae = (DIR > 0) ? shfl_up_c(A, 1) : shfl_down_c(A, 1);
-        cplx Be = (DIR > 0) ? shfl_up_c(B, 1) : shfl_down_c(B, 1);
+        const cplx Be = (DIR > 0) ? shfl_up_c(B, 1) : shfl_down_c(B, 1);
         const bool first = (DIR > 0) ? (lane == 0) : (lane == 31);
-        // (Ae, Be) after the warp composite (cA, cB):  x -> Ae (cA x + cB) + Be
-        Aex = first ? cA : cmul(Ae, cA);
-        Bex = first ? cB : cfma(Ae, cB, Be);
-    };
-
-    // inflow of this CTA from the other CTAs of its cluster (level 3); every thread returns the same value.
-    // The aggregates travel by asynchronous DSMEM stores that signal the receiver's mbarrier: a CTA waits only for
-    // the CTAs it depends on, never for the whole cluster.  A sender can never be a whole tile ahead of a receiver,
-    // because it needs that receiver's aggregate of the opposite direction to finish its own tile.
-    uint32_t xphase = 0;
-    auto cluster_inflow = [&](auto dirtag, cplx aggA, cplx aggB) -> cplx {
-        constexpr int DIR = decltype(dirtag)::value;
-        if (CL == 1) return zero;
-        cplx *mA = s_mail + (DIR > 0 ? 0 : 16), *mB = mA + 8;
-        uint64_t *mb = bar + (DIR > 0 ? 1 : 2);
-        if (warp == 0 && lane < CL) {
-            const bool wants = (DIR > 0) ? ((uint32_t)lane > rank) : ((uint32_t)lane < rank);
-            if (wants) {
-                dsmem_store_signal(mA + rank, mb, (uint32_t)lane, aggA);
-                dsmem_store_signal(mB + rank, mb, (uint32_t)lane, aggB);
-            }
-        }
-        const int nsend = (DIR > 0) ? (int)rank : CL - 1 - (int)rank;
-        if (nsend > 0) mbar_wait(mb, xphase);
-        cplx in = zero;
-        if (DIR > 0) {
-            for (int u = 0; u < (int)rank; ++u) in = cfma(mA[u], in, mB[u]);
-        } else {
-            for (int u = CL - 1; u > (int)rank; --u) in = cfma(mA[u], in, mB[u]);
-        }
-        return in;
+        return first ? cB : cfma(s_Ae[di * TPB + t], cB, Be);
     };
 
     uint32_t phase = 0;
@@ -231,9 +289,9 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
         // stores its new rows only after it has received this CTA's aggregates of this tile)
         cplx vlo = zero, vhi = zero;
         if (CL > 1) {
-            if (t == 0) { // arm this tile's mailboxes: 32 bytes (A, B) from every CTA this one depends on
-                if (rank > 0) mbar_expect_tx(bar + 1, rank * 32u);
-                if (rank < CL - 1) mbar_expect_tx(bar + 2, (CL - 1 - rank) * 32u);
+            if (t == 0) { // arm this tile's mailboxes: 16 bytes (B) from every CTA this one depends on
+                if (rank > 0) mbar_expect_tx(bar + 1, rank * 16u);
+                if (rank < CL - 1) mbar_expect_tx(bar + 2, (CL - 1 - rank) * 16u);
             }
             const cplx *row = prm.psi_raw + tile * prm.sys_stride;
             if (t == 0 && rank > 0) vlo = row[8 * pos - 1];
@@ -263,10 +321,8 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
         cplx D = zero;
 #pragma unroll
         for (int j = 0; j < 8; ++j) D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
-        cplx Aex, Bex, aggA, aggB;
-        scan_cta(std::integral_constant<int, +1>{}, fwdA, D, Aex, Bex, aggA, aggB);
-        cplx cin = cluster_inflow(std::integral_constant<int, +1>{}, aggA, aggB);
-        D = sysFirst ? zero : cfma(Aex, cin, Bex);
+        D = inflow(std::integral_constant<int, +1>{}, D);
+        if (sysFirst) D = zero;
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
             D = cfnma((j == 0) ? qm1 : qv[j - 1], D, E[j]);
@@ -276,9 +332,8 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
         cplx X = zero;
 #pragma unroll
         for (int j = 7; j >= 0; --j) X = cmul(qv[j], csub(E[j], X));
-        scan_cta(std::integral_constant<int, -1>{}, bwdA, X, Aex, Bex, aggA, aggB);
-        cin = cluster_inflow(std::integral_constant<int, -1>{}, aggA, aggB);
-        X = sysLast ? zero : cfma(Aex, cin, Bex);
+        X = inflow(std::integral_constant<int, -1>{}, X);
+        if (sysLast) X = zero;
 #pragma unroll
         for (int j = 7; j >= 0; --j) {
             X = cmul(qv[j], csub(E[j], X));
