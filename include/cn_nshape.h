@@ -77,6 +77,9 @@ typedef enum {
     CN_OPT_RS_TOP_IN_SUBST = 12, /* 1 (default) = a last level of at most 256 rows is solved inside the substitution
                                kernel of the level below it, redundantly by every CTA (one launch less per step);
                                a value v > 1 sets the row limit to min(v, 1024); 0 = always by its own kernel */
+    CN_OPT_BY_COLS = 14,    /* systems per strip of the interleaved-layout kernel of cn_batched_sweep: 0 = auto, 8 = strips
+                               128 B wide, 4 = strips 64 B wide (systems of >= 128 rows): twice the rows per CTA, so
+                               half the CTAs per cluster for systems of 2048 rows and more */
     CN_OPT_KEEP_P = 13      /* 0 (default) = unless the caller's blocks already have 8 * 2^k <= 256 rows, the tiled path
                                partitions the system itself: blocks of the largest 8 * 2^k <= 256 rows that divides N
                                (cn_plan_info.P_effective; psi does not depend on the partition);

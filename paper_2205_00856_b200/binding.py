@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(PKG, "libcn_nshape.so")
 CN_OK, CN_EINVAL, CN_ENOMEM, CN_ECUDA, CN_ENOTFACTORIZED, CN_EBREAKDOWN, CN_ETOOLARGE = range(7)
 CN_STATIC_NMAX = 4096
 CN_OPT_PATH, CN_OPT_TILE_THREADS, CN_OPT_RS_TOPMAX, CN_OPT_RS_LEVELS, CN_OPT_PROFILE, CN_OPT_PDL, CN_OPT_ONCHIP = 1, 2, 3, 5, 6, 7, 8
-CN_OPT_RS_GROUP, CN_OPT_RS_SERIAL_TOP, CN_OPT_RS_TOP_IN_SUBST, CN_OPT_KEEP_P = 10, 11, 12, 13
+CN_OPT_RS_GROUP, CN_OPT_RS_SERIAL_TOP, CN_OPT_RS_TOP_IN_SUBST, CN_OPT_KEEP_P, CN_OPT_BY_COLS = 10, 11, 12, 13, 14
 PATH_AUTO, PATH_GENERIC, PATH_TILED, PATH_ONCHIP = 0, 1, 2, 3
 
 EXPORTS = ["cn_plan_create", "cn_plan_set_device_budget", "cn_plan_set_option", "cn_factorize", "cn_step",
@@ -365,7 +365,8 @@ class Plan:
             cn_plan_set_option(self.h, {"rs_topmax": CN_OPT_RS_TOPMAX,
                                         "rs_levels": CN_OPT_RS_LEVELS, "profile": CN_OPT_PROFILE,
                                         "pdl": CN_OPT_PDL, "onchip": CN_OPT_ONCHIP, "rs_group": CN_OPT_RS_GROUP,
-                                        "rs_serial_top": CN_OPT_RS_SERIAL_TOP, "rs_top_in_subst": CN_OPT_RS_TOP_IN_SUBST, "keep_p": CN_OPT_KEEP_P}[k], v)
+                                        "rs_serial_top": CN_OPT_RS_SERIAL_TOP, "rs_top_in_subst": CN_OPT_RS_TOP_IN_SUBST, "keep_p": CN_OPT_KEEP_P,
+                                        "by_cols": CN_OPT_BY_COLS}[k], v)
 
     def factorize(self, stream=None):
         cn_factorize(self.h, stream)

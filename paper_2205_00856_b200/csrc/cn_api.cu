@@ -65,7 +65,7 @@ struct cn_plan {
     int64_t noff0 = 0;       // number of such groups
     // configuration
     int opt_path = 0, opt_tile_threads = 0, opt_rs_topmax = 4096, opt_rs_levels = 0, opt_profile = 0, opt_onchip = 1;
-    int opt_pdl = 1, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0, opt_rs_top_in_subst = 1, opt_keep_p = 0;
+    int opt_pdl = 1, opt_rs_group = CN_RS_G, opt_rs_serial_top = 0, opt_rs_top_in_subst = 1, opt_keep_p = 0, opt_by_cols = 0;
     int64_t opt_rs_top_in_subst_max = 256; // measured at C2: faster up to 256 rows (160.8 vs 163.0 us), slower from 512 on
     // time-dependent H (cn_step_td): spatial shape g of the driving term, the potential of the current step and the
     // temporaries of the factorization kept alive so that cn_step_td never allocates
@@ -315,6 +315,11 @@ extern "C" cn_status cn_plan_set_option(cn_plan *plan, cn_option key, int64_t va
     case CN_OPT_KEEP_P:
         plan->opt_keep_p = value ? 1 : 0;
         plan->factorized = false;
+        return CN_OK;
+    case CN_OPT_BY_COLS:
+        if (value != 0 && value != 4 && value != 8) return CN_EINVAL;
+        plan->opt_by_cols = (int)value;
+        plan->tmBatchFor = nullptr;
         return CN_OK;
     case CN_OPT_RS_LEVELS:
         if (value < -1 || value > 8) return CN_EINVAL;
@@ -1446,6 +1451,7 @@ extern "C" cn_status cn_tridiag_solve(cn_tridiag *t, const void *d, void *x, voi
 // ---- batched sweep (config C4) --------------------------------------------------------------------------
 typedef void (*bx_kernel_t)(const CUtensorMap, const cn_bx_params);
 typedef void (*by_kernel_t)(const CUtensorMap, const cn_by_params);
+#define CN_BY_COLS4_FROM_LOG2N 99 // auto: strips of 4 columns for systems of at least 2^this rows
 
 static bx_kernel_t bx_kernel(int logc, int cl)
 {
@@ -1467,27 +1473,43 @@ static bx_kernel_t bx_kernel(int logc, int cl)
     return nullptr;
 }
 
-static by_kernel_t by_kernel(int logg, int cl, size_t *smem)
+static by_kernel_t by_kernel(int logg, int cl, int nc, size_t *smem)
 {
-#define CN_BY(L, C)                          \
-    {                                        \
-        *smem = batched_y_smem_bytes<L>();   \
-        return k_batched_y<L, C>;            \
+#define CN_BY(L, C, NC)                          \
+    {                                            \
+        *smem = batched_y_smem_bytes<L, NC>();   \
+        return k_batched_y<L, C, NC>;            \
+    }
+    if (nc == 4) { // strips of 4 columns: up to 2048 rows per CTA
+        if (cl == 1) {
+            switch (logg) {
+            case 3: CN_BY(3, 1, 4)
+            case 4: CN_BY(4, 1, 4)
+            case 5: CN_BY(5, 1, 4)
+            case 6: CN_BY(6, 1, 4)
+            case 7: CN_BY(7, 1, 4)
+            }
+            return nullptr;
+        }
+        if (logg != 7) return nullptr;
+        if (cl == 2) CN_BY(7, 2, 4)
+        if (cl == 4) CN_BY(7, 4, 4)
+        return nullptr;
     }
     if (cl == 1) {
         switch (logg) {
-        case 2: CN_BY(2, 1)
-        case 3: CN_BY(3, 1)
-        case 4: CN_BY(4, 1)
-        case 5: CN_BY(5, 1)
-        case 6: CN_BY(6, 1)
+        case 2: CN_BY(2, 1, 8)
+        case 3: CN_BY(3, 1, 8)
+        case 4: CN_BY(4, 1, 8)
+        case 5: CN_BY(5, 1, 8)
+        case 6: CN_BY(6, 1, 8)
         }
         return nullptr;
     }
     if (logg != 6) return nullptr;
-    if (cl == 2) CN_BY(6, 2)
-    if (cl == 4) CN_BY(6, 4)
-    if (cl == 8) CN_BY(6, 8)
+    if (cl == 2) CN_BY(6, 2, 8)
+    if (cl == 4) CN_BY(6, 4, 8)
+    if (cl == 8) CN_BY(6, 8, 8)
 #undef CN_BY
     return nullptr;
 }
@@ -1576,6 +1598,8 @@ extern "C" cn_status cn_batched_sweep(cn_plan *p, void *psi_, int64_t nsys, int6
     if ((N & (N - 1)) == 0)
         for (lg = 0; (1LL << lg) < N; ++lg) {}
     int path = 0, logp = 0, cl = 1; // 0 generic, 1 x, 2 y
+    // columns per strip of the y kernel: 4 from 2048 rows on (half the CTAs per cluster), else 8
+    const int nc = (lg >= 7 && (p->opt_by_cols == 4 || (p->opt_by_cols == 0 && lg >= CN_BY_COLS4_FROM_LOG2N))) ? 4 : 8;
     if (p->opt_path != 1 && lg >= 6 && lg <= 14 && nsys < (1LL << 31) && ss < (1LL << 36) && es < (1LL << 36)) {
         if (xs && lg <= 14) {
             path = 1;
@@ -1585,11 +1609,12 @@ extern "C" cn_status cn_batched_sweep(cn_plan *p, void *psi_, int64_t nsys, int6
                 logp = 8;
             }
         } else if (ys && lg <= 13 && nsys >= 8) {
+            const int cap = (nc == 4) ? 7 : 6; // row groups of 16 rows per CTA: 512 threads
             path = 2;
             logp = lg - 4;
-            if (logp > 6) {
-                cl = 1 << (logp - 6);
-                logp = 6;
+            if (logp > cap) {
+                cl = 1 << (logp - cap);
+                logp = cap;
             }
         }
     }
@@ -1623,20 +1648,20 @@ extern "C" cn_status cn_batched_sweep(cn_plan *p, void *psi_, int64_t nsys, int6
         }
     } else if (path == 2) {
         size_t smem = 0;
-        by_kernel_t k = by_kernel(logp, cl, &smem);
+        by_kernel_t k = by_kernel(logp, cl, nc, &smem);
         if (!k) return CN_EINVAL;
-        const int tpb = 8 << logp, rc = 16 << logp;
+        const int tpb = nc << logp, rc = 16 << logp;
         if (fresh) {
             if ((st = get_encoder(p)) != CN_OK) return st;
             cuuint64_t dims[2] = {(cuuint64_t)(2 * nsys), (cuuint64_t)N};
             cuuint64_t strides[1] = {(cuuint64_t)es * 16};
-            cuuint32_t box[2] = {16, (cuuint32_t)(rc < 256 ? rc : 256)};
+            cuuint32_t box[2] = {(cuuint32_t)(2 * nc), (cuuint32_t)(rc < 256 ? rc : 256)};
             cuuint32_t estr[2] = {1, 1};
             CUresult r = p->encode(&p->tmBatch, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, psi_, dims, strides, box, estr,
                                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) return cuda_fail(p, cudaErrorInvalidValue);
-            if ((st = persistent_grid(p, k, tpb, smem, cl, (nsys + 7) / 8, &p->batchGrid)) != CN_OK) return st;
+            if ((st = persistent_grid(p, k, tpb, smem, cl, (nsys + nc - 1) / nc, &p->batchGrid)) != CN_OK) return st;
         }
         cn_by_params prm{nsys, es, p->rho, psi, p->qB, p->gam};
         for (int64_t s = 0; s < nsteps && e == cudaSuccess; ++s) {

@@ -370,65 +370,82 @@ struct cn_by_params {
     const double *gam;
 };
 
-// padded index of the per-row constants in shared memory: one pad slot per 16 rows, so that the four row
+// padded index of the per-row constants in shared memory: one pad slot per 16 rows, so that the row
 // groups of a warp (16 rows apart) broadcast from different banks
 CN_DEVINL int by_pad(int l) { return l + (l >> 4); }
 
-template <int LOGG>
+// NC = columns (systems) of a strip: 8 (128 B per row) or 4 (64 B per row: twice the rows per CTA at the same tile size,
+// so half the CTAs per cluster for a long system).  GPW = 32 / NC row groups per warp.
+template <int LOGG, int NC>
 struct by_layout {
-    static constexpr int G = 1 << LOGG, RC = 16 * G, NW = (G / 4 > 0) ? G / 4 : 1;
-    static constexpr size_t off_q = (size_t)RC * 128;                         // after psi [RC rows][8 columns]
-    static constexpr size_t n_q = RC + RC / 16 + 2;                           // logical index row + 1, padded
+    static constexpr int G = 1 << LOGG, RC = 16 * G, GPW = 32 / NC, NW = (G / GPW > 0) ? G / GPW : 1;
+    static constexpr int L1 = (NC == 8) ? 2 : 3;                               // log2(GPW)
+    static constexpr size_t off_q = (size_t)RC * NC * 16;                      // after psi [RC rows][NC columns]
+    static constexpr size_t n_q = RC + RC / 16 + 2;                            // logical index row + 1, padded
     static constexpr size_t off_g = off_q + n_q * 16;
     static constexpr size_t n_g = (RC + RC / 16 + 2) & ~(size_t)1;
-    static constexpr size_t off_agg = off_g + n_g * 8;                        // [2 dirs][A[NW], B[NW][8]]
-    static constexpr size_t off_mail = off_agg + (size_t)2 * (NW + NW * 8) * 16; // [2 dirs][8 ranks][A, B[8]]
-    static constexpr size_t off_bar = off_mail + (size_t)2 * 8 * 9 * 16;
+    static constexpr size_t off_M1 = off_g + n_g * 8;                          // [2 dirs][L1][G]   level-1 multipliers
+    static constexpr size_t off_Ae = off_M1 + (size_t)2 * L1 * G * 16;         // [2][G]     inclusive A of the group before
+    static constexpr size_t off_aggA = off_Ae + (size_t)2 * G * 16;            // [2][NW]    A aggregate of every warp
+    static constexpr size_t off_cA = off_aggA + (size_t)2 * NW * 16;           // [2][NW]    A of the warps before a warp
+    static constexpr size_t off_rM = off_cA + (size_t)2 * NW * 16;             // [2][L1][GPW] multipliers over the roles
+    static constexpr size_t off_aggB = off_rM + (size_t)2 * L1 * GPW * 16;     // [2][NW][NC] per-strip B aggregates
+    static constexpr size_t off_mailA = off_aggB + (size_t)2 * NW * NC * 16;   // [2][8 ranks]
+    static constexpr size_t off_mailB = off_mailA + (size_t)2 * 8 * 16;        // [2][8 ranks][NC]
+    static constexpr size_t off_bar = off_mailB + (size_t)2 * 8 * NC * 16;
     static constexpr size_t bytes = off_bar + 32; // [0] TMA loads, [1] downward mailbox, [2] upward mailbox
 };
-template <int LOGG>
+template <int LOGG, int NC>
 constexpr size_t batched_y_smem_bytes()
 {
-    return by_layout<LOGG>::bytes;
+    return by_layout<LOGG, NC>::bytes;
 }
 
-// Thread (g, c): rows 16 g .. 16 g + 15 of this CTA's part of column c of the strip.  lane = c + 8 (g & 3),
-// warp = g >> 2.  G = 2^LOGG row groups per CTA, TPB = 8 G threads, CL CTAs per system (CL > 1 needs LOGG == 6).
-template <int LOGG, int CL>
-__global__ void __launch_bounds__(8 << LOGG, 1)
+// Thread (g, c): rows 16 g .. 16 g + 15 of this CTA's part of column c of the strip.  lane = c + NC gl,
+// g = GPW warp + gl.  G = 2^LOGG row groups per CTA, TPB = NC G threads, CL CTAs per system (CL > 1 needs TPB = 512).
+// As in k_batched_x the A side of every scan is computed once per kernel (the matrix is shared by all systems); the
+// multipliers of a thread depend on its row group alone, so they are stored per group and broadcast to its NC lanes.
+template <int LOGG, int CL, int NC>
+__global__ void __launch_bounds__(NC << LOGG, 1) // (two CTAs of 256 threads at 128 registers: slower, measured)
 k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
 {
-    constexpr int G = 1 << LOGG, TPB = 8 * G, RC = 16 * G;
-    constexpr int NW = (G / 4 > 0) ? G / 4 : 1;
-    constexpr int KW = (NW + 3) / 4; // warps covered by one lane role in the cross-warp scan
+    typedef by_layout<LOGG, NC> LY;
+    constexpr int G = LY::G, TPB = NC * G, RC = LY::RC, GPW = LY::GPW, NW = LY::NW, L1 = LY::L1;
+    constexpr int KW = (NW + GPW - 1) / GPW; // warps covered by one lane role in the cross-warp scan
     constexpr int BOXR = RC < 256 ? RC : 256;
-    static_assert(LOGG >= 2 && LOGG <= 6, "32..512 threads");
-    static_assert(CL == 1 || LOGG == 6, "a cluster chains whole CTAs");
+    static_assert(NC == 8 || NC == 4, "columns per strip");
+    static_assert(G >= GPW && TPB <= 512, "32..512 threads");
+    static_assert(CL == 1 || TPB == 512, "a cluster chains whole CTAs");
 
-    typedef by_layout<LOGG> LY;
     extern __shared__ __align__(1024) uint8_t smem[];
     cplx *const s_psi = (cplx *)smem;
     cplx *const s_q = (cplx *)(smem + LY::off_q);
     double *const s_g = (double *)(smem + LY::off_g);
-    cplx *const s_agg = (cplx *)(smem + LY::off_agg);
-    cplx *const s_mail = (cplx *)(smem + LY::off_mail);
+    cplx *const s_M1 = (cplx *)(smem + LY::off_M1);
+    cplx *const s_Ae = (cplx *)(smem + LY::off_Ae);
+    cplx *const s_aggA = (cplx *)(smem + LY::off_aggA);
+    cplx *const s_cA = (cplx *)(smem + LY::off_cA);
+    cplx *const s_rM = (cplx *)(smem + LY::off_rM);
+    cplx *const s_aggB = (cplx *)(smem + LY::off_aggB);
+    cplx *const s_mailA = (cplx *)(smem + LY::off_mailA);
+    cplx *const s_mailB = (cplx *)(smem + LY::off_mailB);
     uint64_t *const bar = (uint64_t *)(smem + LY::off_bar);
 
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    const int c = lane & 7, gl = lane >> 3, g = 4 * warp + gl;
+    const int c = lane & (NC - 1), gl = lane / NC, g = GPW * warp + gl;
     const uint32_t rank = (CL > 1) ? cluster_ctarank() : 0u;
     const int64_t cid = blockIdx.x / CL, ncl = gridDim.x / CL;
-    const int64_t nstrips = (prm.nsys + 7) / 8;
+    const int64_t nstrips = (prm.nsys + NC - 1) / NC;
     const int64_t grow0 = (int64_t)rank * RC + 16 * g; // first row of this thread inside its system
     const bool sysFirst = (rank == 0 && g == 0), sysLast = (rank == CL - 1 && g == G - 1);
     const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
     const double rho = prm.rho;
 
     auto issue_load = [&](int64_t strip) {
-        mbar_expect_tx(bar, (uint32_t)(RC * 128));
+        mbar_expect_tx(bar, (uint32_t)(RC * NC * 16));
 #pragma unroll
         for (int r = 0; r < RC; r += BOXR)
-            tma_load_2d((uint8_t *)s_psi + (size_t)r * 128, &tmPsi, bar, (int)(strip * 16), (int)(rank * RC + r));
+            tma_load_2d((uint8_t *)s_psi + (size_t)r * NC * 16, &tmPsi, bar, (int)(strip * 2 * NC), (int)(rank * RC + r));
     };
 
     // ---- constants of the shared matrix for this CTA's rows: shared memory, loaded once ---------------
@@ -443,152 +460,180 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
         mbar_init(bar + 2, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    pdl_wait();
-    pdl_launch_dependents();
-    if (t == 0 && cid < nstrips) issue_load(cid);
-    if (CL > 1) {
+    if (CL > 1) { // every CTA of the cluster is resident before anything is stored into its shared memory
         cluster_arrive();
         cluster_wait();
     } else {
         __syncthreads();
     }
-    // chunk multipliers (constant): fwdA = prod_{j<16} (-q_{row0+j-1}), bwdA = prod_{j<16} (-q_{row0+j})
-    cplx fwdA, bwdA;
+
+    // chain positions: roles of the cross-warp scan (role r composes chain positions [r KW, r KW + KW))
+    const int posF = warp, posB = NW - 1 - warp; // chain position of this warp, downward / upward
+    // ---- the A side of every scan, once ---------------------------------------------------------
     {
         cplx pm = one; // prod_{j=0..14} (-q_{row0+j})
 #pragma unroll
         for (int j = 0; j < 15; ++j) pm = cmul(pm, cneg(s_q[by_pad(16 * g + j + 1)]));
-        fwdA = sysFirst ? zero : cmul(cneg(s_q[by_pad(16 * g)]), pm);
-        bwdA = sysLast ? zero : cmul(pm, cneg(s_q[by_pad(16 * g + 16)]));
-    }
-
-    // exclusive map (Aex, Bex) of the row groups of this CTA before (DIR > 0) / after (DIR < 0) this thread in
-    // its column, and the aggregate of the whole CTA for this column
-    auto scan_cta = [&](auto dirtag, cplx A, cplx B, cplx &Aex, cplx &Bex, cplx &aggA, cplx &aggB) {
-        constexpr int DIR = decltype(dirtag)::value;
-        // level 1: the four row groups of a warp (lanes 8 apart)
+        const cplx chunkA[2] = {sysFirst ? zero : cmul(cneg(s_q[by_pad(16 * g)]), pm),
+                                sysLast ? zero : cmul(pm, cneg(s_q[by_pad(16 * g + 16)]))};
 #pragma unroll
-        for (int d = 8; d < 32; d <<= 1) {
-            cplx As = (DIR > 0) ? shfl_up_c(A, d) : shfl_down_c(A, d);
-            cplx Bs = (DIR > 0) ? shfl_up_c(B, d) : shfl_down_c(B, d);
-            const bool ok = (DIR > 0) ? (lane >= d) : (lane + d < 32);
-            if (ok) {
-                B = cfma(A, Bs, B);
-                A = cmul(A, As);
+        for (int di = 0; di < 2; ++di) { // 0: downward (to higher rows), 1: upward
+            cplx A = chunkA[di];
+#pragma unroll
+            for (int k = 0; k < L1; ++k) { // level 1: the row groups of a warp (lanes NC apart)
+                const int d = NC << k;
+                const bool ok = (di == 0) ? (lane >= d) : (lane + d < 32);
+                if (c == 0) s_M1[(di * L1 + k) * G + g] = ok ? A : zero;
+                const cplx As = (di == 0) ? shfl_up_c(A, d) : shfl_down_c(A, d);
+                if (ok) A = cmul(A, As);
+            }
+            {
+                const cplx Ae = (di == 0) ? shfl_up_c(A, NC) : shfl_down_c(A, NC);
+                if (c == 0) s_Ae[di * G + g] = Ae;
+            }
+            const int lastRoleLane = c + NC * ((di == 0) ? GPW - 1 : 0);
+            cplx aggA = shfl_c(A, lastRoleLane), cA = one;
+            if (NW > 1) { // level 2: warps.  chain position of warp w: w (downward) or NW-1-w (upward)
+                if (lane == lastRoleLane && c == 0) s_aggA[di * NW + warp] = A;
+                __syncthreads();
+                const int role = (di == 0) ? gl : GPW - 1 - gl;
+                cplx a = one;
+#pragma unroll
+                for (int i = 0; i < KW; ++i) {
+                    const int p = role * KW + i;
+                    if (p < NW) a = cmul(s_aggA[di * NW + ((di == 0) ? p : NW - 1 - p)], a);
+                }
+#pragma unroll
+                for (int k = 0; k < L1; ++k) { // inclusive over roles
+                    const int d = NC << k;
+                    const bool ok = (di == 0) ? (lane >= d) : (lane + d < 32);
+                    if (warp == 0 && c == 0) s_rM[(di * L1 + k) * GPW + gl] = ok ? a : zero;
+                    const cplx as = (di == 0) ? shfl_up_c(a, d) : shfl_down_c(a, d);
+                    if (ok) a = cmul(a, as);
+                }
+                aggA = shfl_c(a, lastRoleLane);
+                // exclusive over roles, then the warps of the own role before the own warp
+                const int mypos = (di == 0) ? posF : posB, grole = mypos / KW, irole = mypos % KW;
+                cplx ea = (di == 0) ? shfl_up_c(a, NC) : shfl_down_c(a, NC);
+                if (role == 0) ea = one;
+                cA = shfl_c(ea, c + NC * ((di == 0) ? grole : GPW - 1 - grole));
+#pragma unroll
+                for (int i = 0; i < KW - 1; ++i) {
+                    if (i < irole) {
+                        const int p = grole * KW + i;
+                        cA = cmul(s_aggA[di * NW + ((di == 0) ? p : NW - 1 - p)], cA);
+                    }
+                }
+                if (lane == 0) s_cA[di * NW + warp] = cA;
+            }
+            if (CL > 1 && warp == 0 && c == 0) { // the aggregate of this CTA to the CTAs that chain after it
+#pragma unroll
+                for (int k = 0; k < (8 + GPW - 1) / GPW; ++k) {
+                    const uint32_t dst = (uint32_t)gl + GPW * k;
+                    const bool wants = dst < (uint32_t)CL && ((di == 0) ? (dst > rank) : (dst < rank));
+                    if (wants) dsmem_store(s_mailA + di * 8 + rank, dst, aggA);
+                }
             }
         }
-        cplx cA = one, cB = zero; // composite of the warps before this warp in chain order
-        aggA = A;
-        aggB = B;
+    }
+    pdl_wait();
+    pdl_launch_dependents();
+    if (t == 0 && cid < nstrips) issue_load(cid);
+    if (CL > 1) { // the A aggregates have arrived everywhere
+        cluster_arrive();
+        cluster_wait();
+    } else {
+        __syncthreads();
+    }
+
+    // value entering this thread's 16 rows from the rows before them in direction DIR, for its column (B: what leaves
+    // the 16 rows when nothing enters them); level 3 as in k_batched_x: asynchronous DSMEM stores that signal the
+    // receiver's mbarrier (16 NC bytes per sender: the per-column B)
+    uint32_t xphase = 0;
+    auto inflow = [&](auto dirtag, cplx B) -> cplx {
+        constexpr int DIR = decltype(dirtag)::value;
+        constexpr int di = DIR > 0 ? 0 : 1;
+#pragma unroll
+        for (int k = 0; k < L1; ++k) {
+            const cplx Bs = (DIR > 0) ? shfl_up_c(B, NC << k) : shfl_down_c(B, NC << k);
+            B = cfma(s_M1[(di * L1 + k) * G + g], Bs, B);
+        }
+        const int lastRoleLane = c + NC * ((DIR > 0) ? GPW - 1 : 0);
+        cplx cB = zero, aggB;
         if (NW > 1) {
-            // level 2: warps.  chain position of warp w: w (DIR > 0) or NW-1-w (DIR < 0)
-            cplx *sA = s_agg + (DIR > 0 ? 0 : (NW + NW * 8)), *sB = sA + NW;
-            if (gl == (DIR > 0 ? 3 : 0)) {
-                if (c == 0) sA[warp] = A;
-                sB[warp * 8 + c] = B;
-            }
+            cplx *const sB = s_aggB + di * NW * NC;
+            const cplx *const sA = s_aggA + di * NW;
+            if (gl == (DIR > 0 ? GPW - 1 : 0)) sB[warp * NC + c] = B;
             __syncthreads();
-            const int role = (DIR > 0) ? gl : 3 - gl;    // this lane composes chain positions [role KW, role KW + KW)
-            cplx a = one, b = zero;
+            const int role = (DIR > 0) ? gl : GPW - 1 - gl;
+            cplx b = zero;
 #pragma unroll
             for (int i = 0; i < KW; ++i) {
                 const int p = role * KW + i;
                 if (p < NW) {
                     const int w = (DIR > 0) ? p : NW - 1 - p;
-                    const cplx Au = sA[w], Bu = sB[w * 8 + c];
-                    b = cfma(Au, b, Bu);
-                    a = cmul(Au, a);
+                    b = cfma(sA[w], b, sB[w * NC + c]);
                 }
             }
 #pragma unroll
-            for (int d = 8; d < 32; d <<= 1) { // inclusive over roles
-                cplx as = (DIR > 0) ? shfl_up_c(a, d) : shfl_down_c(a, d);
-                cplx bs = (DIR > 0) ? shfl_up_c(b, d) : shfl_down_c(b, d);
-                const bool ok = (DIR > 0) ? (lane >= d) : (lane + d < 32);
-                if (ok) {
-                    b = cfma(a, bs, b);
-                    a = cmul(a, as);
-                }
+            for (int k = 0; k < L1; ++k) { // inclusive over roles
+                const cplx bs = (DIR > 0) ? shfl_up_c(b, NC << k) : shfl_down_c(b, NC << k);
+                b = cfma(s_rM[(di * L1 + k) * GPW + gl], bs, b);
             }
-            const int lastRoleLane = c + 8 * ((DIR > 0) ? 3 : 0);
-            aggA = shfl_c(a, lastRoleLane);
             aggB = shfl_c(b, lastRoleLane);
-            // exclusive over roles, then the warps of the own role before the own warp
-            const int mypos = (DIR > 0) ? warp : NW - 1 - warp;
-            const int grole = mypos / KW, irole = mypos % KW;
-            cplx ea = (DIR > 0) ? shfl_up_c(a, 8) : shfl_down_c(a, 8);
-            cplx eb = (DIR > 0) ? shfl_up_c(b, 8) : shfl_down_c(b, 8);
-            if (role == 0) {
-                ea = one;
-                eb = zero;
-            }
-            const int srcLane = c + 8 * ((DIR > 0) ? grole : 3 - grole);
-            cA = shfl_c(ea, srcLane);
-            cB = shfl_c(eb, srcLane);
+            const int mypos = (DIR > 0) ? posF : posB, grole = mypos / KW, irole = mypos % KW;
+            cplx eb = (DIR > 0) ? shfl_up_c(b, NC) : shfl_down_c(b, NC);
+            if (role == 0) eb = zero;
+            cB = shfl_c(eb, c + NC * ((DIR > 0) ? grole : GPW - 1 - grole));
 #pragma unroll
             for (int i = 0; i < KW - 1; ++i) {
                 if (i < irole) {
                     const int p = grole * KW + i;
                     const int w = (DIR > 0) ? p : NW - 1 - p;
-                    const cplx Au = sA[w], Bu = sB[w * 8 + c];
-                    cB = cfma(Au, cB, Bu);
-                    cA = cmul(Au, cA);
+                    cB = cfma(sA[w], cB, sB[w * NC + c]);
                 }
             }
         } else {
-            const int lastLane = c + 8 * ((DIR > 0) ? 3 : 0);
-            aggA = shfl_c(A, lastLane);
-            aggB = shfl_c(B, lastLane);
+            aggB = shfl_c(B, lastRoleLane);
         }
-        cplx Ae = (DIR > 0) ? shfl_up_c(A, 8) : shfl_down_c(A, 8);
-        cplx Be = (DIR > 0) ? shfl_up_c(B, 8) : shfl_down_c(B, 8);
-        const bool first = (DIR > 0) ? (gl == 0) : (gl == 3);
-        Aex = first ? cA : cmul(Ae, cA);
-        Bex = first ? cB : cfma(Ae, cB, Be);
-    };
-
-    // level 3 as in k_batched_x: asynchronous DSMEM stores that signal the receiver's mbarrier (144 bytes per sender:
-    // A and the 8 per-column B)
-    uint32_t xphase = 0;
-    auto cluster_inflow = [&](auto dirtag, cplx aggA, cplx aggB) -> cplx {
-        constexpr int DIR = decltype(dirtag)::value;
-        if (CL == 1) return zero;
-        cplx *m = s_mail + (DIR > 0 ? 0 : 8 * 9); // [rank][A, B[8]]
-        uint64_t *mb = bar + (DIR > 0 ? 1 : 2);
-        if (warp == 0) {
-            // lane (c, gl): destination ranks gl, gl + 4
+        if (CL > 1) {
+            const cplx *mA = s_mailA + di * 8;
+            cplx *mB = s_mailB + di * 8 * NC;
+            uint64_t *mb = bar + 1 + di;
+            if (warp == 0) { // lane (c, gl): destination ranks gl, gl + GPW
 #pragma unroll
-            for (int k = 0; k < 2; ++k) {
-                const uint32_t dst = (uint32_t)gl + 4 * k;
-                const bool wants = dst < (uint32_t)CL && ((DIR > 0) ? (dst > rank) : (dst < rank));
-                if (wants) {
-                    if (c == 0) dsmem_store_signal(m + rank * 9, mb, dst, aggA);
-                    dsmem_store_signal(m + rank * 9 + 1 + c, mb, dst, aggB);
+                for (int k = 0; k < (8 + GPW - 1) / GPW; ++k) {
+                    const uint32_t dst = (uint32_t)gl + GPW * k;
+                    const bool wants = dst < (uint32_t)CL && ((DIR > 0) ? (dst > rank) : (dst < rank));
+                    if (wants) dsmem_store_signal(mB + rank * NC + c, mb, dst, aggB);
                 }
             }
+            const int nsend = (DIR > 0) ? (int)rank : CL - 1 - (int)rank;
+            if (nsend > 0) mbar_wait(mb, xphase);
+            cplx cin = zero;
+            if (DIR > 0) {
+                for (int u = 0; u < (int)rank; ++u) cin = cfma(mA[u], cin, mB[u * NC + c]);
+            } else {
+                for (int u = CL - 1; u > (int)rank; --u) cin = cfma(mA[u], cin, mB[u * NC + c]);
+            }
+            cB = (NW > 1) ? cfma(s_cA[di * NW + warp], cin, cB) : cin;
         }
-        const int nsend = (DIR > 0) ? (int)rank : CL - 1 - (int)rank;
-        if (nsend > 0) mbar_wait(mb, xphase);
-        cplx in = zero;
-        if (DIR > 0) {
-            for (int u = 0; u < (int)rank; ++u) in = cfma(m[u * 9], in, m[u * 9 + 1 + c]);
-        } else {
-            for (int u = CL - 1; u > (int)rank; --u) in = cfma(m[u * 9], in, m[u * 9 + 1 + c]);
-        }
-        return in;
+        const cplx Be = (DIR > 0) ? shfl_up_c(B, NC) : shfl_down_c(B, NC);
+        const bool first = (DIR > 0) ? (gl == 0) : (gl == GPW - 1);
+        return first ? cB : cfma(s_Ae[di * G + g], cB, Be);
     };
 
     uint32_t phase = 0;
     for (int64_t strip = cid; strip < nstrips; strip += ncl) {
-        const int64_t col = strip * 8 + c;
+        const int64_t col = strip * NC + c;
         const bool colOK = col < prm.nsys;
         cplx *const gcol = prm.psi + col;
         // halo rows at the CTA edges inside a cluster: old psi from global memory (the neighbour CTA stores its
         // new rows only after it has received this CTA's aggregates of this strip)
         cplx vlo = zero, vhi = zero;
         if (CL > 1 && t == 0) { // arm this strip's mailboxes
-            if (rank > 0) mbar_expect_tx(bar + 1, rank * 144u);
-            if (rank < CL - 1) mbar_expect_tx(bar + 2, (CL - 1 - rank) * 144u);
+            if (rank > 0) mbar_expect_tx(bar + 1, rank * (uint32_t)(16 * NC));
+            if (rank < CL - 1) mbar_expect_tx(bar + 2, (CL - 1 - rank) * (uint32_t)(16 * NC));
         }
         if (CL > 1 && colOK) {
             if (g == 0 && rank > 0) vlo = gcol[(grow0 - 1) * prm.pitch];
@@ -598,9 +643,9 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
         phase ^= 1;
         cplx v[16];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) v[j] = s_psi[(16 * g + j) * 8 + c];
-        if (g > 0) vlo = s_psi[(16 * g - 1) * 8 + c];
-        if (g < G - 1) vhi = s_psi[(16 * g + 16) * 8 + c];
+        for (int j = 0; j < 16; ++j) v[j] = s_psi[(16 * g + j) * NC + c];
+        if (g > 0) vlo = s_psi[(16 * g - 1) * NC + c];
+        if (g < G - 1) vhi = s_psi[(16 * g + 16) * NC + c];
         fence_proxy_async(); // generic reads above before the async-proxy refill below (see cn_pass_tiled.cuh)
         __syncthreads();
         if (t == 0 && strip + ncl < nstrips) issue_load(strip + ncl);
@@ -620,10 +665,8 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
         cplx D = zero;
 #pragma unroll
         for (int j = 0; j < 16; ++j) D = cfnma(s_q[by_pad(16 * g + j)], D, v[j]);
-        cplx Aex, Bex, aggA, aggB;
-        scan_cta(std::integral_constant<int, +1>{}, fwdA, D, Aex, Bex, aggA, aggB);
-        cplx cin = cluster_inflow(std::integral_constant<int, +1>{}, aggA, aggB);
-        D = sysFirst ? zero : cfma(Aex, cin, Bex);
+        D = inflow(std::integral_constant<int, +1>{}, D);
+        if (sysFirst) D = zero;
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
             D = cfnma(s_q[by_pad(16 * g + j)], D, v[j]);
@@ -633,9 +676,8 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
         cplx X = zero;
 #pragma unroll
         for (int j = 15; j >= 0; --j) X = cmul(s_q[by_pad(16 * g + j + 1)], csub(v[j], X));
-        scan_cta(std::integral_constant<int, -1>{}, bwdA, X, Aex, Bex, aggA, aggB);
-        cin = cluster_inflow(std::integral_constant<int, -1>{}, aggA, aggB);
-        X = sysLast ? zero : cfma(Aex, cin, Bex);
+        X = inflow(std::integral_constant<int, -1>{}, X);
+        if (sysLast) X = zero;
 #pragma unroll
         for (int j = 15; j >= 0; --j) {
             X = cmul(s_q[by_pad(16 * g + j + 1)], csub(v[j], X));

@@ -85,6 +85,35 @@ def test_y_sweep(N, nsys, pad):
         assert np.all(out[:, nsys:] == 7.0 + 7.0j)
 
 
+@pytest.mark.parametrize("kind,N,nsys,opts", [
+    ("x", 64, 40, {}), ("x", 2048, 5, {}), ("x", 4096, 3, {}), ("x", 8192, 3, {}), ("x", 16384, 2, {}),
+    ("y", 64, 40, {}), ("y", 1024, 11, {}), ("y", 2048, 9, {}), ("y", 8192, 10, {}),
+    # strips of 4 columns (CN_OPT_BY_COLS = 4): in-CTA up to 2048 rows, clusters of 2 / 4 CTAs above
+    ("y", 128, 13, {"by_cols": 4}), ("y", 1024, 6, {"by_cols": 4}), ("y", 2048, 9, {"by_cols": 4}),
+    ("y", 4096, 5, {"by_cols": 4}), ("y", 8192, 7, {"by_cols": 4}),
+])
+def test_sweeps_strong_coupling(kind, N, nsys, opts):
+    """s = dt / (4 dx^2) = 12.5: |q| is close to 1, so the map of a chunk does not decay and the inflow of a chunk
+    carries information from the whole system -- every level of the scans (lanes, warps, CTAs of a cluster) with its
+    multipliers computed once per kernel matters at the 1e-10 bar.  Also the 4-column strips of the y kernel."""
+    torch = torch_()
+    V, psi = rand_batch(N, nsys, 8)
+    dx, dt = 0.01, 0.005
+    for nsteps in (1, 3):
+        ref = oracle_batch(dx, dt, V, psi, nsteps)
+        d = torch.from_numpy(psi.copy() if kind == "x" else np.ascontiguousarray(psi.T)).cuda()
+        with B.Plan(N, 2, dx, dt, V, **opts) as plan:
+            plan.factorize()
+            if kind == "x":
+                plan.batched_sweep(d, nsys, 1, N, nsteps)
+            else:
+                plan.batched_sweep(d, nsys, nsys, 1, nsteps)
+            torch.cuda.synchronize()
+        out = d.cpu().numpy()
+        err = np.max(np.abs((out if kind == "x" else out.T) - ref))
+        assert err <= TOL_PSI, (kind, N, nsys, opts, nsteps, err)
+
+
 @pytest.mark.parametrize("n", [256, 1024, 2048])
 def test_c4_lie_split_scaled(n):
     """Config C4's recipe at n x n: x-sweep then y-sweep per step, one plan per direction, against the oracle."""
