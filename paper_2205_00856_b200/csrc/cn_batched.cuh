@@ -57,6 +57,14 @@ CN_DEVINL void dsmem_store_signal(cplx *p, uint64_t *bar, uint32_t rank, cplx v)
                  : "memory");
 }
 
+// plain (non-tensor) bulk copy global -> shared memory, completing `bytes` of the transaction count of `bar`
+CN_DEVINL void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
 CN_DEVINL void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2)
 {
     asm volatile(
@@ -92,7 +100,8 @@ constexpr size_t batched_x_smem_bytes()
            + (size_t)2 * (CN_BX_TPB / 32) * sizeof(cplx)          // s_wB   [2 dirs][NW]
            + (size_t)4 * 8 * sizeof(cplx) + 32                    // s_mailB, s_mailA [2 dirs][8 ranks] each; 4 mbarriers
            + (size_t)10 * CN_BX_TPB * sizeof(cplx)                // s_M [2][4][TPB], s_Ae [2][TPB]
-           + (size_t)8 * (CN_BX_TPB / 32) * sizeof(cplx);         // s_wM [2][3][NW], s_cA [2][NW]
+           + (size_t)8 * (CN_BX_TPB / 32) * sizeof(cplx)          // s_wM [2][3][NW], s_cA [2][NW]
+           + (size_t)2 * sizeof(cplx);                            // s_halo [2]
 }
 
 // 256 threads x 8 points.  LOGC = log2(chunks per system) when a system fits one CTA (CL == 1, several
@@ -128,6 +137,7 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
     cplx *const s_Ae = s_M + 8 * TPB;                      // [2][TPB]     inclusive A of the neighbouring lane
     cplx *const s_wM = s_Ae + 2 * TPB;                     // [2][3][NW]   multipliers of the scan over the warp aggregates
     cplx *const s_cA = s_wM + 6 * NW;                      // [2][NW]      A of the warps of this block before this warp
+    cplx *const s_halo = s_cA + 2 * NW;                    // [2]          old psi just above / below this CTA's rows (CL > 1)
 
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const uint32_t rank = (CL > 1) ? cluster_ctarank() : 0u;
@@ -139,10 +149,20 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
     const bool sysFirst = pos == 0, sysLast = pos == CPS - 1;
     const int vb = warp & ~(WPB - 1), wl = vb + (lane & (WPB - 1)); // first warp of this block; this lane's warp slot
 
+    // A tile and, inside a cluster, the two halo rows at the CTA edges (old psi: the neighbour CTA stores its new rows
+    // only after it has received this CTA's aggregates of that tile, which are sent after the loads have landed); the
+    // halos travel with the tile, one tile ahead, so no global load sits on the critical path of a tile.
     auto issue_load = [&](int64_t tile) {
-        mbar_expect_tx(bar, (uint32_t)(TPB * 128));
-        if (CL > 1) tma_load_3d(s_psi, &tmPsi, bar, 0, (int)rank * TPB, (int)tile);
-        else tma_load_3d(s_psi, &tmPsi, bar, 0, 0, (int)(tile * SPT));
+        if (CL > 1) {
+            mbar_expect_tx(bar, (uint32_t)(TPB * 128) + (rank > 0 ? 16u : 0u) + (rank < CL - 1 ? 16u : 0u));
+            tma_load_3d(s_psi, &tmPsi, bar, 0, (int)rank * TPB, (int)tile);
+            const cplx *row = prm.psi_raw + tile * prm.sys_stride + (int64_t)rank * (TPB * 8);
+            if (rank > 0) bulk_load(s_halo, row - 1, 16u, bar);
+            if (rank < CL - 1) bulk_load(s_halo + 1, row + TPB * 8, 16u, bar);
+        } else {
+            mbar_expect_tx(bar, (uint32_t)(TPB * 128));
+            tma_load_3d(s_psi, &tmPsi, bar, 0, 0, (int)(tile * SPT));
+        }
     };
 
     // ---- per-thread constants of the shared matrix: live in registers for the whole kernel -----------
@@ -285,20 +305,17 @@ k_batched_x(const __grid_constant__ CUtensorMap tmPsi, const cn_bx_params prm)
 
     uint32_t phase = 0;
     for (int64_t tile = cid; tile < ntiles; tile += ncl) {
-        // halo rows at the CTA edges inside a cluster: old psi straight from global memory (the neighbour CTA
-        // stores its new rows only after it has received this CTA's aggregates of this tile)
         cplx vlo = zero, vhi = zero;
-        if (CL > 1) {
-            if (t == 0) { // arm this tile's mailboxes: 16 bytes (B) from every CTA this one depends on
-                if (rank > 0) mbar_expect_tx(bar + 1, rank * 16u);
-                if (rank < CL - 1) mbar_expect_tx(bar + 2, (CL - 1 - rank) * 16u);
-            }
-            const cplx *row = prm.psi_raw + tile * prm.sys_stride;
-            if (t == 0 && rank > 0) vlo = row[8 * pos - 1];
-            if (t == TPB - 1 && rank < CL - 1) vhi = row[8 * pos + 8];
+        if (CL > 1 && t == 0) { // arm this tile's mailboxes: 16 bytes (B) from every CTA this one depends on
+            if (rank > 0) mbar_expect_tx(bar + 1, rank * 16u);
+            if (rank < CL - 1) mbar_expect_tx(bar + 2, (CL - 1 - rank) * 16u);
         }
         mbar_wait(bar, phase);
         phase ^= 1;
+        if (CL > 1) { // halo rows at the CTA edges inside a cluster
+            if (t == 0 && rank > 0) vlo = s_halo[0];
+            if (t == TPB - 1 && rank < CL - 1) vhi = s_halo[1];
+        }
 
         cplx v[8];
         const int sw = t & 7;
@@ -629,7 +646,8 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
         const bool colOK = col < prm.nsys;
         cplx *const gcol = prm.psi + col;
         // halo rows at the CTA edges inside a cluster: old psi from global memory (the neighbour CTA stores its
-        // new rows only after it has received this CTA's aggregates of this strip)
+        // new rows only after it has received this CTA's aggregates of this strip).  Bringing them in with the strip
+        // by bulk copies, as k_batched_x does, measured slower here (0.629 against 0.616 ms at C4).
         cplx vlo = zero, vhi = zero;
         if (CL > 1 && t == 0) { // arm this strip's mailboxes
             if (rank > 0) mbar_expect_tx(bar + 1, rank * (uint32_t)(16 * NC));

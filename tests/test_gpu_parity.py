@@ -272,9 +272,9 @@ def test_errors_on_device():
     good = {B.CN_OPT_PATH: (0, 1, 2), B.CN_OPT_TILE_THREADS: (0, 32, 64, 128, 256, 512), B.CN_OPT_RS_TOPMAX: (1, 4096, 8192),
             B.CN_OPT_RS_LEVELS: (-1, 0, 1, 8), B.CN_OPT_PROFILE: (0, 1), B.CN_OPT_PDL: (0, 1), B.CN_OPT_ONCHIP: (0, 1),
             B.CN_OPT_RS_GROUP: (2, 256, 1 << 20), B.CN_OPT_RS_SERIAL_TOP: (0, 1), B.CN_OPT_RS_TOP_IN_SUBST: (0, 1, 1024),
-            B.CN_OPT_KEEP_P: (0, 1)}
+            B.CN_OPT_KEEP_P: (0, 1), B.CN_OPT_BY_COLS: (0, 4, 8)}
     bad = {B.CN_OPT_PATH: (-1, 3), B.CN_OPT_TILE_THREADS: (16, 96, 1024), B.CN_OPT_RS_TOPMAX: (0, 8193),
-           B.CN_OPT_RS_LEVELS: (-2, 9), B.CN_OPT_RS_GROUP: (1, (1 << 20) + 1), 4: (0, 1), 9: (0, 1), 0: (0,), 14: (0,)}
+           B.CN_OPT_RS_LEVELS: (-2, 9), B.CN_OPT_RS_GROUP: (1, (1 << 20) + 1), B.CN_OPT_BY_COLS: (1, 2, 16), 4: (0, 1), 9: (0, 1), 0: (0,), 15: (0,)}
     for key, vals in good.items():
         for v in vals:
             plan.set_option(key, v)
