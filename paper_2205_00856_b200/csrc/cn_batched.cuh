@@ -451,14 +451,15 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const int c = lane & (NC - 1), gl = lane / NC, g = GPW * warp + gl;
     const uint32_t rank = (CL > 1) ? cluster_ctarank() : 0u;
-    const int64_t cid = blockIdx.x / CL, ncl = gridDim.x / CL;
-    const int64_t nstrips = (prm.nsys + NC - 1) / NC;
-    const int64_t grow0 = (int64_t)rank * RC + 16 * g; // first row of this thread inside its system
+    const int cid = (int)(blockIdx.x / CL), ncl = (int)(gridDim.x / CL);
+    const int nstrips = (int)((prm.nsys + NC - 1) / NC);
+    const int grow0 = (int)rank * RC + 16 * g; // first row of this thread inside its system
+    cplx *const gthread = prm.psi + c + (int64_t)grow0 * prm.pitch; // row grow0 of column c of strip 0
     const bool sysFirst = (rank == 0 && g == 0), sysLast = (rank == CL - 1 && g == G - 1);
     const cplx zero = cmake(0.0, 0.0), one = cmake(1.0, 0.0);
     const double rho = prm.rho;
 
-    auto issue_load = [&](int64_t strip) {
+    auto issue_load = [&](int strip) {
         mbar_expect_tx(bar, (uint32_t)(RC * NC * 16));
 #pragma unroll
         for (int r = 0; r < RC; r += BOXR)
@@ -566,7 +567,7 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
     // value entering this thread's 16 rows from the rows before them in direction DIR, for its column (B: what leaves
     // the 16 rows when nothing enters them); level 3 as in k_batched_x: asynchronous DSMEM stores that signal the
     // receiver's mbarrier (16 NC bytes per sender: the per-column B)
-    uint32_t xphase = 0;
+    uint32_t par = 0; // parity of the number of strips this CTA has finished: the phase of all three mbarriers
     auto inflow = [&](auto dirtag, cplx B) -> cplx {
         constexpr int DIR = decltype(dirtag)::value;
         constexpr int di = DIR > 0 ? 0 : 1;
@@ -626,7 +627,7 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
                 }
             }
             const int nsend = (DIR > 0) ? (int)rank : CL - 1 - (int)rank;
-            if (nsend > 0) mbar_wait(mb, xphase);
+            if (nsend > 0) mbar_wait(mb, par);
             cplx cin = zero;
             if (DIR > 0) {
                 for (int u = 0; u < (int)rank; ++u) cin = cfma(mA[u], cin, mB[u * NC + c]);
@@ -640,11 +641,12 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
         return first ? cB : cfma(s_Ae[di * G + g], cB, Be);
     };
 
-    uint32_t phase = 0;
-    for (int64_t strip = cid; strip < nstrips; strip += ncl) {
-        const int64_t col = strip * NC + c;
-        const bool colOK = col < prm.nsys;
-        cplx *const gcol = prm.psi + col;
+    const int nit = (cid < nstrips) ? (nstrips - cid + ncl - 1) / ncl : 0; // strips of this cluster
+    for (int it = 0; it < nit;) { // one loop-carried counter: the strip and the mbarrier phase follow from it
+        const int strip = cid + it * ncl;
+        par = (uint32_t)it & 1u;
+        const bool colOK = (int64_t)strip * NC + c < prm.nsys;
+        cplx *const gcol = gthread + (int64_t)strip * NC; // this thread's first row of its column of this strip
         // halo rows at the CTA edges inside a cluster: old psi from global memory (the neighbour CTA stores its
         // new rows only after it has received this CTA's aggregates of this strip).  Bringing them in with the strip
         // by bulk copies, as k_batched_x does, measured slower here (0.629 against 0.616 ms at C4).
@@ -654,11 +656,10 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
             if (rank < CL - 1) mbar_expect_tx(bar + 2, (CL - 1 - rank) * (uint32_t)(16 * NC));
         }
         if (CL > 1 && colOK) {
-            if (g == 0 && rank > 0) vlo = gcol[(grow0 - 1) * prm.pitch];
-            if (g == G - 1 && rank < CL - 1) vhi = gcol[(grow0 + 16) * prm.pitch];
+            if (g == 0 && rank > 0) vlo = gcol[-prm.pitch];
+            if (g == G - 1 && rank < CL - 1) vhi = gcol[16 * prm.pitch];
         }
-        mbar_wait(bar, phase);
-        phase ^= 1;
+        mbar_wait(bar, par);
         cplx v[16];
 #pragma unroll
         for (int j = 0; j < 16; ++j) v[j] = s_psi[(16 * g + j) * NC + c];
@@ -666,7 +667,7 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
         if (g < G - 1) vhi = s_psi[(16 * g + 16) * NC + c];
         fence_proxy_async(); // generic reads above before the async-proxy refill below (see cn_pass_tiled.cuh)
         __syncthreads();
-        if (t == 0 && strip + ncl < nstrips) issue_load(strip + ncl);
+        if (t == 0 && it + 1 < nit) issue_load(strip + ncl);
 
         // ---- Eq. 3 in place: v_j <- E_j ------------------------------------------------------------------
         {
@@ -701,11 +702,16 @@ k_batched_y(const __grid_constant__ CUtensorMap tmPsi, const cn_by_params prm)
             X = cmul(s_q[by_pad(16 * g + j + 1)], csub(v[j], X));
             v[j] = X;
         }
+        // The loop control is decided BEFORE the stores: the register allocator keeps the trip count in local memory,
+        // and a reload issued after the 16 stores of a strip waits behind them in the load/store queue (6 % of the
+        // stall samples of this kernel).
+        int more = (++it < nit);
+        asm volatile("" : "+r"(more));
         if (colOK) {
 #pragma unroll
-            for (int j = 0; j < 16; ++j) gcol[(grow0 + j) * prm.pitch] = v[j];
+            for (int j = 0; j < 16; ++j) gcol[j * prm.pitch] = v[j];
         }
-        xphase ^= 1;
+        if (!more) break;
     }
     if (CL > 1) {
         cluster_arrive();
